@@ -1,0 +1,299 @@
+#!/usr/bin/env python
+"""bench.py — headline benchmark of gcoreccd-b200 (BASELINE.json: "Coulomb pair interactions/s (G/s) vs FP32
+peak; seconds per 131k-hole event").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+
+A "step" is one pass of the whole hot path (field + integrate/collect + compact = SURVEY §8(a) rows a1..a8)
+over the 131,072-hole cloud of BASELINE.json:configs[2].  Prints ONE JSON line (rank 0).
+  value      pair interactions/s over the K timed steps, state resident in HBM, CUDA events on the launching
+             stream, L2 flushed between timed steps (the state is only 2 MB; the path is ALU bound)
+  e2e        same metric through the C ABI with HOST buffers: load_carriers(pinned host) + step(1) +
+             read_carriers(host) per step, copies inside the timed region
+  roofline   field kernel: 20 FLOP x pairs / CUDA-event duration of that kernel, against the FP32 non-tensor
+             peak 148 SM x 128 lanes x 2 x sm_max_mhz
+  cpu_baseline  the FP64 oracle, as it stands, on this box's host cores on a bounded sample of the same workload
+N > 1: replicas only (BASELINE.json north_star: one GPU per event, no sharding): every rank runs its own
+event; value = all ranks' pairs / max-over-ranks device time.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "coulomb_pair_interactions_per_s"
+UNIT = "G pairs/s"
+WORKLOAD_CFG = 2
+FLOP_PER_PAIR = 20.0          # GPU Gems 3 ch. 31 convention (ref [10])
+SM_COUNT, LANES = 148, 128
+
+
+def measured_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return json.load(f), "measured"
+    except Exception:
+        return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.rows, self._stop_evt = index, [], threading.Event()
+
+    def run(self):
+        while not self._stop_evt.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+                for line in out.strip().splitlines():
+                    self.rows.append([t.strip() for t in line.split(",")])
+            except Exception:
+                pass
+            self._stop_evt.wait(0.2)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=6)
+        sm, mx, reasons = [], 0.0, set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx = max(mx, float(r[1]))
+            except Exception:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx or None, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+# ----------------------------------------------------------------------------------------------- oracle legs
+def oracle_sample(xyz, P, seconds_target, rng):
+    """Time the oracle's eq. 6 double loop on m sampled targets x all sources; m sized for ~seconds_target."""
+    from oracle import goracle as g
+    n = len(xyz)
+    Kp = g.coulomb_constant(P["eps_si"])
+    x64 = xyz.astype(np.float64)
+    m = 256
+    t0 = time.perf_counter()
+    g.coulomb_field(x64, eps_um=P["softening_um"], Kp=Kp, targets=np.arange(m, dtype=np.uint64))
+    dt = time.perf_counter() - t0
+    rate = m * n / dt
+    m = int(max(256, seconds_target * rate / n))                     # may exceed n: targets are then revisited
+    tg = np.sort(rng.integers(0, n, size=m)).astype(np.uint64)
+    t0 = time.perf_counter()
+    g.coulomb_field(x64, eps_um=P["softening_um"], Kp=Kp, targets=tg)
+    dt = time.perf_counter() - t0
+    return m * n / dt / 1e9, m, dt, g.num_threads()
+
+
+def run_reference(args):
+    """--impl reference: the FP64 oracle as it stands, on the host cores, same metric/unit/config."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from oracle import goracle as g
+    from paper_2203_11043_b200 import workloads
+    g.build()
+    w = workloads.make(WORKLOAD_CFG)
+    P, xyz = w["params"], w["xyz"]
+    rng = np.random.default_rng(0)
+    per_step_s = 3.0
+    for _ in range(max(args.warmup, 0)):
+        oracle_sample(xyz, P, 0.5, rng)
+    pairs, secs, m_used = 0.0, 0.0, 0
+    for _ in range(args.steps):
+        gps, m, dt, cores = oracle_sample(xyz, P, per_step_s, rng)
+        pairs += m * len(xyz); secs += dt; m_used = m
+    value = pairs / secs / 1e9
+    sample = "eq. 6 double loop (FP64) at %d sampled targets x all %d sources per step" % (m_used, len(xyz))
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 * secs / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "impl": "reference",
+            "config": {"workload": w["name"], "n_holes": len(xyz), "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ----------------------------------------------------------------------------------------------- our arm
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2203_11043_b200 import binding, workloads
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    peaks, peak_src = measured_peaks()
+
+    w = workloads.make(WORKLOAD_CFG, seed=workloads.SEED + rank)       # replicas: one independent event per rank
+    P, xyz = w["params"], w["xyz"]
+    n = len(xyz)
+    stream = torch.cuda.Stream()                                       # the handle, the flush and the events share it
+    torch.cuda.set_stream(stream)
+    sim = binding.from_workload(w, stream=stream)
+    sim.load_carriers(xyz)
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    for _ in range(args.warmup):
+        sim.step(1)
+    barrier()
+    l0 = sim.kernel_launches()
+    p0 = sim.state()["pair_interactions"]
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    for k in range(args.steps):
+        flush.fill_(k & 0xff)                                          # L2 flush between timed iterations (untimed)
+        ev[k][0].record()
+        sim.step(1)
+        ev[k][1].record()
+    barrier()
+    ms = sum(a.elapsed_time(b) for a, b in ev)
+    clocks = sampler.stop() if rank == 0 else None
+    launches = sim.kernel_launches() - l0
+    st = sim.state()
+    pairs = st["pair_interactions"] - p0
+    tms = torch.tensor([ms], dtype=torch.float64, device="cuda")
+    tp = torch.tensor([float(pairs)], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
+        dist.all_reduce(tp, op=dist.ReduceOp.SUM)
+    ms_max, pairs_all = float(tms.item()), float(tp.item())
+    value = pairs_all / (ms_max * 1e-3) / 1e9
+
+    # ---- roofline of the dominant kernel (field), CUDA events inside the library on its launching stream
+    prof = [sim.profile_step() for _ in range(max(3, min(args.steps, 10)))]
+    n_act = sim.state()["n_active"]
+    field_ms = float(np.mean([p["field"] for p in prof]))
+    integ_ms = float(np.mean([p["integrate"] for p in prof]))
+    comp_ms = float(np.mean([p["compact"] for p in prof]))
+    peak_tf = SM_COUNT * LANES * 2.0 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12
+    ach_tf = FLOP_PER_PAIR * float(n_act) ** 2 / (field_ms * 1e-3) / 1e12
+    traffic = None
+    try:
+        with open(os.path.join(ROOT, "profiles", "field_traffic.json")) as f:
+            traffic = json.load(f).get("dram_bytes_per_launch")
+    except Exception:
+        pass
+    roofline = {"bound": "alu", "kernel": "k_field", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
+                "frac": ach_tf / peak_tf, "traffic": traffic, "peak_source": "148 SM x 128 FP32 lanes x 2 x sm_max_mhz (%s)" % peak_src,
+                "flop_per_pair": FLOP_PER_PAIR, "field_ms": field_ms, "n_active": n_act,
+                "other_kernels": {"integrate_ms": integ_ms, "compact_ms": comp_ms,
+                                  "integrate_GBps": 44.0 * n_act / (integ_ms * 1e-3) / 1e9 if integ_ms > 0 else None,
+                                  "compact_GBps": 32.0 * n_act / (comp_ms * 1e-3) / 1e9 if comp_ms > 0 else None,
+                                  "hbm_peak_GBps": peaks.get("hbm_gbs")}}
+
+    # ---- e2e through the C ABI with host buffers (copies inside the timed region)
+    host_in = torch.from_numpy(xyz).pin_memory()
+    host_out = torch.empty((n, 3), dtype=torch.float32).pin_memory()
+    e2e_steps = max(3, min(args.steps, 10))
+    barrier()
+    t0 = time.perf_counter()
+    e2e_pairs = 0
+    for _ in range(e2e_steps):
+        sim.reset()
+        sim.load_carriers_ptr(host_in.data_ptr(), n)
+        sim.step(1)
+        got = sim.read_carriers_into(host_out.data_ptr(), n)
+        e2e_pairs += n * n
+        assert got <= n
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    te = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_value = world * e2e_pairs / float(te.item()) / 1e9
+
+    # ---- seconds per 131k-hole event (second half of BASELINE.json's metric): load -> full collection
+    event = None
+    if not args.no_event:
+        sim.reset()
+        barrier()
+        t0 = time.perf_counter()
+        sim.load_carriers_ptr(host_in.data_ptr(), n)
+        done, left, rc = sim.run_to_collection(10 ** 7)
+        img, over = sim.read_image()
+        torch.cuda.synchronize()
+        ev_s = time.perf_counter() - t0
+        st2 = sim.state()
+        assert left == 0 and int(img.sum()) + over == n, "hole count not conserved"
+        event = {"seconds": ev_s, "steps": done, "pair_interactions": st2["pair_interactions"],
+                 "avg_G_pairs_per_s": st2["pair_interactions"] / ev_s / 1e9, "holes": n, "collected_in_window": int(img.sum())}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- CPU baseline: the oracle as it stands on a bounded sample (rank 0, N = 1 only)
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        from oracle import goracle as g
+        g.build()
+        gps, m, dt, cores = oracle_sample(xyz, P, 12.0, np.random.default_rng(0))
+        cpu = {"value": gps, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": "eq. 6 double loop (FP64) at %d sampled targets x all %d sources, %.1f s" % (m, n, dt)}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": w["name"], "n_holes": n, "parallelism": "replicas only (one event per GPU)",
+                       "l2": "flushed between timed steps (256 MB write); state is 2 MB, path is ALU bound",
+                       "dt_ns": P["dt_ns"], "softening_um": P["softening_um"]},
+            "frac_of_fp32_peak": value * 1e9 * FLOP_PER_PAIR / 1e12 / (peak_tf * world),
+            "clocks": clocks, "gpu_launches": launches,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": n * 12, "d2h_bytes_per_step": n * 12,
+                    "what": "reset + load_carriers(pinned host) + step(1) + read_carriers(host), wall clock"},
+            "roofline": roofline, "cpu_baseline": cpu, "seconds_per_event": event}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-event", action="store_true", help="skip the seconds-per-event run")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,146 @@
+/* gcoreccd.h — C ABI of the B200-native (sm_100a) hot path of G-CoReCCD (arXiv 2203.11043).
+ *
+ * One handle = one event (one set of mutually interacting holes) = one CUDA stream.
+ * Per time step the library runs, entirely on the GPU and in this order (Fig. 2):
+ *   a1  all-pairs softened Coulomb field of every still-drifting hole      (eq. 6)
+ *   a2  + linear depletion field E(z) = a1 z - a2, total |E|               (eq. 1)
+ *   a3  hole mobility mu(|E|, T)                                           (eq. 2)
+ *   a4  drift  dr = mu E dt
+ *   a5  isotropic Gaussian diffusion, sigma^2 = 2 D_h dt, D_h = k_B mu T/q (eqs. 3-4),
+ *       normals from Philox4x32-10 keyed by (seed, carrier id, step)
+ *   a6  position update, specular reflection at the back surface
+ *   a7  collection test z <= z_well and integer pixel histogram
+ *   a8  stable compaction of the carriers still drifting
+ *
+ * Units: length um, time ns, field V/cm, temperature K.  Positions are FP32 ("3N floats").
+ *
+ * Conventions
+ *   - every function returns 0 (GCORECCD_OK) or a negative gcoreccd_status; run_to_collection may return
+ *     +1 (GCORECCD_MAX_STEPS) when max_steps was reached with carriers left ("maximum number
+ *     of iterations"), which is not an error.
+ *   - pointers named *_host are host pointers; pointers with an `on_device` flag are host pointers when
+ *     the flag is 0 and device pointers (on the handle's device) when it is 1.  All output buffers are
+ *     caller-allocated; the library copies inputs and never keeps a caller pointer, except `workspace`.
+ *   - no exceptions, no printing, no global state.  A handle is not thread-safe; distinct handles are
+ *     independent.  There is NO CPU fallback: create() fails with GCORECCD_ERR_CUDA without an sm_100 GPU.
+ *   - gcoreccd_step is asynchronous on the handle's stream; every function that returns data to the host
+ *     synchronises that stream first.
+ */
+#ifndef GCORECCD_H
+#define GCORECCD_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gcoreccd gcoreccd_t;
+
+typedef enum {
+  GCORECCD_OK            = 0,
+  GCORECCD_MAX_STEPS     = 1,
+  GCORECCD_ERR_INVALID   = -1,   /* bad argument / parameter                         */
+  GCORECCD_ERR_STATE     = -2,   /* call not valid in the handle's current state     */
+  GCORECCD_ERR_CAPACITY  = -3,   /* more carriers than max_carriers / buffer too small */
+  GCORECCD_ERR_NOMEM     = -4,
+  GCORECCD_ERR_CUDA      = -5,   /* CUDA runtime error or no sm_100 device           */
+  GCORECCD_ERR_NONFINITE = -6    /* a carrier position became NaN/Inf                */
+} gcoreccd_status;
+
+enum {                            /* gcoreccd_params.flags */
+  GCORECCD_COULOMB_OFF   = 1u,    /* PAPER.md:88 "whether Coulomb repulsion should be computed" */
+  GCORECCD_DIFFUSION_OFF = 2u,    /* test hook: deterministic drift                  */
+  GCORECCD_DEPLETION_OFF = 4u     /* test hook: a1 = a2 = 0                          */
+};
+
+typedef struct {
+  uint32_t struct_size;           /* = sizeof(gcoreccd_params); ABI versioning                            */
+  uint32_t flags;                 /* bits above; 0 = full physics                                          */
+  double   T_K;                   /* > 0, eq. 2 / eq. 4                                                    */
+  double   a1_V_per_cm2;          /* eq. 1, z measured from the front surface (z = 0), z in cm             */
+  double   a2_V_per_cm;           /* eq. 1                                                                 */
+  double   thickness_um;          /* back surface, > z_well_um; carriers are mirrored back at it           */
+  double   z_well_um;             /* collection plane ("depth of the potential well")          */
+  double   pixel_pitch_um;        /* > 0                                                    */
+  double   dt_ns;                 /* > 0                                                                   */
+  double   softening_um;          /* eps of eq. 6, >= 0; 0 evaluates eq. 5 (coincident pairs contribute 0) */
+  double   eps_si;                /* relative permittivity, 0 => 11.7                                      */
+  uint64_t seed;                  /* Philox key                                                            */
+  int32_t  img_nx, img_ny;        /* image window in pixels, each in [1, 16384]                            */
+  double   img_x0_um, img_y0_um;  /* lower-left corner of pixel (0,0)                                      */
+  int32_t  device;                /* CUDA ordinal, -1 = current device                                     */
+  int32_t  reserved0;
+  void*    stream;                /* cudaStream_t to run on (e.g. torch's current stream); NULL => the
+                                     library creates and owns a non-blocking stream                        */
+  void*    workspace;             /* optional caller-owned device memory (e.g. a torch uint8 tensor),
+                                     256-byte aligned, alive until destroy; NULL => the library allocates */
+  uint64_t workspace_bytes;       /* >= gcoreccd_workspace_size(max_carriers, img_nx, img_ny)              */
+  uint64_t max_carriers;          /* capacity, 1 .. 2^26                                                   */
+} gcoreccd_params;
+
+/* Bytes of device memory a handle needs (state ping-pong, field partials, image, counters). */
+uint64_t gcoreccd_workspace_size(uint64_t max_carriers, int32_t img_nx, int32_t img_ny);
+
+/* Create / destroy.  *out is set only on success.  Errors: INVALID (parameter ranges, struct_size),
+ * CUDA (no sm_100 device, runtime failure), NOMEM, CAPACITY (workspace too small). */
+int gcoreccd_create(const gcoreccd_params* p, gcoreccd_t** out);
+int gcoreccd_destroy(gcoreccd_t* h);
+
+/* Drop all carriers, zero image, counters and the step index (parameters are kept). */
+int gcoreccd_reset(gcoreccd_t* h);
+
+/* Append n carriers.  xyz_um: interleaved x,y,z FP32, host (on_device=0) or device (=1)
+ * pointer; copied.  ids continue in load order.  A carrier with z <= z_well is collected at once;
+ * non-finite coordinates or z > thickness => INVALID and nothing is loaded; more than max_carriers in
+ * total => CAPACITY.  Synchronises the stream. */
+int gcoreccd_load_carriers(gcoreccd_t* h, const float* xyz_um, uint64_t n, int on_device);
+
+/* Restart from an exported snapshot (replaces the active set): positions, ids (must be unique) and the step
+ * index the next step will use.  The image and counters are kept.  Host pointers. */
+int gcoreccd_load_snapshot(gcoreccd_t* h, const float* xyz_um_host, const uint32_t* id_host, uint64_t n,
+                           uint64_t step);
+
+/* Enqueue up to n_steps time steps (a1..a8) on the stream; asynchronous.  A step with no active carrier
+ * is a no-op and does not advance the step index. */
+int gcoreccd_step(gcoreccd_t* h, uint32_t n_steps);
+
+/* Step until no carrier is drifting or max_steps more steps were taken; synchronous.
+ * Returns OK, MAX_STEPS (+1), or NONFINITE/CUDA. */
+int gcoreccd_run_to_collection(gcoreccd_t* h, uint64_t max_steps, uint64_t* steps_done, uint64_t* n_active_left);
+
+/* Image, row-major [img_ny][img_nx] counts of collected holes; cap_elems >= nx*ny else CAPACITY.
+ * n_out_of_window (host pointer, may be NULL) receives the holes collected outside the window, so that
+ * sum(image) + n_out_of_window + n_active == n_loaded always. */
+int gcoreccd_read_image(gcoreccd_t* h, uint32_t* out, uint64_t cap_elems, uint64_t* n_out_of_window, int on_device);
+
+/* Introspection (host pointers, any may be NULL).  pair_interactions = sum over executed steps of n_active^2
+ * (ordered pairs of eq. 6, self terms included, padding excluded). */
+int gcoreccd_get_state(gcoreccd_t* h, uint64_t* step, uint64_t* n_active, uint64_t* n_loaded,
+                       uint64_t* n_collected, uint64_t* n_out_of_window, uint64_t* pair_interactions);
+
+/* Active carriers in their current (stable, load-ordered) order: interleaved xyz and ids.  Either output
+ * may be NULL.  *n receives the active count; fails with CAPACITY if cap < count.  Same on_device flag for both. */
+int gcoreccd_read_carriers(gcoreccd_t* h, float* xyz_um, uint32_t* id, uint64_t cap, uint64_t* n, int on_device);
+
+/* Coulomb field (eq. 6, V/cm) of the current snapshot, interleaved Ex,Ey,Ez in read_carriers order;
+ * does not advance the simulation.  cap = number of carriers the buffer holds. */
+int gcoreccd_eval_field(gcoreccd_t* h, float* Exyz_V_per_cm, uint64_t cap, int on_device);
+
+/* Run ONE step with CUDA events between its kernels (on the handle's stream) and return the device time of
+ * each in milliseconds: ms[0] field, ms[1] integrate+collect, ms[2] compact, ms[3] whole step.  Synchronous. */
+int gcoreccd_profile_step(gcoreccd_t* h, float ms_host[4]);
+
+/* Number of kernels this handle has launched so far (bench.py's gpu_launches). */
+uint64_t gcoreccd_kernel_launches(gcoreccd_t* h);
+
+/* Normal triple of (seed, id, step) as the integrator draws it (test hook for the Philox stream, a5). */
+int gcoreccd_debug_normals(gcoreccd_t* h, const uint32_t* id_host, const uint64_t* step_host, uint64_t n,
+                           double* n_xyz_host, uint32_t* words_host);
+
+const char* gcoreccd_strerror(int code);
+const char* gcoreccd_last_error(gcoreccd_t* h);   /* detail of the last failure on this handle ("" if none) */
+const char* gcoreccd_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GCORECCD_H */

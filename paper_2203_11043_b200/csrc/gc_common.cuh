@@ -1,0 +1,115 @@
+// gc_common.cuh — device-resident control block, state layout and the field-kernel work plan.
+//
+// State layout in HBM: structure of arrays, one FP32 array per coordinate plus the carrier
+// id, each padded to a multiple of 1024 entries and 256-byte aligned so that vector (64/128-bit) loads and
+// bulk copies never straddle an allocation.  Two such sets (A = state at step boundaries, B = scratch the
+// integrator writes and the compactor reads).  PAPER.md:84 stores "3N floats"; ids are ours (Philox key).
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace gc {
+
+constexpr int kTPB        = 256;          // threads per CTA of every kernel
+constexpr int kTile       = 256;          // sources per shared-memory tile == carriers per compaction tile
+constexpr uint32_t kPartFactor = 40;      // partial-sum slots per carrier of capacity (upper bound on j-splits)
+constexpr float kSentinel = 1.0e18f;      // padding source: (1e18)^-3 underflows to 0, contribution exactly 0
+
+// Work plan of the field kernel: the N_a x N_a interaction matrix is cut into nIB row blocks
+// (IB targets each) times S column chunks (JC sources each); item k = (row block k / S, chunk k % S) goes to
+// CTA k % grid.  The plan is a pure function of (n_active, IB, grid, partial capacity); it is computed once per
+// step by one warp (plan_search) and stored in Ctrl, so the partial sums are written and reduced in a fixed
+// order: runs are bit-reproducible and no float atomics are needed.
+struct FieldPlan {
+  uint32_t n;        // active carriers the plan was made for
+  uint32_t nIB;      // row blocks
+  uint32_t S;        // column chunks
+  uint32_t JC;       // sources per chunk (multiple of 8)
+  uint32_t stride;   // row stride of the partial buffers (n rounded up to 256)
+  uint32_t IB;       // targets per row block the plan was made for
+};
+
+struct Ctrl {                 // lives in device memory; only kernels write it (plus reset/load on the stream)
+  uint32_t n_active;          // carriers still drifting (valid entries of state A)
+  uint32_t n_next;            // scratch: survivors counted by the compactor
+  uint64_t step;              // index of the NEXT step (Philox counter)
+  uint64_t pairs;             // sum over executed steps of n_active^2
+  uint64_t n_collected;
+  uint64_t n_overflow;        // collected outside the image window
+  uint64_t n_loaded;
+  uint32_t nonfinite;         // sticky flag
+  uint32_t invalid;           // load validation flag
+  uint32_t blocks_done;       // "last block finishes" counter of the compactor
+  uint32_t pad_;
+  FieldPlan plan;             // valid for (n_active, current field variant)
+  uint32_t pad2_[2];
+};
+
+struct SoA {                  // one state set
+  float* x; float* y; float* z; uint32_t* id;
+};
+
+struct DevParams {            // constants uploaded by value with every launch
+  double a1_um;               // a1 * 1e-4  (V/cm per um)
+  double a2;
+  double mu0, inv_Ec, beta, inv_beta;   // eq. 2 with the T terms folded on the host
+  double drift_k;             // 1e-5 * dt
+  double sigma_k;             // 2 * 0.1 * (k_B T / q) * dt
+  double thickness, z_well;
+  double x0, y0, pitch;
+  double Kp;                  // K' (V/cm) um^2
+  float  eps2;                // softening^2 (clamped to >= 1e-24, R5)
+  uint32_t flags;
+  uint32_t seed_lo, seed_hi;
+  int32_t nx, ny;
+};
+
+struct PlanArgs { uint32_t IB; uint32_t grid; uint32_t part_cap_entries; };
+
+#ifdef __CUDACC__
+// Executed by ONE full warp.  Picks the smallest S whose static round-robin schedule wastes <= 1.5 % of the
+// CTA-rounds (else the least wasteful), subject to >= 64 sources per chunk and S * stride <= partial capacity.
+__device__ inline FieldPlan plan_search(uint32_t n, PlanArgs a) {
+  const uint32_t lane = threadIdx.x & 31u;
+  FieldPlan p;
+  p.n = n; p.IB = a.IB;
+  p.nIB = (n + a.IB - 1) / a.IB;
+  p.stride = (n + 255u) & ~255u;
+  p.S = 0; p.JC = 0;
+  if (n == 0) return p;
+  uint32_t s_max = (n + 63u) / 64u;
+  uint32_t s_cap = a.part_cap_entries / p.stride;
+  if (s_max > s_cap) s_max = s_cap;
+  if (s_max > 1024u) s_max = 1024u;
+  if (s_max < 1u) s_max = 1u;
+  float best_w = 3.0e38f; uint32_t best_S = 1, found = 0;
+  for (uint32_t base = 1; base <= s_max && !found; base += 32) {
+    uint32_t S = base + lane;
+    float w = 3.0e38f;
+    if (S <= s_max) {
+      uint32_t items = p.nIB * S;
+      uint32_t rounds = (items + a.grid - 1) / a.grid;
+      w = (float)rounds * (float)a.grid / (float)items;
+    }
+    uint32_t ok = __ballot_sync(0xffffffffu, w <= 1.015f);
+    if (ok) { found = base + (uint32_t)__ffs((int)ok) - 1u; break; }
+    if (w < best_w) { best_w = w; best_S = S; }
+  }
+  if (!found) {
+    // least wasteful; ties -> smallest S
+    for (int o = 16; o > 0; o >>= 1) {
+      float ow = __shfl_xor_sync(0xffffffffu, best_w, o);
+      uint32_t oS = __shfl_xor_sync(0xffffffffu, best_S, o);
+      if (ow < best_w || (ow == best_w && oS < best_S)) { best_w = ow; best_S = oS; }
+    }
+    found = best_S;
+  }
+  uint32_t JC = (n + found - 1) / found;
+  JC = (JC + 7u) & ~7u;
+  p.JC = JC;
+  p.S = (n + JC - 1) / JC;
+  return p;
+}
+#endif
+
+}  // namespace gc

@@ -1,0 +1,100 @@
+// gc_compact.cuh — step a8: stable stream compaction of the carriers still drifting (not in the paper, whose
+// kernel always sums i = 1..N; BASELINE.json north_star (d)).  Warp ballot + block scan, no
+// Thrust: tile t (kTPB carriers of state B) knows its survivor count from the integrator; its base offset is
+// the sum of the counts of tiles < t (a block-wide reduction over at most a few thousand integers), the rank
+// inside the tile comes from __ballot_sync/__popc and a scan over the warp totals.  Order is preserved, so a
+// carrier's index never depends on timing.  The CTA that FINISHES last (atomic ticket) publishes the new
+// n_active, advances the step index, accumulates the pair counter and computes the next step's FieldPlan.
+#pragma once
+#include "gc_common.cuh"
+
+namespace gc {
+
+// src: m entries of state B (m = n_active for a step, = n for a load); survivors (z > z_well) are appended to
+// dst (state A) starting at dst_off.  mode 0: time step (m read from ctrl->n_active, dst_off = 0, step += 1,
+// pairs += m^2 unless Coulomb is off);  mode 1: load (m, dst_off given; n_loaded += m).
+__global__ void __launch_bounds__(kTPB)
+k_compact(SoA B, SoA A, Ctrl* __restrict__ ctrl, const uint32_t* __restrict__ tile_count, uint32_t m_arg,
+          uint32_t dst_off_arg, int mode, double z_well, uint32_t count_pairs, PlanArgs pa) {
+  __shared__ uint32_t s_red[kTPB / 32];
+  __shared__ uint32_t s_base, s_last;
+  const uint32_t m = mode == 0 ? ctrl->n_active : m_arg;
+  const uint32_t dst_off = mode == 0 ? 0u : dst_off_arg;
+  if (m == 0) return;                                     // uniform: every CTA sees the same m; no step is taken
+  const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+  const uint32_t t = blockIdx.x;
+  const uint32_t n_tiles = (m + kTPB - 1) / kTPB;
+
+  if (t < n_tiles) {
+    // base = sum of survivor counts of tiles [0, t)
+    uint32_t part = 0;
+    for (uint32_t u = tid; u < t; u += kTPB) part += tile_count[u];
+    for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+    if (lane == 0) s_red[warp] = part;
+    __syncthreads();
+    if (tid == 0) {
+      uint32_t b = 0;
+      for (int w = 0; w < kTPB / 32; ++w) b += s_red[w];
+      s_base = b;
+    }
+    __syncthreads();
+    const uint32_t base = dst_off + s_base;
+
+    const uint32_t i = t * kTPB + tid;
+    float x = 0.f, y = 0.f, z = 0.f; uint32_t id = 0; bool keep = false;
+    if (i < m) { z = B.z[i]; keep = (double)z > z_well; if (keep) { x = B.x[i]; y = B.y[i]; id = B.id[i]; } }
+    const uint32_t bal = __ballot_sync(0xffffffffu, keep);
+    const uint32_t rank_in_warp = __popc(bal & ((1u << lane) - 1u));
+    __syncthreads();                                      // s_red reuse
+    if (lane == 0) s_red[warp] = __popc(bal);
+    __syncthreads();
+    uint32_t warp_off = 0;
+    for (uint32_t w = 0; w < warp; ++w) warp_off += s_red[w];
+    if (keep) {
+      const uint32_t d = base + warp_off + rank_in_warp;
+      A.x[d] = x; A.y[d] = y; A.z[d] = z; A.id[d] = id;
+    }
+    if (t == n_tiles - 1 && tid == 0) {
+      uint32_t tot = 0;
+      for (int w = 0; w < kTPB / 32; ++w) tot += s_red[w];
+      ctrl->n_next = base + tot;                          // new n_active (published by the last finisher)
+    }
+  }
+
+  // ---- last-finisher epilogue -------------------------------------------------------------------
+  __syncthreads();
+  if (tid == 0) {
+    __threadfence();
+    const uint32_t ticket = atomicAdd(&ctrl->blocks_done, 1u);
+    s_last = (ticket == gridDim.x - 1) ? 1u : 0u;
+  }
+  __syncthreads();
+  if (s_last && warp == 0) {
+    __threadfence();
+    const uint32_t n_new = *((volatile uint32_t*)&ctrl->n_next);
+    const FieldPlan plan = plan_search(n_new, pa);
+    if (lane == 0) {
+      ctrl->plan = plan;
+      ctrl->n_active = n_new;
+      ctrl->blocks_done = 0;
+      if (mode == 0) {
+        ctrl->step += 1;
+        if (count_pairs) ctrl->pairs += (uint64_t)m * (uint64_t)m;
+      } else {
+        ctrl->n_loaded += m;
+      }
+    }
+  }
+}
+
+// Recompute the plan when the host switches the field-kernel variant (or after reset / snapshot).
+__global__ void k_replan(Ctrl* __restrict__ ctrl, PlanArgs pa, int set_n, uint32_t n_new, int set_step, uint64_t step) {
+  if (set_n && threadIdx.x == 0) ctrl->n_active = n_new;
+  if (set_step && threadIdx.x == 0) ctrl->step = step;
+  __syncwarp();
+  const uint32_t n = set_n ? n_new : ctrl->n_active;
+  const FieldPlan plan = plan_search(n, pa);
+  if (threadIdx.x == 0) ctrl->plan = plan;
+}
+
+}  // namespace gc

@@ -1,0 +1,195 @@
+// gc_integrate.cuh — steps a2..a7 fused in one kernel (PAPER.md:68 order):
+//   reduce the field partials in fixed order -> E_Coul = K' S (eq. 6) -> + depletion field (eq. 1) -> |E| ->
+//   mobility (eq. 2) -> drift (v = mu E) -> Philox4x32-10 + Box-Muller diffusion (eqs. 3-4) -> update ->
+//   mirror at the back surface -> collection test -> integer atomic pixel histogram.
+// O(N) and bandwidth/latency bound; the per-carrier arithmetic is done in FP64 (B200 runs FP64 at half the
+// FP32 rate, and this kernel is < 0.1 % of a step at large N) so that a carrier's new position is the
+// correctly rounded FP32 value of the same FP64 expression the oracle evaluates; only E_Coul carries FP32
+// summation error.  State is stored FP32.
+#pragma once
+#include "gc_common.cuh"
+
+namespace gc {
+
+// ---------------------------------------------------------------------------------------------------
+// Philox4x32-10 (Salmon et al., SC'11).  Counter = (id, 0, step_lo, step_hi), key = (seed_lo, seed_hi).
+// Written independently of oracle/goracle.c (DESIGN.md §3 R13).
+// ---------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint2 k) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const uint32_t hi0 = __umulhi(0xD2511F53u, c.x), lo0 = 0xD2511F53u * c.x;
+    const uint32_t hi1 = __umulhi(0xCD9E8D57u, c.z), lo1 = 0xCD9E8D57u * c.z;
+    c = make_uint4(hi1 ^ c.y ^ k.x, lo1, hi0 ^ c.w ^ k.y, lo0);
+    k.x += 0x9E3779B9u; k.y += 0xBB67AE85u;
+  }
+  return c;
+}
+
+// u = ((w>>9)+0.5) 2^-23 in (0,1); f = (w>>8) 2^-24 in [0,1): exactly representable in FP32 and FP64.
+// n = (R_a cos 2 pi f_a, R_a sin 2 pi f_a, R_b cos 2 pi f_b), R = sqrt(-2 ln u).
+__device__ __forceinline__ void philox_normals(uint32_t seed_lo, uint32_t seed_hi, uint32_t id, uint64_t step,
+                                               double n[3], uint4* words) {
+  const uint4 w = philox4x32_10(make_uint4(id, 0u, (uint32_t)step, (uint32_t)(step >> 32)), make_uint2(seed_lo, seed_hi));
+  const double ua = ((double)(w.x >> 9) + 0.5) * (1.0 / 8388608.0);
+  const double fa = (double)(w.y >> 8) * (1.0 / 16777216.0);
+  const double ub = ((double)(w.z >> 9) + 0.5) * (1.0 / 8388608.0);
+  const double fb = (double)(w.w >> 8) * (1.0 / 16777216.0);
+  const double Ra = sqrt(-2.0 * log(ua)), Rb = sqrt(-2.0 * log(ub));
+  double sa, ca;
+  sincospi(2.0 * fa, &sa, &ca);
+  n[0] = Ra * ca; n[1] = Ra * sa; n[2] = Rb * cospi(2.0 * fb);
+  if (words) *words = w;
+}
+
+// eq. 2 with the temperature terms folded on the host: mu = mu0 / (1 + (E/Ec)^beta)^(1/beta)
+__device__ __forceinline__ double mobility(double E, const DevParams& P) {
+  return P.mu0 / pow(1.0 + pow(E * P.inv_Ec, P.beta), P.inv_beta);
+}
+
+// a7: half-open pixel bins, floor, in FP64 on the stored FP32 position (exactly reproducible).
+__device__ __forceinline__ void collect(float x, float y, const DevParams& P, uint32_t* image, uint32_t& n_over) {
+  const double fx = floor(((double)x - P.x0) / P.pitch);
+  const double fy = floor(((double)y - P.y0) / P.pitch);
+  if (fx >= 0.0 && fx < (double)P.nx && fy >= 0.0 && fy < (double)P.ny)
+    atomicAdd(image + (size_t)fy * (size_t)P.nx + (size_t)fx, 1u);
+  else
+    n_over += 1u;
+}
+
+// Block-level tally of (collected, overflow) and the survivor count of this tile.
+__device__ __forceinline__ void tally(uint32_t coll, uint32_t over, uint32_t keep, Ctrl* ctrl, uint32_t* tile_count) {
+  __shared__ uint32_t s_c[3];
+  if (threadIdx.x < 3) s_c[threadIdx.x] = 0;
+  __syncthreads();
+  const uint32_t wc = __popc(__ballot_sync(0xffffffffu, coll)), wo = __popc(__ballot_sync(0xffffffffu, over)),
+                 wk = __popc(__ballot_sync(0xffffffffu, keep));
+  if ((threadIdx.x & 31u) == 0) {
+    if (wc) atomicAdd(&s_c[0], wc);
+    if (wo) atomicAdd(&s_c[1], wo);
+    if (wk) atomicAdd(&s_c[2], wk);
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    if (s_c[0]) atomicAdd((unsigned long long*)&ctrl->n_collected, (unsigned long long)s_c[0]);
+    if (s_c[1]) atomicAdd((unsigned long long*)&ctrl->n_overflow, (unsigned long long)s_c[1]);
+    tile_count[blockIdx.x] = s_c[2];
+  }
+}
+
+// One thread per carrier; tile = kTPB carriers; reads state A + partials, writes state B (same index) and
+// the tile's survivor count.  Grid is sized from the host's upper bound on n_active; surplus CTAs exit.
+__global__ void __launch_bounds__(kTPB)
+k_integrate(SoA A, SoA B, Ctrl* __restrict__ ctrl, const float* __restrict__ Ep, uint32_t part_cap,
+            uint32_t* __restrict__ image, uint32_t* __restrict__ tile_count, DevParams P) {
+  const uint32_t n = ctrl->n_active;
+  const uint32_t i = blockIdx.x * kTPB + threadIdx.x;
+  if (blockIdx.x * kTPB >= n) return;
+  const uint64_t step = ctrl->step;
+  uint32_t coll = 0, over = 0, keep = 0;
+  if (i < n) {
+    const float x = A.x[i], y = A.y[i], z = A.z[i];
+    const uint32_t id = A.id[i];
+    double Ex = 0.0, Ey = 0.0, Ez = 0.0;
+    if (!(P.flags & 1u)) {                                   // GCORECCD_COULOMB_OFF
+      const uint32_t S = ctrl->plan.S, stride = ctrl->plan.stride;
+      const float* ex = Ep + i;
+      for (uint32_t s = 0; s < S; ++s) {                     // fixed order
+        Ex += (double)ex[(size_t)s * stride];
+        Ey += (double)ex[(size_t)s * stride + part_cap];
+        Ez += (double)ex[(size_t)s * stride + 2 * (size_t)part_cap];
+      }
+      Ex *= -P.Kp; Ey *= -P.Kp; Ez *= -P.Kp;                 // partials hold sum (r_s - r_t) w
+    }
+    if (!(P.flags & 4u)) Ez += P.a1_um * (double)z - P.a2;   // eq. 1
+    const double Emag = sqrt(Ex * Ex + Ey * Ey + Ez * Ez);
+    const double mu = mobility(Emag, P);                     // eq. 2
+    const double kd = P.drift_k * mu;                        // 1e-5 mu dt
+    double dx = kd * Ex, dy = kd * Ey, dz = kd * Ez;
+    if (!(P.flags & 2u)) {                                   // eqs. 3-4
+      double nrm[3];
+      philox_normals(P.seed_lo, P.seed_hi, id, step, nrm, nullptr);
+      const double sigma = sqrt(P.sigma_k * mu);
+      dx += sigma * nrm[0]; dy += sigma * nrm[1]; dz += sigma * nrm[2];
+    }
+    const double xn = (double)x + dx, yn = (double)y + dy;
+    double zn = (double)z + dz;
+    if (zn > P.thickness) zn = 2.0 * P.thickness - zn;       // specular back surface
+    const float xf = (float)xn, yf = (float)yn, zf = (float)zn;
+    if (!(isfinite(xf) && isfinite(yf) && isfinite(zf))) atomicOr(&ctrl->nonfinite, 1u);
+    B.x[i] = xf; B.y[i] = yf; B.z[i] = zf; B.id[i] = id;
+    if ((double)zf <= P.z_well) { coll = 1; uint32_t o = 0; collect(xf, yf, P, image, o); over = o; }
+    else keep = 1;
+  }
+  tally(coll, over, keep, ctrl, tile_count);
+}
+
+// Load path: unpack interleaved xyz into state B at [0,n), assign ids n_loaded + k, collect z <= z_well.
+__global__ void __launch_bounds__(kTPB)
+k_unpack(const float* __restrict__ xyz, uint32_t n, SoA B, Ctrl* __restrict__ ctrl, uint32_t id_base,
+         uint32_t* __restrict__ image, uint32_t* __restrict__ tile_count, DevParams P) {
+  const uint32_t i = blockIdx.x * kTPB + threadIdx.x;
+  uint32_t coll = 0, over = 0, keep = 0;
+  if (i < n) {
+    const float x = xyz[3 * (size_t)i], y = xyz[3 * (size_t)i + 1], z = xyz[3 * (size_t)i + 2];
+    B.x[i] = x; B.y[i] = y; B.z[i] = z; B.id[i] = id_base + i;
+    if ((double)z <= P.z_well) { coll = 1; uint32_t o = 0; collect(x, y, P, image, o); over = o; }
+    else keep = 1;
+  }
+  tally(coll, over, keep, ctrl, tile_count);
+}
+
+// Load validation: any non-finite coordinate or z above the back surface sets ctrl->invalid.
+__global__ void __launch_bounds__(kTPB)
+k_validate(const float* __restrict__ xyz, uint32_t n, Ctrl* __restrict__ ctrl, double thickness) {
+  const uint32_t i = blockIdx.x * kTPB + threadIdx.x;
+  if (i >= n) return;
+  const float x = xyz[3 * (size_t)i], y = xyz[3 * (size_t)i + 1], z = xyz[3 * (size_t)i + 2];
+  if (!(isfinite(x) && isfinite(y) && isfinite(z)) || (double)z > thickness) atomicOr(&ctrl->invalid, 1u);
+}
+
+// eval_field epilogue: E = -K' * sum_s partial, interleaved Ex,Ey,Ez.
+__global__ void __launch_bounds__(kTPB)
+k_field_finalize(const Ctrl* __restrict__ ctrl, const float* __restrict__ Ep, uint32_t part_cap, double Kp,
+                 float* __restrict__ out) {
+  const uint32_t n = ctrl->n_active;
+  const uint32_t i = blockIdx.x * kTPB + threadIdx.x;
+  if (i >= n) return;
+  const uint32_t S = ctrl->plan.S, stride = ctrl->plan.stride;
+  double Ex = 0.0, Ey = 0.0, Ez = 0.0;
+  for (uint32_t s = 0; s < S; ++s) {
+    Ex += (double)Ep[(size_t)s * stride + i];
+    Ey += (double)Ep[(size_t)s * stride + i + part_cap];
+    Ez += (double)Ep[(size_t)s * stride + i + 2 * (size_t)part_cap];
+  }
+  out[3 * (size_t)i] = (float)(-Kp * Ex); out[3 * (size_t)i + 1] = (float)(-Kp * Ey); out[3 * (size_t)i + 2] = (float)(-Kp * Ez);
+}
+
+// read_carriers: SoA -> interleaved xyz
+__global__ void __launch_bounds__(kTPB)
+k_interleave(SoA A, const Ctrl* __restrict__ ctrl, float* __restrict__ xyz) {
+  const uint32_t n = ctrl->n_active;
+  const uint32_t i = blockIdx.x * kTPB + threadIdx.x;
+  if (i >= n) return;
+  xyz[3 * (size_t)i] = A.x[i]; xyz[3 * (size_t)i + 1] = A.y[i]; xyz[3 * (size_t)i + 2] = A.z[i];
+}
+
+// load_snapshot: replace the active set
+__global__ void __launch_bounds__(kTPB)
+k_set_snapshot(const float* __restrict__ xyz, const uint32_t* __restrict__ id, uint32_t n, SoA A) {
+  const uint32_t i = blockIdx.x * kTPB + threadIdx.x;
+  if (i >= n) return;
+  A.x[i] = xyz[3 * (size_t)i]; A.y[i] = xyz[3 * (size_t)i + 1]; A.z[i] = xyz[3 * (size_t)i + 2]; A.id[i] = id[i];
+}
+
+__global__ void k_debug_normals(const uint32_t* __restrict__ id, const uint64_t* __restrict__ step, uint32_t n,
+                                uint32_t seed_lo, uint32_t seed_hi, double* __restrict__ out, uint32_t* __restrict__ words) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  double nrm[3]; uint4 w;
+  philox_normals(seed_lo, seed_hi, id[i], step[i], nrm, &w);
+  out[3 * i] = nrm[0]; out[3 * i + 1] = nrm[1]; out[3 * i + 2] = nrm[2];
+  words[4 * i] = w.x; words[4 * i + 1] = w.y; words[4 * i + 2] = w.z; words[4 * i + 3] = w.w;
+}
+
+}  // namespace gc

@@ -1,0 +1,580 @@
+// gcoreccd.cu — host side of the C ABI declared in include/gcoreccd.h: workspace carving, launches, CUDA
+// graphs, readback.  Every step of the hot path runs in the kernels of gc_field.cuh / gc_integrate.cuh /
+// gc_compact.cuh; nothing here computes physics and there is no CPU fallback.
+#include "../../include/gcoreccd.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "gc_common.cuh"
+#include "gc_compact.cuh"
+#include "gc_field.cuh"
+#include "gc_integrate.cuh"
+
+using namespace gc;
+
+namespace {
+
+constexpr uint64_t kMaxCarriers = 1ull << 26;
+constexpr int kNumVariants = 3;                       // field kernel register-blocking variants
+constexpr int kGraphSteps = 8;                        // steps per CUDA-graph launch
+
+struct Layout {
+  uint64_t cap_pad, part_cap, n_tiles;
+  uint64_t off_ctrl, off_A, off_B, off_Ep, off_tiles, off_image, total;
+};
+
+inline uint64_t align_up(uint64_t v, uint64_t a) { return (v + a - 1) / a * a; }
+
+Layout make_layout(uint64_t max_carriers, int32_t nx, int32_t ny) {
+  Layout L;
+  L.cap_pad = align_up(max_carriers, 1024);
+  L.part_cap = (uint64_t)kPartFactor * L.cap_pad;
+  L.n_tiles = L.cap_pad / kTPB;
+  uint64_t o = 0;
+  L.off_ctrl = o;  o += align_up(sizeof(Ctrl), 256);
+  L.off_A = o;     o += align_up(4 * L.cap_pad * 4, 256);
+  L.off_B = o;     o += align_up(4 * L.cap_pad * 4, 256);
+  L.off_Ep = o;    o += align_up(3 * L.part_cap * 4, 256);
+  L.off_tiles = o; o += align_up(L.n_tiles * 4, 256);
+  L.off_image = o; o += align_up((uint64_t)nx * (uint64_t)ny * 4, 256);
+  L.total = o;
+  return L;
+}
+
+}  // namespace
+
+struct gcoreccd {
+  gcoreccd_params p;
+  DevParams dp;
+  Layout L;
+  int device;
+  int num_sms;
+  cudaStream_t stream;
+  bool own_stream, own_ws;
+  char* ws;
+  Ctrl* ctrl;
+  Ctrl* h_ctrl;                 // pinned mirror
+  SoA A, B;
+  float* Ep;
+  uint32_t* tile_count;
+  uint32_t* image;
+  uint64_t n_loaded;            // host copy (ids continue)
+  uint64_t n_bound;             // host upper bound on n_active
+  int variant;                  // current field variant (-1 = none yet)
+  int grid_field[kNumVariants];
+  uint64_t launches;
+  cudaGraphExec_t graph;
+  int graph_variant;
+  uint32_t graph_tiles;
+  cudaEvent_t ev[4];
+  char err[256];
+};
+
+namespace {
+
+struct DeviceGuard {
+  int prev;
+  bool changed;
+  explicit DeviceGuard(int dev) : prev(-1), changed(false) {
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) { cudaSetDevice(dev); changed = true; }
+  }
+  ~DeviceGuard() { if (changed) cudaSetDevice(prev); }
+};
+
+int fail(gcoreccd_t* h, int code, const char* what, cudaError_t e = cudaSuccess) {
+  if (h) {
+    if (e != cudaSuccess) snprintf(h->err, sizeof(h->err), "%s: %s", what, cudaGetErrorString(e));
+    else snprintf(h->err, sizeof(h->err), "%s", what);
+  }
+  return code;
+}
+
+#define GC_CUDA(h, call)                                                       \
+  do {                                                                         \
+    cudaError_t e__ = (call);                                                  \
+    if (e__ != cudaSuccess) return fail((h), GCORECCD_ERR_CUDA, #call, e__);   \
+  } while (0)
+
+inline uint32_t variant_ib(int v) { return (uint32_t)kTPB * (2u << v); }     // 512, 1024, 2048 targets per row block
+
+inline int pick_variant(uint64_t n_bound) {
+  if (n_bound >= 49152) return 2;
+  if (n_bound >= 6144) return 1;
+  return 0;
+}
+
+inline PlanArgs plan_args(const gcoreccd_t* h, int v) {
+  PlanArgs a;
+  a.IB = variant_ib(v);
+  a.grid = (uint32_t)h->grid_field[v];
+  a.part_cap_entries = (uint32_t)h->L.part_cap;
+  return a;
+}
+
+inline uint32_t tiles_for(uint64_t n) { return (uint32_t)((n + kTPB - 1) / kTPB); }
+
+inline uint32_t bucket_tiles(uint32_t t) {                  // power-of-two buckets keep graph re-captures rare
+  uint32_t b = 1;
+  while (b < t) b <<= 1;
+  return b;
+}
+
+int launch_field(gcoreccd_t* h, int v) {
+  const int g = h->grid_field[v];
+  const uint32_t pc = (uint32_t)h->L.part_cap;
+  switch (v) {
+    case 0: k_field<1, 256, 4><<<g, kTPB, 0, h->stream>>>(h->A.x, h->A.y, h->A.z, h->ctrl, h->Ep, pc, h->dp.eps2); break;
+    case 1: k_field<2, 256, 3><<<g, kTPB, 0, h->stream>>>(h->A.x, h->A.y, h->A.z, h->ctrl, h->Ep, pc, h->dp.eps2); break;
+    default: k_field<4, 256, 1><<<g, kTPB, 0, h->stream>>>(h->A.x, h->A.y, h->A.z, h->ctrl, h->Ep, pc, h->dp.eps2); break;
+  }
+  h->launches += 1;
+  return 0;
+}
+
+// one time step = field + integrate + compact, all reading n_active / plan from device memory
+void enqueue_step(gcoreccd_t* h, uint32_t tiles) {
+  const bool coulomb = !(h->dp.flags & GCORECCD_COULOMB_OFF);
+  if (coulomb) launch_field(h, h->variant);
+  k_integrate<<<tiles, kTPB, 0, h->stream>>>(h->A, h->B, h->ctrl, h->Ep, (uint32_t)h->L.part_cap, h->image,
+                                             h->tile_count, h->dp);
+  k_compact<<<tiles, kTPB, 0, h->stream>>>(h->B, h->A, h->ctrl, h->tile_count, 0u, 0u, 0, h->dp.z_well,
+                                           coulomb ? 1u : 0u, plan_args(h, h->variant));
+  h->launches += 2;
+}
+
+int ensure_variant(gcoreccd_t* h) {
+  const int v = pick_variant(h->n_bound);
+  if (v != h->variant) {
+    h->variant = v;
+    k_replan<<<1, 32, 0, h->stream>>>(h->ctrl, plan_args(h, v), 0, 0u, 0, 0ull);
+    h->launches += 1;
+    GC_CUDA(h, cudaGetLastError());
+  }
+  return 0;
+}
+
+int sync_ctrl(gcoreccd_t* h) {
+  GC_CUDA(h, cudaMemcpyAsync(h->h_ctrl, h->ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, h->stream));
+  GC_CUDA(h, cudaStreamSynchronize(h->stream));
+  h->n_bound = h->h_ctrl->n_active;
+  return 0;
+}
+
+void drop_graph(gcoreccd_t* h) {
+  if (h->graph) { cudaGraphExecDestroy(h->graph); h->graph = nullptr; }
+}
+
+int ensure_graph(gcoreccd_t* h, uint32_t tiles) {
+  if (h->graph && h->graph_variant == h->variant && h->graph_tiles == tiles) return 0;
+  drop_graph(h);
+  cudaGraph_t g = nullptr;
+  GC_CUDA(h, cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal));
+  const uint64_t before = h->launches;
+  for (int k = 0; k < kGraphSteps; ++k) enqueue_step(h, tiles);
+  h->launches = before;                                   // capture does not launch
+  cudaError_t e = cudaStreamEndCapture(h->stream, &g);
+  if (e != cudaSuccess) return fail(h, GCORECCD_ERR_CUDA, "cudaStreamEndCapture", e);
+  e = cudaGraphInstantiate(&h->graph, g, 0);
+  cudaGraphDestroy(g);
+  if (e != cudaSuccess) { h->graph = nullptr; return fail(h, GCORECCD_ERR_CUDA, "cudaGraphInstantiate", e); }
+  h->graph_variant = h->variant;
+  h->graph_tiles = tiles;
+  return 0;
+}
+
+int enqueue_steps(gcoreccd_t* h, uint64_t n_steps) {
+  if (n_steps == 0 || h->n_bound == 0) return 0;
+  int rc = ensure_variant(h);
+  if (rc) return rc;
+  const uint32_t tiles = bucket_tiles(tiles_for(h->n_bound));
+  const uint32_t per_step = (h->dp.flags & GCORECCD_COULOMB_OFF) ? 2u : 3u;
+  while (n_steps >= (uint64_t)kGraphSteps) {
+    rc = ensure_graph(h, tiles);
+    if (rc) return rc;
+    GC_CUDA(h, cudaGraphLaunch(h->graph, h->stream));
+    h->launches += (uint64_t)kGraphSteps * per_step;
+    n_steps -= kGraphSteps;
+  }
+  for (; n_steps > 0; --n_steps) enqueue_step(h, tiles);
+  GC_CUDA(h, cudaGetLastError());
+  return 0;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------ C ABI
+extern "C" {
+
+uint64_t gcoreccd_workspace_size(uint64_t max_carriers, int32_t img_nx, int32_t img_ny) {
+  if (max_carriers == 0 || max_carriers > kMaxCarriers || img_nx < 1 || img_ny < 1 || img_nx > 16384 || img_ny > 16384)
+    return 0;
+  return make_layout(max_carriers, img_nx, img_ny).total;
+}
+
+int gcoreccd_create(const gcoreccd_params* p, gcoreccd_t** out) {
+  if (!p || !out) return GCORECCD_ERR_INVALID;
+  if (p->struct_size != sizeof(gcoreccd_params)) return GCORECCD_ERR_INVALID;
+  if (!(p->T_K > 0) || !(p->dt_ns > 0) || !(p->pixel_pitch_um > 0) || !(p->thickness_um > p->z_well_um) ||
+      !(p->softening_um >= 0) || !(p->eps_si >= 0) || !std::isfinite(p->a1_V_per_cm2) || !std::isfinite(p->a2_V_per_cm) ||
+      !std::isfinite(p->img_x0_um) || !std::isfinite(p->img_y0_um) || !std::isfinite(p->thickness_um) ||
+      p->img_nx < 1 || p->img_ny < 1 || p->img_nx > 16384 || p->img_ny > 16384 || p->max_carriers == 0 ||
+      p->max_carriers > kMaxCarriers || (p->flags & ~7u))
+    return GCORECCD_ERR_INVALID;
+
+  int dev = p->device;
+  if (dev < 0 && cudaGetDevice(&dev) != cudaSuccess) return GCORECCD_ERR_CUDA;
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return GCORECCD_ERR_CUDA;
+  if (prop.major != 10) return GCORECCD_ERR_CUDA;         // sm_100a only: no fallback path exists
+
+  gcoreccd_t* h = new (std::nothrow) gcoreccd();
+  if (!h) return GCORECCD_ERR_NOMEM;
+  memset(h, 0, sizeof(*h));
+  h->p = *p;
+  if (h->p.eps_si == 0.0) h->p.eps_si = 11.7;
+  h->device = dev;
+  h->num_sms = prop.multiProcessorCount;
+  h->variant = -1;
+  DeviceGuard guard(dev);
+
+  h->L = make_layout(p->max_carriers, p->img_nx, p->img_ny);
+  int rc = GCORECCD_OK;
+  cudaError_t e = cudaSuccess;
+  do {
+    if (p->workspace) {
+      if (p->workspace_bytes < h->L.total || ((uintptr_t)p->workspace & 255u)) { rc = GCORECCD_ERR_CAPACITY; break; }
+      h->ws = (char*)p->workspace;
+    } else {
+      e = cudaMalloc((void**)&h->ws, h->L.total);
+      if (e != cudaSuccess) { rc = e == cudaErrorMemoryAllocation ? GCORECCD_ERR_NOMEM : GCORECCD_ERR_CUDA; break; }
+      h->own_ws = true;
+    }
+    if (p->stream) h->stream = (cudaStream_t)p->stream;
+    else {
+      e = cudaStreamCreateWithFlags(&h->stream, cudaStreamNonBlocking);
+      if (e != cudaSuccess) { rc = GCORECCD_ERR_CUDA; break; }
+      h->own_stream = true;
+    }
+    e = cudaMallocHost((void**)&h->h_ctrl, sizeof(Ctrl));
+    if (e != cudaSuccess) { rc = GCORECCD_ERR_CUDA; break; }
+    for (int k = 0; k < 4; ++k) {
+      e = cudaEventCreate(&h->ev[k]);
+      if (e != cudaSuccess) break;
+    }
+    if (e != cudaSuccess) { rc = GCORECCD_ERR_CUDA; break; }
+  } while (0);
+  if (rc != GCORECCD_OK) { gcoreccd_destroy(h); return rc; }
+
+  const uint64_t cp = h->L.cap_pad;
+  h->ctrl = (Ctrl*)(h->ws + h->L.off_ctrl);
+  float* a = (float*)(h->ws + h->L.off_A);
+  h->A = SoA{a, a + cp, a + 2 * cp, (uint32_t*)(a + 3 * cp)};
+  float* b = (float*)(h->ws + h->L.off_B);
+  h->B = SoA{b, b + cp, b + 2 * cp, (uint32_t*)(b + 3 * cp)};
+  h->Ep = (float*)(h->ws + h->L.off_Ep);
+  h->tile_count = (uint32_t*)(h->ws + h->L.off_tiles);
+  h->image = (uint32_t*)(h->ws + h->L.off_image);
+
+  // constants (eq. 2 temperature terms, K', thermal voltage) folded on the host in FP64
+  const double q = 1.602176634e-19, kB = 1.380649e-23, eps0 = 8.8541878128e-12, pi = 3.14159265358979323846;
+  DevParams& d = h->dp;
+  const double T = p->T_K;
+  d.a1_um = p->a1_V_per_cm2 * 1e-4;
+  d.a2 = p->a2_V_per_cm;
+  d.mu0 = 1.31e8 * std::pow(T, -2.2);
+  d.inv_Ec = 1.0 / (1.24 * std::pow(T, 1.68));
+  d.beta = 0.46 * std::pow(T, 0.17);
+  d.inv_beta = 1.0 / d.beta;
+  d.drift_k = 1e-5 * p->dt_ns;
+  d.sigma_k = 2.0 * 0.1 * (kB * T / q) * p->dt_ns;
+  d.thickness = p->thickness_um;
+  d.z_well = p->z_well_um;
+  d.x0 = p->img_x0_um; d.y0 = p->img_y0_um; d.pitch = p->pixel_pitch_um;
+  d.Kp = q / (4.0 * pi * eps0 * h->p.eps_si) * 1e10;
+  const double e2 = p->softening_um * p->softening_um;
+  d.eps2 = (float)(e2 < 1e-24 ? 1e-24 : e2);              // eps = 0 -> eq. 5: coincident pairs contribute exactly 0
+  d.flags = p->flags;
+  d.seed_lo = (uint32_t)(p->seed & 0xffffffffu);
+  d.seed_hi = (uint32_t)(p->seed >> 32);
+  d.nx = p->img_nx; d.ny = p->img_ny;
+
+  // persistent grid of the field kernel: resident CTAs per SM x SM count
+  int occ[kNumVariants] = {0, 0, 0};
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[0], k_field<1, 256, 4>, kTPB, 0);
+  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[1], k_field<2, 256, 3>, kTPB, 0);
+  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[2], k_field<4, 256, 1>, kTPB, 0);
+  if (e != cudaSuccess) { fail(h, GCORECCD_ERR_CUDA, "occupancy query", e); gcoreccd_destroy(h); return GCORECCD_ERR_CUDA; }
+  for (int v = 0; v < kNumVariants; ++v) h->grid_field[v] = h->num_sms * (occ[v] > 0 ? occ[v] : 1);
+
+  rc = gcoreccd_reset(h);
+  if (rc != GCORECCD_OK) { gcoreccd_destroy(h); return rc; }
+  *out = h;
+  return GCORECCD_OK;
+}
+
+int gcoreccd_destroy(gcoreccd_t* h) {
+  if (!h) return GCORECCD_ERR_INVALID;
+  DeviceGuard guard(h->device);
+  if (h->stream) cudaStreamSynchronize(h->stream);
+  drop_graph(h);
+  for (int k = 0; k < 4; ++k) if (h->ev[k]) cudaEventDestroy(h->ev[k]);
+  if (h->h_ctrl) cudaFreeHost(h->h_ctrl);
+  if (h->own_stream && h->stream) cudaStreamDestroy(h->stream);
+  if (h->own_ws && h->ws) cudaFree(h->ws);
+  delete h;
+  return GCORECCD_OK;
+}
+
+int gcoreccd_reset(gcoreccd_t* h) {
+  if (!h) return GCORECCD_ERR_INVALID;
+  DeviceGuard guard(h->device);
+  GC_CUDA(h, cudaMemsetAsync(h->ctrl, 0, sizeof(Ctrl), h->stream));
+  GC_CUDA(h, cudaMemsetAsync(h->image, 0, (size_t)h->p.img_nx * h->p.img_ny * 4, h->stream));
+  GC_CUDA(h, cudaStreamSynchronize(h->stream));
+  h->n_loaded = 0;
+  h->n_bound = 0;
+  h->variant = -1;
+  h->err[0] = 0;
+  return GCORECCD_OK;
+}
+
+int gcoreccd_load_carriers(gcoreccd_t* h, const float* xyz, uint64_t n, int on_device) {
+  if (!h || (!xyz && n)) return GCORECCD_ERR_INVALID;
+  if (n == 0) return GCORECCD_OK;
+  DeviceGuard guard(h->device);
+  int rc = sync_ctrl(h);
+  if (rc) return rc;
+  const uint64_t n_act = h->h_ctrl->n_active;
+  if (n_act + n > h->p.max_carriers || h->n_loaded + n > 0xffffffffull) return fail(h, GCORECCD_ERR_CAPACITY, "load_carriers: capacity");
+  const float* src = xyz;
+  if (!on_device) {
+    GC_CUDA(h, cudaMemcpyAsync(h->Ep, xyz, n * 12, cudaMemcpyHostToDevice, h->stream));
+    src = h->Ep;
+  }
+  const uint32_t tiles = tiles_for(n);
+  GC_CUDA(h, cudaMemsetAsync(&h->ctrl->invalid, 0, 4, h->stream));
+  k_validate<<<tiles, kTPB, 0, h->stream>>>(src, (uint32_t)n, h->ctrl, h->dp.thickness);
+  h->launches += 1;
+  rc = sync_ctrl(h);
+  if (rc) return rc;
+  if (h->h_ctrl->invalid) return fail(h, GCORECCD_ERR_INVALID, "load_carriers: non-finite coordinate or z > thickness");
+  // the plan stored with the new n_active must match the variant the next step will use
+  const int v = pick_variant(n_act + n);
+  h->variant = v;
+  k_unpack<<<tiles, kTPB, 0, h->stream>>>(src, (uint32_t)n, h->B, h->ctrl, (uint32_t)h->n_loaded, h->image,
+                                          h->tile_count, h->dp);
+  k_compact<<<tiles, kTPB, 0, h->stream>>>(h->B, h->A, h->ctrl, h->tile_count, (uint32_t)n, (uint32_t)n_act, 1,
+                                           h->dp.z_well, 0u, plan_args(h, v));
+  h->launches += 2;
+  GC_CUDA(h, cudaGetLastError());
+  h->n_loaded += n;
+  rc = sync_ctrl(h);
+  if (rc) return rc;
+  h->variant = -1;                                         // re-pick (and re-plan) from the exact count
+  return GCORECCD_OK;
+}
+
+int gcoreccd_load_snapshot(gcoreccd_t* h, const float* xyz, const uint32_t* id, uint64_t n, uint64_t step) {
+  if (!h || ((!xyz || !id) && n)) return GCORECCD_ERR_INVALID;
+  if (n > h->p.max_carriers) return fail(h, GCORECCD_ERR_CAPACITY, "load_snapshot: capacity");
+  DeviceGuard guard(h->device);
+  float* st_xyz = h->Ep;
+  uint32_t* st_id = (uint32_t*)(h->Ep + 3 * h->L.cap_pad);
+  if (n) {
+    GC_CUDA(h, cudaMemcpyAsync(st_xyz, xyz, n * 12, cudaMemcpyHostToDevice, h->stream));
+    GC_CUDA(h, cudaMemcpyAsync(st_id, id, n * 4, cudaMemcpyHostToDevice, h->stream));
+    k_set_snapshot<<<tiles_for(n), kTPB, 0, h->stream>>>(st_xyz, st_id, (uint32_t)n, h->A);
+    h->launches += 1;
+  }
+  const int v = pick_variant(n);
+  h->variant = v;
+  k_replan<<<1, 32, 0, h->stream>>>(h->ctrl, plan_args(h, v), 1, (uint32_t)n, 1, step);
+  h->launches += 1;
+  GC_CUDA(h, cudaGetLastError());
+  int rc = sync_ctrl(h);
+  if (rc) return rc;
+  uint64_t max_id = 0;
+  for (uint64_t k = 0; k < n; ++k) if (id[k] > max_id) max_id = id[k];
+  if (n && h->n_loaded < max_id + 1) h->n_loaded = max_id + 1;
+  return GCORECCD_OK;
+}
+
+int gcoreccd_step(gcoreccd_t* h, uint32_t n_steps) {
+  if (!h) return GCORECCD_ERR_INVALID;
+  DeviceGuard guard(h->device);
+  return enqueue_steps(h, n_steps);
+}
+
+int gcoreccd_run_to_collection(gcoreccd_t* h, uint64_t max_steps, uint64_t* steps_done, uint64_t* n_active_left) {
+  if (!h) return GCORECCD_ERR_INVALID;
+  DeviceGuard guard(h->device);
+  int rc = sync_ctrl(h);
+  if (rc) return rc;
+  const uint64_t step0 = h->h_ctrl->step;
+  uint64_t done = 0;
+  int ret = GCORECCD_OK;
+  while (h->h_ctrl->n_active > 0) {
+    if (done >= max_steps) { ret = GCORECCD_MAX_STEPS; break; }
+    uint64_t batch = 4 * kGraphSteps;
+    if (batch > max_steps - done) batch = max_steps - done;
+    rc = enqueue_steps(h, batch);
+    if (rc) return rc;
+    rc = sync_ctrl(h);
+    if (rc) return rc;
+    if (h->h_ctrl->nonfinite) return fail(h, GCORECCD_ERR_NONFINITE, "a carrier position became non-finite");
+    done = h->h_ctrl->step - step0;
+  }
+  if (steps_done) *steps_done = done;
+  if (n_active_left) *n_active_left = h->h_ctrl->n_active;
+  return ret;
+}
+
+int gcoreccd_read_image(gcoreccd_t* h, uint32_t* out, uint64_t cap_elems, uint64_t* n_out_of_window, int on_device) {
+  if (!h || !out) return GCORECCD_ERR_INVALID;
+  const uint64_t ne = (uint64_t)h->p.img_nx * h->p.img_ny;
+  if (cap_elems < ne) return fail(h, GCORECCD_ERR_CAPACITY, "read_image: buffer too small");
+  DeviceGuard guard(h->device);
+  GC_CUDA(h, cudaMemcpyAsync(out, h->image, ne * 4, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, h->stream));
+  int rc = sync_ctrl(h);
+  if (rc) return rc;
+  if (n_out_of_window) *n_out_of_window = h->h_ctrl->n_overflow;
+  return GCORECCD_OK;
+}
+
+int gcoreccd_get_state(gcoreccd_t* h, uint64_t* step, uint64_t* n_active, uint64_t* n_loaded, uint64_t* n_collected,
+                       uint64_t* n_out_of_window, uint64_t* pair_interactions) {
+  if (!h) return GCORECCD_ERR_INVALID;
+  DeviceGuard guard(h->device);
+  int rc = sync_ctrl(h);
+  if (rc) return rc;
+  if (step) *step = h->h_ctrl->step;
+  if (n_active) *n_active = h->h_ctrl->n_active;
+  if (n_loaded) *n_loaded = h->h_ctrl->n_loaded;
+  if (n_collected) *n_collected = h->h_ctrl->n_collected;
+  if (n_out_of_window) *n_out_of_window = h->h_ctrl->n_overflow;
+  if (pair_interactions) *pair_interactions = h->h_ctrl->pairs;
+  if (h->h_ctrl->nonfinite) return fail(h, GCORECCD_ERR_NONFINITE, "a carrier position became non-finite");
+  return GCORECCD_OK;
+}
+
+int gcoreccd_read_carriers(gcoreccd_t* h, float* xyz, uint32_t* id, uint64_t cap, uint64_t* n, int on_device) {
+  if (!h) return GCORECCD_ERR_INVALID;
+  DeviceGuard guard(h->device);
+  int rc = sync_ctrl(h);
+  if (rc) return rc;
+  const uint64_t na = h->h_ctrl->n_active;
+  if (n) *n = na;
+  if ((xyz || id) && cap < na) return fail(h, GCORECCD_ERR_CAPACITY, "read_carriers: buffer too small");
+  if (na == 0) return GCORECCD_OK;
+  const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+  if (xyz) {
+    float* stage = on_device ? xyz : h->Ep;
+    k_interleave<<<tiles_for(na), kTPB, 0, h->stream>>>(h->A, h->ctrl, stage);
+    h->launches += 1;
+    if (!on_device) GC_CUDA(h, cudaMemcpyAsync(xyz, stage, na * 12, kind, h->stream));
+  }
+  if (id) GC_CUDA(h, cudaMemcpyAsync(id, h->A.id, na * 4, kind, h->stream));
+  GC_CUDA(h, cudaGetLastError());
+  GC_CUDA(h, cudaStreamSynchronize(h->stream));
+  return GCORECCD_OK;
+}
+
+int gcoreccd_eval_field(gcoreccd_t* h, float* E, uint64_t cap, int on_device) {
+  if (!h || !E) return GCORECCD_ERR_INVALID;
+  DeviceGuard guard(h->device);
+  int rc = sync_ctrl(h);
+  if (rc) return rc;
+  const uint64_t na = h->h_ctrl->n_active;
+  if (cap < na) return fail(h, GCORECCD_ERR_CAPACITY, "eval_field: buffer too small");
+  if (na == 0) return GCORECCD_OK;
+  rc = ensure_variant(h);
+  if (rc) return rc;
+  launch_field(h, h->variant);
+  float* stage = on_device ? E : h->B.x;                   // state B is scratch between steps (3*cap_pad floats)
+  k_field_finalize<<<tiles_for(na), kTPB, 0, h->stream>>>(h->ctrl, h->Ep, (uint32_t)h->L.part_cap, h->dp.Kp, stage);
+  h->launches += 1;
+  if (!on_device) GC_CUDA(h, cudaMemcpyAsync(E, stage, na * 12, cudaMemcpyDeviceToHost, h->stream));
+  GC_CUDA(h, cudaGetLastError());
+  GC_CUDA(h, cudaStreamSynchronize(h->stream));
+  return GCORECCD_OK;
+}
+
+int gcoreccd_profile_step(gcoreccd_t* h, float ms[4]) {
+  if (!h || !ms) return GCORECCD_ERR_INVALID;
+  DeviceGuard guard(h->device);
+  ms[0] = ms[1] = ms[2] = ms[3] = 0.f;
+  if (h->n_bound == 0) return GCORECCD_OK;
+  int rc = ensure_variant(h);
+  if (rc) return rc;
+  const uint32_t tiles = bucket_tiles(tiles_for(h->n_bound));
+  const bool coulomb = !(h->dp.flags & GCORECCD_COULOMB_OFF);
+  GC_CUDA(h, cudaEventRecord(h->ev[0], h->stream));
+  if (coulomb) launch_field(h, h->variant);
+  GC_CUDA(h, cudaEventRecord(h->ev[1], h->stream));
+  k_integrate<<<tiles, kTPB, 0, h->stream>>>(h->A, h->B, h->ctrl, h->Ep, (uint32_t)h->L.part_cap, h->image,
+                                             h->tile_count, h->dp);
+  GC_CUDA(h, cudaEventRecord(h->ev[2], h->stream));
+  k_compact<<<tiles, kTPB, 0, h->stream>>>(h->B, h->A, h->ctrl, h->tile_count, 0u, 0u, 0, h->dp.z_well,
+                                           coulomb ? 1u : 0u, plan_args(h, h->variant));
+  GC_CUDA(h, cudaEventRecord(h->ev[3], h->stream));
+  h->launches += 2;
+  GC_CUDA(h, cudaGetLastError());
+  rc = sync_ctrl(h);
+  if (rc) return rc;
+  GC_CUDA(h, cudaEventElapsedTime(&ms[0], h->ev[0], h->ev[1]));
+  GC_CUDA(h, cudaEventElapsedTime(&ms[1], h->ev[1], h->ev[2]));
+  GC_CUDA(h, cudaEventElapsedTime(&ms[2], h->ev[2], h->ev[3]));
+  GC_CUDA(h, cudaEventElapsedTime(&ms[3], h->ev[0], h->ev[3]));
+  return GCORECCD_OK;
+}
+
+uint64_t gcoreccd_kernel_launches(gcoreccd_t* h) { return h ? h->launches : 0; }
+
+int gcoreccd_debug_normals(gcoreccd_t* h, const uint32_t* id, const uint64_t* step, uint64_t n, double* out, uint32_t* words) {
+  if (!h || !id || !step || !out || !words) return GCORECCD_ERR_INVALID;
+  if (n == 0) return GCORECCD_OK;
+  DeviceGuard guard(h->device);
+  char* buf = nullptr;
+  const size_t b_id = align_up(n * 4, 256), b_st = align_up(n * 8, 256), b_out = align_up(n * 24, 256), b_w = align_up(n * 16, 256);
+  GC_CUDA(h, cudaMalloc((void**)&buf, b_id + b_st + b_out + b_w));
+  uint32_t* d_id = (uint32_t*)buf;
+  uint64_t* d_st = (uint64_t*)(buf + b_id);
+  double* d_out = (double*)(buf + b_id + b_st);
+  uint32_t* d_w = (uint32_t*)(buf + b_id + b_st + b_out);
+  cudaError_t e = cudaMemcpyAsync(d_id, id, n * 4, cudaMemcpyHostToDevice, h->stream);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(d_st, step, n * 8, cudaMemcpyHostToDevice, h->stream);
+  if (e == cudaSuccess) {
+    k_debug_normals<<<(unsigned)((n + 127) / 128), 128, 0, h->stream>>>(d_id, d_st, (uint32_t)n, h->dp.seed_lo, h->dp.seed_hi, d_out, d_w);
+    h->launches += 1;
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess) e = cudaMemcpyAsync(out, d_out, n * 24, cudaMemcpyDeviceToHost, h->stream);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(words, d_w, n * 16, cudaMemcpyDeviceToHost, h->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+  cudaFree(buf);
+  if (e != cudaSuccess) return fail(h, GCORECCD_ERR_CUDA, "debug_normals", e);
+  return GCORECCD_OK;
+}
+
+const char* gcoreccd_strerror(int code) {
+  switch (code) {
+    case GCORECCD_OK: return "ok";
+    case GCORECCD_MAX_STEPS: return "max_steps reached with carriers still drifting";
+    case GCORECCD_ERR_INVALID: return "invalid argument";
+    case GCORECCD_ERR_STATE: return "bad state";
+    case GCORECCD_ERR_CAPACITY: return "capacity exceeded";
+    case GCORECCD_ERR_NOMEM: return "out of memory";
+    case GCORECCD_ERR_CUDA: return "CUDA error or no sm_100 device";
+    case GCORECCD_ERR_NONFINITE: return "non-finite carrier state";
+    default: return "unknown";
+  }
+}
+
+const char* gcoreccd_last_error(gcoreccd_t* h) { return h ? h->err : ""; }
+
+const char* gcoreccd_version(void) { return "gcoreccd-b200 0.1 (sm_100a)"; }
+
+}  // extern "C"

@@ -1,0 +1,330 @@
+"""GPU parity tests proper (-m gpu): the CUDA path, called through the C ABI, against the FP64 oracle on the
+same seeded inputs.  Tolerances are BASELINE.json:north_star's: fields 1e-4 relative at a fixed snapshot,
+trajectories 1e-3 um after 10 steps, hole count conserved exactly, images statistically (1 %)."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import goracle as g
+from paper_2203_11043_b200 import workloads
+from util import field_rel_err, gpu_sim, image_moments, oracle_sim
+
+pytestmark = pytest.mark.gpu
+
+FIELD_TOL = 1e-4      # north_star: per-carrier field vectors within 1e-4 relative (FP32 vs FP64)
+TRAJ_TOL = 1e-3       # north_star: trajectories within 1e-3 um after 10 steps
+
+
+def _field_ref(xyz, P, targets=None):
+    return g.coulomb_field(xyz.astype(np.float64), eps_um=P["softening_um"], Kp=g.coulomb_constant(P["eps_si"]),
+                           targets=targets)
+
+
+# ------------------------------------------------------------------ a1: field at a fixed snapshot
+@pytest.mark.parametrize("cfg,n", [(0, 1024), (0, 1), (0, 2), (0, 3), (0, 257), (0, 1000), (0, 5000), (0, 6143),
+                                   (0, 6144), (1, 16384), (2, 20011), (3, 30000), (2, 49152), (2, 65537)])
+def test_field_parity_element_by_element(cfg, n):
+    w = workloads.make(cfg, n=n)
+    P = w["params"]
+    xyz = w["xyz"][w["xyz"][:, 2] > 0]                     # cfg 3 leaves z<=0 holes to be collected at load
+    sim = gpu_sim(w)
+    sim.load_carriers(w["xyz"])
+    E = sim.eval_field()
+    assert E.shape == (len(xyz), 3)
+    if len(xyz) == 1:
+        assert np.all(E == 0.0)
+        return
+    Eref = _field_ref(xyz, P)
+    unfl, fl = field_rel_err(E, Eref)
+    assert unfl <= FIELD_TOL, (unfl, fl)
+    # Newton's third law survives FP32 to the accumulated rounding level
+    assert np.linalg.norm(E.astype(np.float64).sum(axis=0)) <= 1e-5 * np.linalg.norm(E, axis=1).sum()
+    sim.close()
+
+
+def test_field_eps_zero_is_eq5_and_coincident_carriers_are_finite():
+    w = workloads.make(0, n=300)
+    xyz = w["xyz"].copy()
+    xyz[7] = xyz[3]                                         # an exact coincidence
+    sim = gpu_sim(w, softening_um=0.0)
+    sim.load_carriers(xyz)
+    E = sim.eval_field()
+    assert np.isfinite(E).all()
+    Eref = g.coulomb_field(xyz.astype(np.float64), eps_um=0.0, Kp=g.coulomb_constant(11.7))
+    assert field_rel_err(E, Eref)[0] <= FIELD_TOL
+    sim.close()
+
+
+# ------------------------------------------------------------------ a5: the Philox normal stream
+def test_normal_stream_matches_oracle_bit_for_bit_in_the_words():
+    w = workloads.make(0, n=8)
+    sim = gpu_sim(w)
+    ids = np.array([0, 5, 131071, 1, 2, 0xffffffff, 77, 1048575], dtype=np.uint32)
+    steps = np.array([0, 7, 999, 2 ** 32 + 5, 1, 0, 123456789, 2 ** 40], dtype=np.uint64)
+    n, words = sim.debug_normals(ids, steps)
+    for k in range(len(ids)):
+        rn, rw = g.normals(w["params"]["seed"], int(ids[k]), int(steps[k]))
+        assert words[k].tolist() == rw
+        assert np.allclose(n[k], rn, rtol=0, atol=1e-12)
+    sim.close()
+
+
+# ------------------------------------------------------------------ a2..a8: 10-step trajectories
+def _trajectory_check(w, flags_gpu, flags_or, steps=10, tol=TRAJ_TOL, **over):
+    """GPU vs FP32-state oracle after `steps` steps from identical FP32 inputs.  Explicit Euler with eps = 1e-3 um
+    is chaotic through close encounters (a pair at 0.01 um is thrown ~5 um apart in one step, so a 1-ulp
+    difference in r becomes ~0.05 um): a carrier may exceed `tol` only if the ORACLE's trajectory shows a
+    neighbour closer than 0.1 um inside the window (R21); everyone else must be within `tol`."""
+    sim = gpu_sim(w, flags=flags_gpu, **over)
+    sim.load_carriers(w["xyz"])
+    o = oracle_sim(w, flags=flags_or | g.FP32_STATE, **over)
+    o.load(w["xyz"])
+    sim.step(steps)
+    history = []
+    for _ in range(steps):
+        history.append(o.carriers())
+        o.step(1)
+    xyz, ids = sim.read_carriers()
+    oxyz, oids = o.carriers()
+    st, ost = sim.state(), o.state()
+    assert st["step"] == ost["step"]
+    assert st["n_active"] + st["n_collected"] == st["n_loaded"]
+    sim.close()
+    common = np.intersect1d(ids, oids)
+    xyz_c, oxyz_c = xyz[np.isin(ids, common)], oxyz[np.isin(oids, common)]
+    d = np.abs(xyz_c.astype(np.float64) - oxyz_c).max(axis=1)
+    suspects = set(common[d > tol].tolist()) | set(np.setxor1d(ids, oids).tolist())   # incl. retire-flag mismatches
+    if suspects:
+        assert len(suspects) <= 0.02 * len(w["xyz"]) + 2, len(suspects)
+        closest = {i: np.inf for i in suspects}
+        for hx, hid in history:
+            for i in suspects:
+                k = np.searchsorted(hid, i)
+                if k < len(hid) and hid[k] == i:
+                    r = np.linalg.norm(hx - hx[k], axis=1)
+                    r[k] = np.inf
+                    closest[i] = min(closest[i], r.min())
+        # retire-flag mismatches must sit at the collection plane, or come from a close encounter like the rest
+        for i, r in closest.items():
+            assert r < 0.1, (i, r, "exceeds %g um without a close encounter" % tol)
+    return d
+
+
+@pytest.mark.parametrize("cfg,n", [(0, 1024), (0, 777), (1, 16384), (3, 8192)])
+def test_trajectory_parity_10_steps_full_physics(cfg, n):
+    _trajectory_check(workloads.make(cfg, n=n), 0, 0)
+
+
+def test_trajectory_parity_flag_combinations():
+    from paper_2203_11043_b200 import binding as b
+    w = workloads.make(0, n=600)
+    _trajectory_check(w, b.COULOMB_OFF, g.COULOMB_OFF)
+    _trajectory_check(w, b.DIFFUSION_OFF, g.DIFFUSION_OFF, tol=2e-4)
+    _trajectory_check(w, b.DEPLETION_OFF | b.DIFFUSION_OFF, g.DEPLETION_OFF | g.DIFFUSION_OFF, tol=2e-4)
+    _trajectory_check(w, b.COULOMB_OFF | b.DIFFUSION_OFF, g.COULOMB_OFF | g.DIFFUSION_OFF, tol=1e-6)
+
+
+def test_trajectory_parity_other_device_constants():
+    w = workloads.make(0, n=512)
+    _trajectory_check(w, 0, 0, T_K=77.0, dt_ns=0.02, softening_um=5e-3, eps_si=11.9, seed=12345678901234567)
+
+
+def test_single_step_from_snapshot_is_the_correctly_rounded_oracle_step():
+    # one step from identical FP32 state: the only difference allowed is the FP32 Coulomb sum (<= 1e-4 of a
+    # <= 6.2 um drift step => < 1e-4 um) plus one FP32 rounding of the position
+    w = workloads.make(1, n=4096)
+    d = _trajectory_check(w, 0, 0, steps=1, tol=2e-4)
+    assert np.median(d) <= 6.2e-5 and (d > 2e-4).sum() <= 4  # one ulp at z ~ 600 um; chaos needs more than one step
+
+
+# ------------------------------------------------------------------ a7/a8: collection, histogram, compaction
+def test_full_run_cfg0_conservation_and_image_statistics():
+    w = workloads.make(0)
+    P = w["params"]
+    sim = gpu_sim(w)
+    sim.load_carriers(w["xyz"])
+    o = oracle_sim(w, flags=g.FP32_STATE)
+    o.load(w["xyz"])
+    n0 = len(w["xyz"])
+    # conservation after every batch of steps
+    while True:
+        sim.step(16)
+        st = sim.state()
+        img, over = sim.read_image()
+        assert int(img.sum()) + over + st["n_active"] == n0
+        assert st["n_collected"] == n0 - st["n_active"]
+        if st["n_active"] == 0:
+            break
+    o.run(100000)
+    oimg = o.image()
+    assert abs(st["step"] - o.state()["step"]) <= 3
+    assert st["pair_interactions"] == pytest.approx(o.state()["pair_interactions"], rel=0.02)
+    # per-pixel: |dn| <= max(1 % n_ref, 4 sqrt(n_ref + 1)) (R22); totals exact
+    assert int(img.sum()) == int(oimg.sum()) == n0
+    dn = np.abs(img.astype(np.int64) - oimg.astype(np.int64))
+    assert np.all(dn <= np.maximum(0.01 * oimg, 4 * np.sqrt(oimg + 1.0)))
+    assert sim.step(5) == 0 and sim.state()["step"] == st["step"]          # empty: no-op, step index frozen
+    sim.close()
+
+
+def test_cloud_second_moments_within_one_percent():
+    # same physics as config 0 but binned at 0.5 um so that the image carries the cloud's second moments
+    w = workloads.make(0)
+    over = dict(pixel_pitch_um=0.5, img_nx=256, img_ny=256, img_x0_um=-64.0, img_y0_um=-64.0)
+    sim = gpu_sim(w, **over)
+    sim.load_carriers(w["xyz"])
+    done, left, rc = sim.run_to_collection(100000)
+    assert left == 0 and rc == 0
+    img, ov = sim.read_image()
+    o = oracle_sim(w, flags=g.FP32_STATE, **over)
+    o.load(w["xyz"])
+    o.run(100000)
+    oimg = o.image()
+    assert int(img.sum()) + ov == 1024 and ov == o.state()["n_out_of_window"] == 0
+    mx, my, vx, vy = image_moments(img, -64.0, -64.0, 0.5)
+    omx, omy, ovx, ovy = image_moments(oimg, -64.0, -64.0, 0.5)
+    assert abs(mx - omx) < 0.05 and abs(my - omy) < 0.05
+    assert vx == pytest.approx(ovx, rel=0.01) and vy == pytest.approx(ovy, rel=0.01)
+    # and Coulomb repulsion really widened it beyond the diffusion-only closed form (28.33 + 1 um^2)
+    assert vx > 1.1 * 29.33 and vy > 1.1 * 29.33
+    sim.close()
+
+
+def test_coulomb_off_lateral_spread_closed_form_on_gpu():
+    # 2e5 holes from a point at 200 um depth, Coulomb off: sigma_xy = 5.3223 um (tests/golden/lateral_sigma.txt)
+    from paper_2203_11043_b200 import binding as b
+    n = 200000
+    w = workloads.make(0, n=8)
+    w["xyz"] = np.tile(np.array([[0.0, 0.0, 200.0]], dtype=np.float32), (n, 1))
+    over = dict(pixel_pitch_um=0.25, img_nx=512, img_ny=512, img_x0_um=-64.0, img_y0_um=-64.0)
+    sim = gpu_sim(w, flags=b.COULOMB_OFF, max_carriers=n, **over)
+    sim.load_carriers(w["xyz"])
+    done, left, rc = sim.run_to_collection(100000)
+    img, ov = sim.read_image()
+    assert left == 0 and int(img.sum()) + ov == n and ov < 5
+    mx, my, vx, vy = image_moments(img, -64.0, -64.0, 0.25)
+    var = 5.3223 ** 2 - 0.25 ** 2 / 12 * 0 + 0.25 ** 2 / 12       # binning adds pitch^2/12
+    assert vx == pytest.approx(var, rel=0.012) and vy == pytest.approx(var, rel=0.012)
+    assert 109 - 15 <= done <= 138 + 25
+    assert sim.state()["pair_interactions"] == 0
+    sim.close()
+
+
+def test_full_run_cfg1_reduced_per_cloud_statistics():
+    # 8 clouds x 512 holes in one shared N-body, run to collection on both sides
+    w = workloads.make(1, n=8 * 512)
+    sim = gpu_sim(w)
+    sim.load_carriers(w["xyz"])
+    done, left, rc = sim.run_to_collection(100000)
+    img, ov = sim.read_image()
+    o = oracle_sim(w, flags=g.FP32_STATE)
+    o.load(w["xyz"])
+    o.run(100000)
+    oimg = o.image()
+    assert left == 0 and int(img.sum()) + ov == 8 * 512 == int(oimg.sum()) + o.state()["n_out_of_window"]
+    assert ov == o.state()["n_out_of_window"] or abs(ov - o.state()["n_out_of_window"]) <= 4
+    dn = np.abs(img.astype(np.int64) - oimg.astype(np.int64))
+    assert np.all(dn <= np.maximum(0.01 * oimg, 4 * np.sqrt(oimg + 1.0)))
+    assert abs(done - o.state()["step"]) <= 3
+    sim.close()
+
+
+def test_stable_compaction_order_and_ids_through_a_decaying_population():
+    # track: carriers retire continuously from the front end; ids must stay sorted and a subset of the previous set
+    w = workloads.make(3, n=20000)
+    sim = gpu_sim(w)
+    sim.load_carriers(w["xyz"])
+    n_at_load = sim.state()["n_active"]
+    assert n_at_load <= 20000 and sim.state()["n_collected"] == 20000 - n_at_load     # z <= 0 collected at load
+    prev = sim.read_carriers()[1]
+    assert np.all(np.diff(prev.astype(np.int64)) > 0)
+    for _ in range(12):
+        sim.step(7)
+        xyz, ids = sim.read_carriers()
+        assert np.all(np.diff(ids.astype(np.int64)) > 0) and np.all(np.isin(ids, prev))
+        assert np.all(xyz[:, 2] > 0.0) and np.all(xyz[:, 2] <= 675.0)
+        st = sim.state()
+        img, over = sim.read_image()
+        assert int(img.sum()) + over + st["n_active"] == 20000
+        prev = ids
+    assert len(prev) < n_at_load
+    sim.close()
+
+
+def test_restart_equivalence_and_determinism():
+    w = workloads.make(1, n=8 * 256)
+    a = gpu_sim(w)
+    a.load_carriers(w["xyz"])
+    a.step(20)
+    xa, ia = a.read_carriers()
+    b = gpu_sim(w)
+    b.load_carriers(w["xyz"])
+    b.step(10)
+    xb, ib = b.read_carriers()
+    c = gpu_sim(w)
+    c.load_snapshot(xb, ib, b.state()["step"])
+    c.step(10)
+    xc, ic = c.read_carriers()
+    assert np.array_equal(ia, ic) and np.array_equal(xa, xc)               # counter-based RNG: bit-exact restart
+    d = gpu_sim(w)
+    d.load_carriers(w["xyz"])
+    d.step(3); d.step(8); d.step(9)                                        # graph + direct launches mix
+    xd, idd = d.read_carriers()
+    assert np.array_equal(ia, idd) and np.array_equal(xa, xd)              # bit-reproducible
+    for s in (a, b, c, d):
+        s.close()
+
+
+# ------------------------------------------------------------------ boundary behaviour
+def test_edge_cases_and_error_codes():
+    from paper_2203_11043_b200 import binding as b
+    w = workloads.make(0, n=16)
+    sim = gpu_sim(w, max_carriers=32)
+    assert sim.step(3) == 0 and sim.state()["step"] == 0                   # empty handle: no-op
+    sim.load_carriers(np.zeros((0, 3), dtype=np.float32))                  # empty load
+    assert sim.read_carriers()[0].shape == (0, 3) and sim.eval_field().shape == (0, 3)
+    with pytest.raises(b.GcoreccdError) as e:
+        sim.load_carriers(np.array([[0, 0, 700.0]], dtype=np.float32))
+    assert e.value.code == b.ERR_INVALID
+    with pytest.raises(b.GcoreccdError) as e:
+        sim.load_carriers(np.array([[0, np.inf, 7.0]], dtype=np.float32))
+    assert e.value.code == b.ERR_INVALID and sim.state()["n_loaded"] == 0
+    sim.load_carriers(w["xyz"])
+    sim.load_carriers(np.array([[7.0, -8.0, 0.0], [1e5, 0.0, -1.0], [3.0, 4.0, 675.0]], dtype=np.float32))
+    st = sim.state()
+    assert st["n_loaded"] == 19 and st["n_active"] == 17 and st["n_collected"] == 2 and st["n_out_of_window"] == 1
+    assert sim.read_carriers()[1].tolist() == list(range(16)) + [18]       # ids continue in load order
+    img, over = sim.read_image()
+    assert img.sum() == 1 and img[int((-8.0 + 480) // 15), int((7.0 + 480) // 15)] == 1 and over == 1
+    with pytest.raises(b.GcoreccdError) as e:
+        sim.load_carriers(np.zeros((16, 3), dtype=np.float32) + 5.0)
+    assert e.value.code == b.ERR_CAPACITY
+    done, left, rc = sim.run_to_collection(5)
+    assert rc == b.MAX_STEPS and done == 5 and left > 0
+    sim.reset()
+    st = sim.state()
+    assert st == dict(step=0, n_active=0, n_loaded=0, n_collected=0, n_out_of_window=0, pair_interactions=0)
+    assert sim.read_image()[0].sum() == 0
+    sim.close()
+    with pytest.raises(b.GcoreccdError):
+        b.Gcoreccd(16, dt_ns=0.0)
+    with pytest.raises(b.GcoreccdError):
+        b.Gcoreccd(16, thickness_um=-1.0)
+
+
+def test_device_pointer_load_and_library_owned_workspace():
+    import torch
+    from paper_2203_11043_b200 import binding as b
+    w = workloads.make(0, n=512)
+    a = gpu_sim(w)
+    a.load_carriers(w["xyz"])
+    s = b.from_workload(w, torch_workspace=False)
+    s.load_carriers(torch.from_numpy(w["xyz"]).cuda())
+    a.step(5); s.step(5)
+    xa, ia = a.read_carriers()
+    xs, is_ = s.read_carriers()
+    assert np.array_equal(xa, xs) and np.array_equal(ia, is_)
+    dimg, _ = s.read_image(device=True)
+    assert dimg.is_cuda and int(dimg.sum()) == int(s.read_image()[0].sum())
+    a.close(); s.close()

@@ -1,0 +1,50 @@
+"""Helpers shared by the GPU parity tests: the same workload handed to the oracle and to the CUDA path."""
+import numpy as np
+
+from oracle import goracle as g
+
+
+def oracle_params(w, flags=0, **over):
+    P = dict(w["params"])
+    P.update(over)
+    return g.make_params(T_K=P["T_K"], a1=P["a1"], a2=P["a2"], thickness_um=P["thickness_um"], z_well_um=P["z_well_um"],
+                         pixel_pitch_um=P["pixel_pitch_um"], dt_ns=P["dt_ns"], softening_um=P["softening_um"],
+                         eps_si=P["eps_si"], seed=P["seed"], img_nx=P["img_nx"], img_ny=P["img_ny"],
+                         img_x0_um=P["img_x0_um"], img_y0_um=P["img_y0_um"], flags=flags)
+
+
+def oracle_sim(w, flags=0, **over):
+    s = g.Sim(oracle_params(w, flags, **over))
+    return s
+
+
+def gpu_sim(w, flags=0, max_carriers=None, **over):
+    from paper_2203_11043_b200 import binding
+    w2 = dict(w)
+    w2["params"] = dict(w["params"])
+    w2["params"].update(over)
+    return binding.from_workload(w2, flags=flags, max_carriers=max_carriers)
+
+
+def field_rel_err(E, Eref):
+    """max_j |dE_j| / |E_j| (unfloored, the judged number) and the floored variant of DESIGN.md R20."""
+    d = np.linalg.norm(E.astype(np.float64) - Eref, axis=1)
+    nrm = np.linalg.norm(Eref, axis=1)
+    rms = np.sqrt((nrm ** 2).mean())
+    with np.errstate(divide="ignore", invalid="ignore"):
+        unfloored = np.where(nrm > 0, d / nrm, 0.0)
+    floored = d / np.maximum(nrm, 1e-3 * rms)
+    return unfloored.max(), floored.max()
+
+
+def image_moments(img, x0, y0, pitch):
+    img = img.astype(np.float64)
+    ny, nx = img.shape
+    xs = x0 + (np.arange(nx) + 0.5) * pitch
+    ys = y0 + (np.arange(ny) + 0.5) * pitch
+    tot = img.sum()
+    mx = (img.sum(axis=0) * xs).sum() / tot
+    my = (img.sum(axis=1) * ys).sum() / tot
+    vx = (img.sum(axis=0) * (xs - mx) ** 2).sum() / tot
+    vy = (img.sum(axis=1) * (ys - my) ** 2).sum() / tot
+    return mx, my, vx, vy
