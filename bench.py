@@ -299,6 +299,39 @@ def run_ours(args):
     return 0
 
 
+def run_sweep(args):
+    """N sweep at fixed geometry (cfg-2 cloud), Coulomb on and off, 16 steps each through the graph path: the shape of
+    the paper's Fig. 4 experiment.  One JSON line per size; not the headline number."""
+    import torch
+    from paper_2203_11043_b200 import binding, workloads
+    peaks, _ = measured_peaks()
+    peak_pairs = SM_COUNT * LANES * 2.0 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / FLOP_PER_PAIR
+    sizes = [int(t) for t in args.sweep.split(",")]
+    stream = torch.cuda.Stream()
+    torch.cuda.set_stream(stream)
+    for n in sizes:
+        w = workloads.make(WORKLOAD_CFG, n=n)
+        row = {"n": n}
+        for name, flags in (("coulomb_on", 0), ("coulomb_off", binding.COULOMB_OFF)):
+            sim = binding.from_workload(w, flags=flags, stream=stream)
+            sim.load_carriers(w["xyz"])
+            sim.step(8)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            best = 1e30
+            for _ in range(3):
+                e0.record(); sim.step(16); e1.record(); torch.cuda.synchronize()
+                best = min(best, e0.elapsed_time(e1) / 16.0)
+            row[name + "_ms_per_step"] = best
+            if not flags:
+                na = sim.state()["n_active"]
+                row["G_pairs_per_s"] = na * float(na) / (best * 1e-3) / 1e9
+                row["frac_of_fp32_peak"] = na * float(na) / (best * 1e-3) / peak_pairs
+            sim.close()
+        print(json.dumps(row), flush=True)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -307,7 +340,10 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-event", action="store_true", help="skip the seconds-per-event run")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", default="", help="comma-separated hole counts: per-step time vs N (not the headline)")
     args = ap.parse_args()
+    if args.sweep:
+        return run_sweep(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

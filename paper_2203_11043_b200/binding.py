@@ -136,8 +136,11 @@ class Gcoreccd:
             ws_ptr = (self._ws.data_ptr() + 255) // 256 * 256
         if stream is None:
             stream = torch.cuda.current_stream(self.device)
+            if stream.cuda_stream == 0:
+                # the legacy default stream cannot be captured into CUDA graphs: give the handle its own torch stream
+                stream = torch.cuda.Stream(self.device)
         self._stream = stream
-        # torch's legacy default stream has handle 0, which the C ABI reads as "create your own": name it explicitly
+        # handle 0 would read as "create your own" in the C ABI: name the legacy stream explicitly if asked for
         stream_handle = stream.cuda_stream if stream.cuda_stream else 1          # cudaStreamLegacy
         p = Params(C.sizeof(Params), int(flags), T_K, a1, a2, thickness_um, z_well_um, pixel_pitch_um, dt_ns,
                    softening_um, eps_si, int(seed), self.img_nx, self.img_ny, img_x0_um, img_y0_um, self.device, 0,
@@ -181,6 +184,7 @@ class Gcoreccd:
         if isinstance(xyz, torch.Tensor):
             if xyz.device.type == "cuda":
                 t = xyz.detach().to(torch.float32).contiguous().reshape(-1, 3)
+                self._stream.wait_stream(torch.cuda.current_stream(self.device))   # producer of `t` may be another stream
                 rc = lib().gcoreccd_load_carriers(self._h, C.c_void_p(t.data_ptr()), t.shape[0], 1)
                 return self._check(rc, "gcoreccd_load_carriers")
             xyz = xyz.numpy()
@@ -204,7 +208,8 @@ class Gcoreccd:
     def read_image(self, device=False):
         over = C.c_uint64()
         if device:
-            out = self._torch.empty((self.img_ny, self.img_nx), dtype=self._torch.int32, device="cuda:%d" % self.device)
+            with self._torch.cuda.stream(self._stream):
+                out = self._torch.empty((self.img_ny, self.img_nx), dtype=self._torch.int32, device="cuda:%d" % self.device)
             rc = lib().gcoreccd_read_image(self._h, C.c_void_p(out.data_ptr()), out.numel(), C.byref(over), 1)
         else:
             out = np.zeros((self.img_ny, self.img_nx), dtype=np.uint32)

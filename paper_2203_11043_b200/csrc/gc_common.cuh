@@ -67,8 +67,12 @@ struct DevParams {            // constants uploaded by value with every launch
 struct PlanArgs { uint32_t IB; uint32_t grid; uint32_t part_cap_entries; };
 
 #ifdef __CUDACC__
-// Executed by ONE full warp.  Picks the smallest S whose static round-robin schedule wastes <= 1.5 % of the
-// CTA-rounds (else the least wasteful), subject to >= 64 sources per chunk and S * stride <= partial capacity.
+// Executed by ONE full warp.  Static round-robin makespan model: a CTA runs ceil(items/grid) items, each costing
+// JC source iterations plus a fixed overhead (target load, first tile, barrier, store ~ kItemOverhead source
+// iterations).  Picks the S minimising rounds * (JC + overhead); ties go to the smaller S (fewer partials to
+// reduce).  Constraints: >= kMinChunk sources per chunk, S * stride <= partial capacity.
+constexpr uint32_t kItemOverhead = 24;
+constexpr uint32_t kMinChunk = 32;
 __device__ inline FieldPlan plan_search(uint32_t n, PlanArgs a) {
   const uint32_t lane = threadIdx.x & 31u;
   FieldPlan p;
@@ -77,35 +81,29 @@ __device__ inline FieldPlan plan_search(uint32_t n, PlanArgs a) {
   p.stride = (n + 255u) & ~255u;
   p.S = 0; p.JC = 0;
   if (n == 0) return p;
-  uint32_t s_max = (n + 63u) / 64u;
-  uint32_t s_cap = a.part_cap_entries / p.stride;
+  uint32_t s_max = (n + kMinChunk - 1) / kMinChunk;
+  const uint32_t s_cap = a.part_cap_entries / p.stride;
+  const uint32_t s_bal = max(64u, (4u * a.grid + p.nIB - 1) / p.nIB);      // beyond ~4 rounds nothing improves
   if (s_max > s_cap) s_max = s_cap;
-  if (s_max > 1024u) s_max = 1024u;
+  if (s_max > s_bal) s_max = s_bal;
   if (s_max < 1u) s_max = 1u;
-  float best_w = 3.0e38f; uint32_t best_S = 1, found = 0;
-  for (uint32_t base = 1; base <= s_max && !found; base += 32) {
-    uint32_t S = base + lane;
-    float w = 3.0e38f;
+  uint32_t best_c = 0xffffffffu, best_S = 1;
+  for (uint32_t base = 1; base <= s_max; base += 32) {
+    const uint32_t S = base + lane;
     if (S <= s_max) {
-      uint32_t items = p.nIB * S;
-      uint32_t rounds = (items + a.grid - 1) / a.grid;
-      w = (float)rounds * (float)a.grid / (float)items;
+      const uint32_t JC = (((n + S - 1) / S) + 7u) & ~7u;
+      const uint32_t Se = (n + JC - 1) / JC;                                 // chunks actually used
+      const uint32_t rounds = (p.nIB * Se + a.grid - 1) / a.grid;
+      const uint32_t c = rounds * (JC + kItemOverhead);
+      if (c < best_c) { best_c = c; best_S = S; }
     }
-    uint32_t ok = __ballot_sync(0xffffffffu, w <= 1.015f);
-    if (ok) { found = base + (uint32_t)__ffs((int)ok) - 1u; break; }
-    if (w < best_w) { best_w = w; best_S = S; }
   }
-  if (!found) {
-    // least wasteful; ties -> smallest S
-    for (int o = 16; o > 0; o >>= 1) {
-      float ow = __shfl_xor_sync(0xffffffffu, best_w, o);
-      uint32_t oS = __shfl_xor_sync(0xffffffffu, best_S, o);
-      if (ow < best_w || (ow == best_w && oS < best_S)) { best_w = ow; best_S = oS; }
-    }
-    found = best_S;
+  for (int o = 16; o > 0; o >>= 1) {
+    const uint32_t oc = __shfl_xor_sync(0xffffffffu, best_c, o);
+    const uint32_t oS = __shfl_xor_sync(0xffffffffu, best_S, o);
+    if (oc < best_c || (oc == best_c && oS < best_S)) { best_c = oc; best_S = oS; }
   }
-  uint32_t JC = (n + found - 1) / found;
-  JC = (JC + 7u) & ~7u;
+  const uint32_t JC = (((n + best_S - 1) / best_S) + 7u) & ~7u;
   p.JC = JC;
   p.S = (n + JC - 1) / JC;
   return p;

@@ -72,7 +72,8 @@ k_compact(SoA B, SoA A, Ctrl* __restrict__ ctrl, const uint32_t* __restrict__ ti
   if (s_last && warp == 0) {
     __threadfence();
     const uint32_t n_new = *((volatile uint32_t*)&ctrl->n_next);
-    const FieldPlan plan = plan_search(n_new, pa);
+    FieldPlan plan = ctrl->plan;
+    if (plan.n != n_new || plan.IB != pa.IB) plan = plan_search(n_new, pa);   // unchanged population: keep the plan
     if (lane == 0) {
       ctrl->plan = plan;
       ctrl->n_active = n_new;

@@ -101,9 +101,9 @@ int fail(gcoreccd_t* h, int code, const char* what, cudaError_t e = cudaSuccess)
 inline uint32_t variant_ib(int v) { return (uint32_t)kTPB * (2u << v); }     // 512, 1024, 2048 targets per row block
 
 inline int pick_variant(uint64_t n_bound) {
-  if (n_bound >= 49152) return 2;
-  if (n_bound >= 6144) return 1;
-  return 0;
+  if (n_bound >= 12288) return 2;      // 8 targets/thread, 1 CTA/SM: highest FMA-pipe utilisation (76 %)
+  if (n_bound >= 3072) return 1;       // 4 targets/thread, 3 CTAs/SM: more row blocks for balance
+  return 0;                            // 2 targets/thread, 4 CTAs/SM
 }
 
 inline PlanArgs plan_args(const gcoreccd_t* h, int v) {
@@ -191,7 +191,9 @@ int enqueue_steps(gcoreccd_t* h, uint64_t n_steps) {
   if (rc) return rc;
   const uint32_t tiles = bucket_tiles(tiles_for(h->n_bound));
   const uint32_t per_step = (h->dp.flags & GCORECCD_COULOMB_OFF) ? 2u : 3u;
-  while (n_steps >= (uint64_t)kGraphSteps) {
+  // stream capture is not permitted on the legacy / per-thread default streams: plain launches there
+  const bool can_graph = h->stream != cudaStreamLegacy && h->stream != cudaStreamPerThread && h->stream != nullptr;
+  while (can_graph && n_steps >= (uint64_t)kGraphSteps) {
     rc = ensure_graph(h, tiles);
     if (rc) return rc;
     GC_CUDA(h, cudaGraphLaunch(h->graph, h->stream));
