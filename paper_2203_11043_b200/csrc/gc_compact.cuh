@@ -26,6 +26,11 @@ k_compact(SoA B, SoA A, Ctrl* __restrict__ ctrl, const uint32_t* __restrict__ ti
   const uint32_t n_tiles = (m + kTPB - 1) / kTPB;
 
   if (t < n_tiles) {
+    // this thread's carrier first: its loads overlap the tile_count reduction below (the kernel is latency bound)
+    const uint32_t i = t * kTPB + tid;
+    float x = 0.f, y = 0.f, z = 0.f; uint32_t id = 0;
+    if (i < m) { x = B.x[i]; y = B.y[i]; z = B.z[i]; id = B.id[i]; }
+    const bool keep = i < m && (double)z > z_well;
     // base = sum of survivor counts of tiles [0, t)
     uint32_t part = 0;
     for (uint32_t u = tid; u < t; u += kTPB) part += tile_count[u];
@@ -40,9 +45,6 @@ k_compact(SoA B, SoA A, Ctrl* __restrict__ ctrl, const uint32_t* __restrict__ ti
     __syncthreads();
     const uint32_t base = dst_off + s_base;
 
-    const uint32_t i = t * kTPB + tid;
-    float x = 0.f, y = 0.f, z = 0.f; uint32_t id = 0; bool keep = false;
-    if (i < m) { z = B.z[i]; keep = (double)z > z_well; if (keep) { x = B.x[i]; y = B.y[i]; id = B.id[i]; } }
     const uint32_t bal = __ballot_sync(0xffffffffu, keep);
     const uint32_t rank_in_warp = __popc(bal & ((1u << lane) - 1u));
     __syncthreads();                                      // s_red reuse

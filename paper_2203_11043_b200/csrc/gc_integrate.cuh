@@ -57,6 +57,27 @@ __device__ __forceinline__ void collect(float x, float y, const DevParams& P, ui
     n_over += 1u;
 }
 
+// Sum of the S column-chunk partials of one target, in FP64 and in fixed (ascending chunk) order.  The loads of
+// a batch of kRedBatch chunks are issued together before any is consumed: the loop is bound by L2 latency, and a
+// load -> convert -> add chain per chunk would serialise S round trips.
+constexpr int kRedBatch = 8;
+__device__ __forceinline__ void reduce_partials(const float* __restrict__ e, uint32_t part_cap, uint32_t S, uint32_t stride,
+                                                double& Ex, double& Ey, double& Ez) {
+  const float* ey = e + part_cap;
+  const float* ez = ey + part_cap;
+  for (uint32_t s0 = 0; s0 < S; s0 += kRedBatch) {
+    float vx[kRedBatch], vy[kRedBatch], vz[kRedBatch];
+#pragma unroll
+    for (int u = 0; u < kRedBatch; ++u) {
+      const bool ok = s0 + u < S;
+      const size_t o = (size_t)(s0 + u) * stride;
+      vx[u] = ok ? __ldg(e + o) : 0.f; vy[u] = ok ? __ldg(ey + o) : 0.f; vz[u] = ok ? __ldg(ez + o) : 0.f;
+    }
+#pragma unroll
+    for (int u = 0; u < kRedBatch; ++u) { Ex += (double)vx[u]; Ey += (double)vy[u]; Ez += (double)vz[u]; }
+  }
+}
+
 // Block-level tally of (collected, overflow) and the survivor count of this tile.
 __device__ __forceinline__ void tally(uint32_t coll, uint32_t over, uint32_t keep, Ctrl* ctrl, uint32_t* tile_count) {
   __shared__ uint32_t s_c[3];
@@ -79,7 +100,7 @@ __device__ __forceinline__ void tally(uint32_t coll, uint32_t over, uint32_t kee
 
 // One thread per carrier; tile = kTPB carriers; reads state A + partials, writes state B (same index) and
 // the tile's survivor count.  Grid is sized from the host's upper bound on n_active; surplus CTAs exit.
-__global__ void __launch_bounds__(kTPB)
+__global__ void __launch_bounds__(kTPB, 4)      // 64 registers: 4 CTAs/SM, 151,552 carriers in one wave on 148 SMs
 k_integrate(SoA A, SoA B, Ctrl* __restrict__ ctrl, const float* __restrict__ Ep, uint32_t part_cap,
             uint32_t* __restrict__ image, uint32_t* __restrict__ tile_count, DevParams P) {
   const uint32_t n = ctrl->n_active;
@@ -92,13 +113,7 @@ k_integrate(SoA A, SoA B, Ctrl* __restrict__ ctrl, const float* __restrict__ Ep,
     const uint32_t id = A.id[i];
     double Ex = 0.0, Ey = 0.0, Ez = 0.0;
     if (!(P.flags & 1u)) {                                   // GCORECCD_COULOMB_OFF
-      const uint32_t S = ctrl->plan.S, stride = ctrl->plan.stride;
-      const float* ex = Ep + i;
-      for (uint32_t s = 0; s < S; ++s) {                     // fixed order
-        Ex += (double)ex[(size_t)s * stride];
-        Ey += (double)ex[(size_t)s * stride + part_cap];
-        Ez += (double)ex[(size_t)s * stride + 2 * (size_t)part_cap];
-      }
+      reduce_partials(Ep + i, part_cap, ctrl->plan.S, ctrl->plan.stride, Ex, Ey, Ez);
       Ex *= -P.Kp; Ey *= -P.Kp; Ez *= -P.Kp;                 // partials hold sum (r_s - r_t) w
     }
     if (!(P.flags & 4u)) Ez += P.a1_um * (double)z - P.a2;   // eq. 1
@@ -155,13 +170,8 @@ k_field_finalize(const Ctrl* __restrict__ ctrl, const float* __restrict__ Ep, ui
   const uint32_t n = ctrl->n_active;
   const uint32_t i = blockIdx.x * kTPB + threadIdx.x;
   if (i >= n) return;
-  const uint32_t S = ctrl->plan.S, stride = ctrl->plan.stride;
   double Ex = 0.0, Ey = 0.0, Ez = 0.0;
-  for (uint32_t s = 0; s < S; ++s) {
-    Ex += (double)Ep[(size_t)s * stride + i];
-    Ey += (double)Ep[(size_t)s * stride + i + part_cap];
-    Ez += (double)Ep[(size_t)s * stride + i + 2 * (size_t)part_cap];
-  }
+  reduce_partials(Ep + i, part_cap, ctrl->plan.S, ctrl->plan.stride, Ex, Ey, Ez);
   out[3 * (size_t)i] = (float)(-Kp * Ex); out[3 * (size_t)i + 1] = (float)(-Kp * Ey); out[3 * (size_t)i + 2] = (float)(-Kp * Ez);
 }
 
