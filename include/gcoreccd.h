@@ -1,6 +1,7 @@
 /* gcoreccd.h — C ABI of the B200-native (sm_100a) hot path of G-CoReCCD (arXiv 2203.11043).
  *
- * One handle = one event (one set of mutually interacting holes) = one CUDA stream.
+ * One handle = one event (one set of mutually interacting holes) = one CUDA stream; or, through the
+ * *_events calls, one batch of independent small events advanced concurrently.
  * Per time step the library runs, entirely on the GPU and in this order (Fig. 2):
  *   a1  all-pairs softened Coulomb field of every still-drifting hole      (eq. 6)
  *   a2  + linear depletion field E(z) = a1 z - a2, total |E|               (eq. 1)
@@ -124,6 +125,37 @@ int gcoreccd_read_carriers(gcoreccd_t* h, float* xyz_um, uint32_t* id, uint64_t 
 /* Coulomb field (eq. 6, V/cm) of the current snapshot, interleaved Ex,Ey,Ez in read_carriers order;
  * does not advance the simulation.  cap = number of carriers the buffer holds. */
 int gcoreccd_eval_field(gcoreccd_t* h, float* Exyz_V_per_cm, uint64_t cap, int on_device);
+
+/* ---- Batched independent events --------------------------------------------------
+ * The paper's X-ray workload is many small clouds (N = E/3.77 eV holes per photon) whose
+ * holes repel each other only inside their own event, and its GPU is under-utilised below ~1e3 holes
+ * (PAPER.md:92).  A batch runs every event exactly as if it had been loaded alone into a fresh handle with the
+ * same parameters (same eq. 6 sum over the event's own holes, same a2..a8, same Philox stream keyed by
+ * (seed, carrier id, the EVENT's step index)), but all events advance concurrently: one thread block owns one
+ * event for its whole life, with the state in shared memory.  All events share the handle's image, counters and
+ * pair_interactions (sum over events and steps of n_event^2).
+ *
+ * load_events: event e owns carriers [event_offsets[e], event_offsets[e+1]) of xyz_um (interleaved x,y,z FP32,
+ *   host or device per on_device); event_offsets is a HOST array of n_events+1 non-decreasing entries starting
+ *   at 0.  Carrier ids continue the handle's load order (id = n_loaded + index).  An event may be empty; none
+ *   may exceed GCORECCD_EVENT_MAX_CARRIERS (CAPACITY; larger events belong in load_carriers), the total may not
+ *   exceed max_carriers (CAPACITY).  Non-finite coordinates or z > thickness => INVALID, nothing loaded.
+ *   Holes loaded at z <= z_well are collected when their event first runs.  STATE if the handle still holds
+ *   drifting carriers (single event or an unfinished batch).  Replaces a finished batch.  Synchronous.
+ * run_events: every unfinished event takes up to max_steps more steps (or runs to full collection).
+ *   Synchronous.  Returns OK when every hole is collected, MAX_STEPS (+1) otherwise; *events_left and
+ *   *carriers_left (host, may be NULL) receive what is still drifting.
+ * get_events: per-event drifting holes and step index as of the last run_events (host arrays of cap_events
+ *   entries, either may be NULL); *n_events receives the batch size.
+ * read_event_carriers: the drifting holes of one event (stable load order), host buffers, either may be NULL. */
+#define GCORECCD_EVENT_MAX_CARRIERS 4096
+int gcoreccd_load_events(gcoreccd_t* h, const float* xyz_um, const uint64_t* event_offsets_host, uint64_t n_events,
+                         int on_device);
+int gcoreccd_run_events(gcoreccd_t* h, uint64_t max_steps, uint64_t* events_left, uint64_t* carriers_left);
+int gcoreccd_get_events(gcoreccd_t* h, uint64_t* n_active_host, uint64_t* step_host, uint64_t cap_events,
+                        uint64_t* n_events);
+int gcoreccd_read_event_carriers(gcoreccd_t* h, uint64_t event, float* xyz_um_host, uint32_t* id_host, uint64_t cap,
+                                 uint64_t* n);
 
 /* Run ONE step with CUDA events between its kernels (on the handle's stream) and return the device time of
  * each in milliseconds: ms[0] field, ms[1] integrate+collect, ms[2] compact, ms[3] whole step.  Synchronous. */

@@ -19,6 +19,7 @@ COULOMB_OFF, DIFFUSION_OFF, DEPLETION_OFF = 1, 2, 4
 EXPORTS = ["gcoreccd_workspace_size", "gcoreccd_create", "gcoreccd_destroy", "gcoreccd_reset",
            "gcoreccd_load_carriers", "gcoreccd_load_snapshot", "gcoreccd_step", "gcoreccd_run_to_collection",
            "gcoreccd_read_image", "gcoreccd_get_state", "gcoreccd_read_carriers", "gcoreccd_eval_field",
+           "gcoreccd_load_events", "gcoreccd_run_events", "gcoreccd_get_events", "gcoreccd_read_event_carriers",
            "gcoreccd_profile_step", "gcoreccd_kernel_launches", "gcoreccd_debug_normals", "gcoreccd_strerror",
            "gcoreccd_last_error", "gcoreccd_version"]
 
@@ -81,6 +82,14 @@ def lib():
     L.gcoreccd_read_carriers.argtypes = [vp, vp, vp, C.c_uint64, u64p, C.c_int]
     L.gcoreccd_eval_field.restype = C.c_int
     L.gcoreccd_eval_field.argtypes = [vp, vp, C.c_uint64, C.c_int]
+    L.gcoreccd_load_events.restype = C.c_int
+    L.gcoreccd_load_events.argtypes = [vp, vp, u64p, C.c_uint64, C.c_int]
+    L.gcoreccd_run_events.restype = C.c_int
+    L.gcoreccd_run_events.argtypes = [vp, C.c_uint64, u64p, u64p]
+    L.gcoreccd_get_events.restype = C.c_int
+    L.gcoreccd_get_events.argtypes = [vp, u64p, u64p, C.c_uint64, u64p]
+    L.gcoreccd_read_event_carriers.restype = C.c_int
+    L.gcoreccd_read_event_carriers.argtypes = [vp, C.c_uint64, vp, vp, C.c_uint64, u64p]
     L.gcoreccd_profile_step.restype = C.c_int
     L.gcoreccd_profile_step.argtypes = [vp, fp]
     L.gcoreccd_kernel_launches.restype = C.c_uint64
@@ -216,6 +225,55 @@ class Gcoreccd:
             rc = lib().gcoreccd_read_image(self._h, C.c_void_p(out.ctypes.data), out.size, C.byref(over), 0)
         self._check(rc, "gcoreccd_read_image")
         return out, int(over.value)
+
+    # ---- batched independent events (one thread block per event)
+    def load_events(self, xyz, offsets):
+        """xyz: (n,3) float32 numpy (host) or torch CUDA tensor; offsets: n_events+1 non-decreasing, offsets[0] = 0."""
+        torch = self._torch
+        off = np.ascontiguousarray(offsets, dtype=np.uint64)
+        offp = off.ctypes.data_as(C.POINTER(C.c_uint64))
+        if isinstance(xyz, torch.Tensor) and xyz.device.type == "cuda":
+            t = xyz.detach().to(torch.float32).contiguous().reshape(-1, 3)
+            self._stream.wait_stream(torch.cuda.current_stream(self.device))
+            rc = lib().gcoreccd_load_events(self._h, C.c_void_p(t.data_ptr()), offp, len(off) - 1, 1)
+        else:
+            a = np.ascontiguousarray(xyz, dtype=np.float32).reshape(-1, 3)
+            rc = lib().gcoreccd_load_events(self._h, C.c_void_p(a.ctypes.data), offp, len(off) - 1, 0)
+        return self._check(rc, "gcoreccd_load_events")
+
+    def load_events_ptr(self, host_ptr, offsets):
+        off = np.ascontiguousarray(offsets, dtype=np.uint64)
+        rc = lib().gcoreccd_load_events(self._h, C.c_void_p(int(host_ptr)), off.ctypes.data_as(C.POINTER(C.c_uint64)),
+                                        len(off) - 1, 0)
+        return self._check(rc, "gcoreccd_load_events")
+
+    def run_events(self, max_steps=10 ** 9):
+        ev, ca = C.c_uint64(), C.c_uint64()
+        rc = self._check(lib().gcoreccd_run_events(self._h, int(max_steps), C.byref(ev), C.byref(ca)), "gcoreccd_run_events")
+        return int(ev.value), int(ca.value), rc
+
+    def events(self):
+        n = C.c_uint64()
+        self._check(lib().gcoreccd_get_events(self._h, None, None, 0, C.byref(n)), "gcoreccd_get_events")
+        k = int(n.value)
+        act = np.zeros(k, dtype=np.uint64)
+        stp = np.zeros(k, dtype=np.uint64)
+        self._check(lib().gcoreccd_get_events(self._h, act.ctypes.data_as(C.POINTER(C.c_uint64)),
+                                              stp.ctypes.data_as(C.POINTER(C.c_uint64)), k, C.byref(n)), "gcoreccd_get_events")
+        return act, stp
+
+    def read_event_carriers(self, event):
+        n = C.c_uint64()
+        self._check(lib().gcoreccd_read_event_carriers(self._h, int(event), None, None, 0, C.byref(n)),
+                    "gcoreccd_read_event_carriers")
+        k = int(n.value)
+        xyz = np.zeros((k, 3), dtype=np.float32)
+        ids = np.zeros(k, dtype=np.uint32)
+        if k:
+            self._check(lib().gcoreccd_read_event_carriers(self._h, int(event), C.c_void_p(xyz.ctypes.data),
+                                                           C.c_void_p(ids.ctypes.data), k, C.byref(n)),
+                        "gcoreccd_read_event_carriers")
+        return xyz, ids
 
     # ---- introspection / test hooks
     def state(self):

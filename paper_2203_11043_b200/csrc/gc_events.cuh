@@ -1,0 +1,230 @@
+// gc_events.cuh — batched independent events: the paper's X-ray workload is MANY small
+// clouds (tens to thousands of holes each) whose holes interact only inside their own event,
+// and its GPU is "under-utilised" below ~1e3 holes because every step is a train of launches.
+//
+// B200 design: ONE CTA OWNS ONE EVENT FOR ITS WHOLE LIFE.  The event's state lives in shared memory (up to
+// 4,096 holes = 176 KB of the SM's 227 KB), already in the pre-duplicated (x,x,y,y)/(z,z) layout the packed
+// field loop consumes; all eight rows a1..a8 of a time step run inside the CTA with two block barriers per
+// step and no global-memory traffic except the integer histogram atomics of collected holes.  A persistent
+// grid pulls events from a queue (largest first), so hundreds of events are in flight and the FP32 pipes see
+// the same packed inner loop as k_field — with zero launches and zero HBM round trips per step.
+//
+// Per step inside the CTA (PAPER.md:68 order, identical arithmetic to k_field / k_integrate / k_compact):
+//   field + integrate:  thread t owns targets {pass*2*NPACK*TPB + (p*TPB + t)*2 + {0,1}}; it sums eq. 6 over all
+//                       sources from shared memory (two-level FP32 accumulation: 256-source tile partials flushed
+//                       into a total), then advances each of its targets in FP64 (advance_carrier) into s_next;
+//   collect + compact:  each thread takes a contiguous run of s_next, bins the holes with z <= z_well into the
+//                       image, block-scans the survivor counts and writes the survivors back, in order (stable),
+//                       into the duplicated layout.  step += 1, pairs += n^2.
+#pragma once
+#include "gc_common.cuh"
+#include "gc_field.cuh"
+#include "gc_integrate.cuh"
+
+namespace gc {
+
+struct EventTable {            // device arrays, one entry per event
+  const uint32_t* off;         // first slot of the event in the state arrays (fixed at load)
+  uint32_t* cnt;               // holes still drifting, compacted at [off, off + cnt)
+  uint64_t* step;              // steps taken so far = index of the event's next step (Philox counter)
+};
+
+constexpr uint32_t kEvCapSmall = 512;      // NPACK = 1 variant: one pass covers 512 targets, several CTAs per SM
+constexpr uint32_t kEvCapLarge = 4096;     // NPACK = 4 variant: 2,048 targets per pass, one CTA per SM
+
+__host__ __device__ constexpr size_t event_smem_bytes(uint32_t cap) {
+  // s_xy float4[cap+4] | s_next float4[cap] | s_z float2[cap+4] | s_id u32[cap]
+  return (size_t)(cap + 4) * 16 + (size_t)cap * 16 + (size_t)(cap + 4) * 8 + (size_t)cap * 4;
+}
+
+// Field of NP packs of this thread against all n sources in shared memory; returns sum (r_s - r_t) w per target.
+template <int NP>
+__device__ __forceinline__ void event_field(const float4* __restrict__ s_xy, const float2* __restrict__ s_z, uint32_t n,
+                                            uint32_t i_first, const float2 eps2v, float2 (&tx)[NP], float2 (&ty)[NP],
+                                            float2 (&tz)[NP]) {
+  float2 ntx[NP], nty[NP], ntz[NP];
+#pragma unroll
+  for (int p = 0; p < NP; ++p) {
+    const uint32_t i0 = i_first + (uint32_t)p * (2u * kTPB);
+    // slots >= n hold sentinels or stale data: keep them out of the arithmetic (their result is never used)
+    const bool v0 = i0 < n, v1 = i0 + 1 < n;
+    const float4 a0 = s_xy[v0 ? i0 : 0], a1 = s_xy[v1 ? i0 + 1 : 0];
+    const float2 b0 = s_z[v0 ? i0 : 0], b1 = s_z[v1 ? i0 + 1 : 0];
+    ntx[p] = make_float2(-a0.x, -a1.x); nty[p] = make_float2(-a0.z, -a1.z); ntz[p] = make_float2(-b0.x, -b1.x);
+    tx[p] = make_float2(0.f, 0.f); ty[p] = tx[p]; tz[p] = tx[p];
+  }
+  for (uint32_t jt = 0; jt < n; jt += kTile) {
+    const int len = (int)min((uint32_t)kTile, (n - jt + 3u) & ~3u);      // tail padded to the unroll factor with sentinels
+    float2 ax[NP], ay[NP], az[NP];
+#pragma unroll
+    for (int p = 0; p < NP; ++p) { ax[p] = make_float2(0.f, 0.f); ay[p] = ax[p]; az[p] = ax[p]; }
+    const float4* sxy = s_xy + jt;
+    const float2* sz = s_z + jt;
+#pragma unroll 4
+    for (int jj = 0; jj < len; ++jj) interact<NP>(sxy[jj], sz[jj], ntx, nty, ntz, eps2v, ax, ay, az);
+#pragma unroll
+    for (int p = 0; p < NP; ++p) {
+      tx[p] = __fadd2_rn(tx[p], ax[p]); ty[p] = __fadd2_rn(ty[p], ay[p]); tz[p] = __fadd2_rn(tz[p], az[p]);
+    }
+  }
+}
+
+// a2..a6 for the 2 NP targets of this thread, results into s_next (x', y', z', id).
+template <int NP>
+__device__ __forceinline__ void event_advance(const float4* __restrict__ s_xy, const float2* __restrict__ s_z,
+                                              const uint32_t* __restrict__ s_id, float4* __restrict__ s_next, uint32_t n,
+                                              uint32_t i_first, uint64_t step, const float2 (&tx)[NP], const float2 (&ty)[NP],
+                                              const float2 (&tz)[NP], const DevParams& P, uint32_t& nonfinite) {
+#pragma unroll
+  for (int p = 0; p < NP; ++p) {
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const uint32_t i = i_first + (uint32_t)p * (2u * kTPB) + (uint32_t)h;
+      if (i < n) {
+        const float x = s_xy[i].x, y = s_xy[i].z, z = s_z[i].x;
+        const uint32_t id = s_id[i];
+        // partials hold sum (r_s - r_t) w = -S_t
+        const double Ex = -P.Kp * (double)(h ? tx[p].y : tx[p].x), Ey = -P.Kp * (double)(h ? ty[p].y : ty[p].x),
+                     Ez = -P.Kp * (double)(h ? tz[p].y : tz[p].x);
+        float xf, yf, zf;
+        if (!advance_carrier(x, y, z, id, step, Ex, Ey, Ez, P, xf, yf, zf)) nonfinite = 1u;
+        s_next[i] = make_float4(xf, yf, zf, __uint_as_float(id));
+      }
+    }
+  }
+}
+
+template <int NP>
+__device__ __forceinline__ void event_pass(const float4* s_xy, const float2* s_z, const uint32_t* s_id, float4* s_next,
+                                           uint32_t n, uint32_t i_first, uint64_t step, const DevParams& P, uint32_t& nonfinite) {
+  float2 tx[NP], ty[NP], tz[NP];
+  if (!(P.flags & 1u)) {                                     // GCORECCD_COULOMB_OFF
+    event_field<NP>(s_xy, s_z, n, i_first, make_float2(P.eps2, P.eps2), tx, ty, tz);
+  } else {
+#pragma unroll
+    for (int p = 0; p < NP; ++p) { tx[p] = make_float2(0.f, 0.f); ty[p] = tx[p]; tz[p] = tx[p]; }
+  }
+  event_advance<NP>(s_xy, s_z, s_id, s_next, n, i_first, step, tx, ty, tz, P, nonfinite);
+}
+
+// Persistent grid; CTA loop: take the next event of `order[0..n_order)`, run it for up to max_steps more steps
+// (or to full collection), store the survivors back.  cap = holes the dynamic shared memory is sized for.
+template <int NPACK, int MINB>                 // NPACK is 1 (small events) or 4 (large events)
+__global__ void __launch_bounds__(kTPB, MINB)
+k_events(SoA A, EventTable ev, const uint32_t* __restrict__ order, uint32_t n_order, uint32_t* __restrict__ queue,
+         Ctrl* __restrict__ ctrl, uint32_t* __restrict__ image, DevParams P, uint64_t max_steps, uint32_t cap) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  float4* s_xy = reinterpret_cast<float4*>(smem);                       // (x,x,y,y), cap + 4 entries
+  float4* s_next = s_xy + (cap + 4);                                    // (x',y',z',id), cap entries
+  float2* s_z = reinterpret_cast<float2*>(s_next + cap);                // (z,z), cap + 4 entries
+  uint32_t* s_id = reinterpret_cast<uint32_t*>(s_z + (cap + 4));        // cap entries
+  __shared__ uint32_t s_warp[kTPB / 32];
+  __shared__ uint32_t s_ev, s_coll, s_over;
+
+  const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+  constexpr uint32_t kPass = 2u * NPACK * kTPB;                          // targets per pass
+  uint32_t nonfinite = 0;
+
+  for (;;) {
+    __syncthreads();                                                    // previous event fully retired
+    if (tid == 0) { s_ev = atomicAdd(queue, 1u); s_coll = 0; s_over = 0; }
+    __syncthreads();
+    if (s_ev >= n_order) break;
+    const uint32_t e = order[s_ev];
+    const uint32_t off = ev.off[e];
+    uint32_t n = ev.cnt[e];
+    uint64_t step = ev.step[e];
+    if (n == 0) continue;
+    for (uint32_t i = tid; i < n; i += kTPB)
+      s_next[i] = make_float4(A.x[off + i], A.y[off + i], A.z[off + i], __uint_as_float(A.id[off + i]));
+    __syncthreads();
+
+    uint64_t pairs = 0, done = 0;
+    bool first = true;
+    for (;;) {
+      // ---- a7 + a8: bin the holes that crossed z_well, compact the survivors (stable) into the field layout
+      const uint32_t per = (n + kTPB - 1) / kTPB;
+      const uint32_t lo = min(tid * per, n), hi = min(lo + per, n);
+      uint32_t keep = 0, coll = 0, over = 0;
+      for (uint32_t i = lo; i < hi; ++i) {
+        const float4 c = s_next[i];
+        if ((double)c.z <= P.z_well) { coll += 1; collect(c.x, c.y, P, image, over); }
+        else keep += 1;
+      }
+      uint32_t incl = keep;                                             // block exclusive scan of the survivor counts
+      for (int o = 1; o < 32; o <<= 1) { const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o); if ((int)lane >= o) incl += v; }
+      if (lane == 31) s_warp[warp] = incl;
+      const uint32_t wc = __reduce_add_sync(0xffffffffu, coll), wo = __reduce_add_sync(0xffffffffu, over);
+      if (lane == 0 && wc) { atomicAdd(&s_coll, wc); if (wo) atomicAdd(&s_over, wo); }
+      __syncthreads();
+      uint32_t base = 0, total = 0;
+#pragma unroll
+      for (int w = 0; w < kTPB / 32; ++w) { const uint32_t v = s_warp[w]; if (w < (int)warp) base += v; total += v; }
+      uint32_t o = base + incl - keep;
+      for (uint32_t i = lo; i < hi; ++i) {
+        const float4 c = s_next[i];
+        if ((double)c.z > P.z_well) {
+          s_xy[o] = make_float4(c.x, c.x, c.y, c.y); s_z[o] = make_float2(c.z, c.z); s_id[o] = __float_as_uint(c.w);
+          ++o;
+        }
+      }
+      if (tid < 4) {                                                    // sentinels up to the unroll factor
+        const uint32_t k = total + tid;
+        if (k < ((total + 3u) & ~3u)) { s_xy[k] = make_float4(kSentinel, kSentinel, kSentinel, kSentinel); s_z[k] = make_float2(kSentinel, kSentinel); }
+      }
+      if (!first) { step += 1; done += 1; if (!(P.flags & 1u)) pairs += (uint64_t)n * (uint64_t)n; }
+      first = false;
+      n = total;
+      __syncthreads();
+      if (n == 0 || done >= max_steps) break;
+
+      // ---- a1..a6: field of every hole of the event, then its Euler-Maruyama update, into s_next
+      for (uint32_t base_i = 0; base_i < n; base_i += kPass) {
+        const uint32_t i_first = base_i + tid * 2u;                     // pack p adds p * 2 * kTPB
+        const uint32_t w_first = base_i + warp * 64u;                   // first target of this warp in pack 0
+        if (w_first >= n) continue;                                     // warp-uniform
+        const uint32_t np = min((uint32_t)NPACK, (n - w_first + 2u * kTPB - 1u) / (2u * kTPB));   // packs with a live target
+        if constexpr (NPACK == 1) {
+          event_pass<1>(s_xy, s_z, s_id, s_next, n, i_first, step, P, nonfinite);
+        } else {
+          if (np == 1) event_pass<1>(s_xy, s_z, s_id, s_next, n, i_first, step, P, nonfinite);
+          else if (np == 2) event_pass<2>(s_xy, s_z, s_id, s_next, n, i_first, step, P, nonfinite);
+          else if (np == 3) event_pass<3>(s_xy, s_z, s_id, s_next, n, i_first, step, P, nonfinite);
+          else event_pass<4>(s_xy, s_z, s_id, s_next, n, i_first, step, P, nonfinite);
+        }
+      }
+      __syncthreads();
+    }
+
+    // ---- retire: survivors (if max_steps stopped the event early) back to the state arrays, counters out
+    for (uint32_t i = tid; i < n; i += kTPB) {
+      A.x[off + i] = s_xy[i].x; A.y[off + i] = s_xy[i].z; A.z[off + i] = s_z[i].x; A.id[off + i] = s_id[i];
+    }
+    if (tid == 0) {
+      ev.cnt[e] = n;
+      ev.step[e] = step;
+      if (s_coll) atomicAdd((unsigned long long*)&ctrl->n_collected, (unsigned long long)s_coll);
+      if (s_over) atomicAdd((unsigned long long*)&ctrl->n_overflow, (unsigned long long)s_over);
+      if (pairs) atomicAdd((unsigned long long*)&ctrl->pairs, (unsigned long long)pairs);
+    }
+  }
+  if (nonfinite) atomicOr(&ctrl->nonfinite, 1u);
+}
+
+// read_event_carriers: one event's survivors, SoA -> interleaved xyz
+__global__ void __launch_bounds__(kTPB)
+k_interleave_range(SoA A, uint32_t off, uint32_t n, float* __restrict__ xyz) {
+  const uint32_t i = blockIdx.x * kTPB + threadIdx.x;
+  if (i >= n) return;
+  xyz[3 * (size_t)i] = A.x[off + i]; xyz[3 * (size_t)i + 1] = A.y[off + i]; xyz[3 * (size_t)i + 2] = A.z[off + i];
+}
+
+// Load path of the batch: interleaved xyz -> state arrays at the same index, ids id_base + index.
+__global__ void __launch_bounds__(kTPB)
+k_unpack_events(const float* __restrict__ xyz, uint32_t n, SoA A, uint32_t id_base) {
+  const uint32_t i = blockIdx.x * kTPB + threadIdx.x;
+  if (i >= n) return;
+  A.x[i] = xyz[3 * (size_t)i]; A.y[i] = xyz[3 * (size_t)i + 1]; A.z[i] = xyz[3 * (size_t)i + 2]; A.id[i] = id_base + i;
+}
+
+}  // namespace gc

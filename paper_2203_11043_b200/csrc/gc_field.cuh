@@ -30,6 +30,30 @@ __device__ __forceinline__ float rsqrt_ftz(float x) {
   return y;
 }
 
+// One source against NP packs (2 NP targets): the 11 packed FP32 instructions + 2 MUFU.RSQ of eq. 6.
+// sxy = (x,x,y,y), sz = (z,z) of the source; nt* = negated target coordinates; a* += (r_s - r_t) / (r^2+eps^2)^{3/2}.
+template <int NP>
+__device__ __forceinline__ void interact(const float4 sxy, const float2 sz, const float2 (&ntx)[NP], const float2 (&nty)[NP],
+                                         const float2 (&ntz)[NP], const float2 eps2v, float2 (&ax)[NP], float2 (&ay)[NP],
+                                         float2 (&az)[NP]) {
+  const float2 sx2 = make_float2(sxy.x, sxy.y), sy2 = make_float2(sxy.z, sxy.w);
+#pragma unroll
+  for (int p = 0; p < NP; ++p) {
+    const float2 dx = __fadd2_rn(sx2, ntx[p]);
+    const float2 dy = __fadd2_rn(sy2, nty[p]);
+    const float2 dz = __fadd2_rn(sz, ntz[p]);
+    float2 r2 = __ffma2_rn(dx, dx, eps2v);
+    r2 = __ffma2_rn(dy, dy, r2);
+    r2 = __ffma2_rn(dz, dz, r2);
+    const float2 inv = make_float2(rsqrt_ftz(r2.x), rsqrt_ftz(r2.y));
+    float2 w = __fmul2_rn(inv, inv);
+    w = __fmul2_rn(w, inv);
+    ax[p] = __ffma2_rn(dx, w, ax[p]);
+    ay[p] = __ffma2_rn(dy, w, ay[p]);
+    az[p] = __ffma2_rn(dz, w, az[p]);
+  }
+}
+
 template <int NPACK, int TPB>
 struct FieldCfg {
   static constexpr int kTargetsPerThread = 2 * NPACK;
@@ -107,24 +131,7 @@ k_field(const float* __restrict__ px, const float* __restrict__ py, const float*
 
 #pragma unroll UNROLL
       for (int jj = 0; jj < len; ++jj) {
-        const float4 a = s_xy[buf][jj];
-        const float2 b = s_z[buf][jj];
-        const float2 sx2 = make_float2(a.x, a.y), sy2 = make_float2(a.z, a.w);
-#pragma unroll
-        for (int p = 0; p < NPACK; ++p) {
-          const float2 dx = __fadd2_rn(sx2, ntx[p]);
-          const float2 dy = __fadd2_rn(sy2, nty[p]);
-          const float2 dz = __fadd2_rn(b, ntz[p]);
-          float2 r2 = __ffma2_rn(dx, dx, eps2v);
-          r2 = __ffma2_rn(dy, dy, r2);
-          r2 = __ffma2_rn(dz, dz, r2);
-          const float2 inv = make_float2(rsqrt_ftz(r2.x), rsqrt_ftz(r2.y));
-          float2 w = __fmul2_rn(inv, inv);
-          w = __fmul2_rn(w, inv);
-          ax[p] = __ffma2_rn(dx, w, ax[p]);
-          ay[p] = __ffma2_rn(dy, w, ay[p]);
-          az[p] = __ffma2_rn(dz, w, az[p]);
-        }
+        interact<NPACK>(s_xy[buf][jj], s_z[buf][jj], ntx, nty, ntz, eps2v, ax, ay, az);
       }
       // flush the tile partial into the chunk total (two-level accumulation)
 #pragma unroll

@@ -78,6 +78,28 @@ __device__ __forceinline__ void reduce_partials(const float* __restrict__ e, uin
   }
 }
 
+// a2..a6 for one carrier: (Ex,Ey,Ez) is its Coulomb field in V/cm (eq. 6); returns the new FP32 position, i.e. the
+// correctly rounded value of the FP64 expression the oracle evaluates.  False if the result is not finite.
+__device__ __forceinline__ bool advance_carrier(float x, float y, float z, uint32_t id, uint64_t step, double Ex, double Ey,
+                                                double Ez, const DevParams& P, float& xf, float& yf, float& zf) {
+  if (!(P.flags & 4u)) Ez += P.a1_um * (double)z - P.a2;     // eq. 1
+  const double Emag = sqrt(Ex * Ex + Ey * Ey + Ez * Ez);
+  const double mu = mobility(Emag, P);                       // eq. 2
+  const double kd = P.drift_k * mu;                          // 1e-5 mu dt
+  double dx = kd * Ex, dy = kd * Ey, dz = kd * Ez;
+  if (!(P.flags & 2u)) {                                     // eqs. 3-4
+    double nrm[3];
+    philox_normals(P.seed_lo, P.seed_hi, id, step, nrm, nullptr);
+    const double sigma = sqrt(P.sigma_k * mu);
+    dx += sigma * nrm[0]; dy += sigma * nrm[1]; dz += sigma * nrm[2];
+  }
+  const double xn = (double)x + dx, yn = (double)y + dy;
+  double zn = (double)z + dz;
+  if (zn > P.thickness) zn = 2.0 * P.thickness - zn;         // specular back surface
+  xf = (float)xn; yf = (float)yn; zf = (float)zn;
+  return isfinite(xf) && isfinite(yf) && isfinite(zf);
+}
+
 // Block-level tally of (collected, overflow) and the survivor count of this tile.
 __device__ __forceinline__ void tally(uint32_t coll, uint32_t over, uint32_t keep, Ctrl* ctrl, uint32_t* tile_count) {
   __shared__ uint32_t s_c[3];
@@ -116,22 +138,8 @@ k_integrate(SoA A, SoA B, Ctrl* __restrict__ ctrl, const float* __restrict__ Ep,
       reduce_partials(Ep + i, part_cap, ctrl->plan.S, ctrl->plan.stride, Ex, Ey, Ez);
       Ex *= -P.Kp; Ey *= -P.Kp; Ez *= -P.Kp;                 // partials hold sum (r_s - r_t) w
     }
-    if (!(P.flags & 4u)) Ez += P.a1_um * (double)z - P.a2;   // eq. 1
-    const double Emag = sqrt(Ex * Ex + Ey * Ey + Ez * Ez);
-    const double mu = mobility(Emag, P);                     // eq. 2
-    const double kd = P.drift_k * mu;                        // 1e-5 mu dt
-    double dx = kd * Ex, dy = kd * Ey, dz = kd * Ez;
-    if (!(P.flags & 2u)) {                                   // eqs. 3-4
-      double nrm[3];
-      philox_normals(P.seed_lo, P.seed_hi, id, step, nrm, nullptr);
-      const double sigma = sqrt(P.sigma_k * mu);
-      dx += sigma * nrm[0]; dy += sigma * nrm[1]; dz += sigma * nrm[2];
-    }
-    const double xn = (double)x + dx, yn = (double)y + dy;
-    double zn = (double)z + dz;
-    if (zn > P.thickness) zn = 2.0 * P.thickness - zn;       // specular back surface
-    const float xf = (float)xn, yf = (float)yn, zf = (float)zn;
-    if (!(isfinite(xf) && isfinite(yf) && isfinite(zf))) atomicOr(&ctrl->nonfinite, 1u);
+    float xf, yf, zf;
+    if (!advance_carrier(x, y, z, id, step, Ex, Ey, Ez, P, xf, yf, zf)) atomicOr(&ctrl->nonfinite, 1u);
     B.x[i] = xf; B.y[i] = yf; B.z[i] = zf; B.id[i] = id;
     if ((double)zf <= P.z_well) { coll = 1; uint32_t o = 0; collect(xf, yf, P, image, o); over = o; }
     else keep = 1;

@@ -7,9 +7,12 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <algorithm>
+#include <cstdlib>
 
 #include "gc_common.cuh"
 #include "gc_compact.cuh"
+#include "gc_events.cuh"
 #include "gc_field.cuh"
 #include "gc_integrate.cuh"
 
@@ -71,6 +74,19 @@ struct gcoreccd {
   uint32_t graph_tiles;
   cudaEvent_t ev[4];
   char err[256];
+  // batched independent events (gc_events.cuh)
+  struct {
+    bool loaded;
+    uint64_t n_events, n_carriers;        // as loaded
+    uint64_t events_left, carriers_left;  // after the last run_events
+    uint32_t n_small, n_large;            // events per queue (order = [small..., large...], each largest first)
+    char* d_buf;                          // one allocation: off | cnt | order | queue | step
+    uint32_t *d_off, *d_cnt, *d_order, *d_queue;
+    uint64_t* d_step;
+    uint32_t *h_off, *h_cnt;              // host mirrors
+    uint64_t* h_step;
+    int grid_small, grid_large;
+  } evb;
 };
 
 namespace {
@@ -205,6 +221,14 @@ int enqueue_steps(gcoreccd_t* h, uint64_t n_steps) {
   return 0;
 }
 
+void drop_events(gcoreccd_t* h) {
+  if (h->evb.d_buf) cudaFree(h->evb.d_buf);
+  free(h->evb.h_off); free(h->evb.h_cnt); free(h->evb.h_step);
+  memset(&h->evb, 0, sizeof(h->evb));
+}
+
+inline bool events_busy(const gcoreccd_t* h) { return h->evb.loaded && h->evb.carriers_left > 0; }
+
 }  // namespace
 
 // ------------------------------------------------------------------------------------------------ C ABI
@@ -322,6 +346,7 @@ int gcoreccd_destroy(gcoreccd_t* h) {
   DeviceGuard guard(h->device);
   if (h->stream) cudaStreamSynchronize(h->stream);
   drop_graph(h);
+  drop_events(h);
   for (int k = 0; k < 4; ++k) if (h->ev[k]) cudaEventDestroy(h->ev[k]);
   if (h->h_ctrl) cudaFreeHost(h->h_ctrl);
   if (h->own_stream && h->stream) cudaStreamDestroy(h->stream);
@@ -336,6 +361,7 @@ int gcoreccd_reset(gcoreccd_t* h) {
   GC_CUDA(h, cudaMemsetAsync(h->ctrl, 0, sizeof(Ctrl), h->stream));
   GC_CUDA(h, cudaMemsetAsync(h->image, 0, (size_t)h->p.img_nx * h->p.img_ny * 4, h->stream));
   GC_CUDA(h, cudaStreamSynchronize(h->stream));
+  drop_events(h);
   h->n_loaded = 0;
   h->n_bound = 0;
   h->variant = -1;
@@ -346,6 +372,7 @@ int gcoreccd_reset(gcoreccd_t* h) {
 int gcoreccd_load_carriers(gcoreccd_t* h, const float* xyz, uint64_t n, int on_device) {
   if (!h || (!xyz && n)) return GCORECCD_ERR_INVALID;
   if (n == 0) return GCORECCD_OK;
+  if (events_busy(h)) return fail(h, GCORECCD_ERR_STATE, "load_carriers: a batch of events is still drifting (run_events or reset first)");
   DeviceGuard guard(h->device);
   int rc = sync_ctrl(h);
   if (rc) return rc;
@@ -382,6 +409,7 @@ int gcoreccd_load_carriers(gcoreccd_t* h, const float* xyz, uint64_t n, int on_d
 int gcoreccd_load_snapshot(gcoreccd_t* h, const float* xyz, const uint32_t* id, uint64_t n, uint64_t step) {
   if (!h || ((!xyz || !id) && n)) return GCORECCD_ERR_INVALID;
   if (n > h->p.max_carriers) return fail(h, GCORECCD_ERR_CAPACITY, "load_snapshot: capacity");
+  if (events_busy(h)) return fail(h, GCORECCD_ERR_STATE, "load_snapshot: a batch of events is still drifting");
   DeviceGuard guard(h->device);
   float* st_xyz = h->Ep;
   uint32_t* st_id = (uint32_t*)(h->Ep + 3 * h->L.cap_pad);
@@ -453,7 +481,7 @@ int gcoreccd_get_state(gcoreccd_t* h, uint64_t* step, uint64_t* n_active, uint64
   int rc = sync_ctrl(h);
   if (rc) return rc;
   if (step) *step = h->h_ctrl->step;
-  if (n_active) *n_active = h->h_ctrl->n_active;
+  if (n_active) *n_active = h->h_ctrl->n_active + (h->evb.loaded ? h->evb.carriers_left : 0);
   if (n_loaded) *n_loaded = h->h_ctrl->n_loaded;
   if (n_collected) *n_collected = h->h_ctrl->n_collected;
   if (n_out_of_window) *n_out_of_window = h->h_ctrl->n_overflow;
@@ -558,6 +586,176 @@ int gcoreccd_debug_normals(gcoreccd_t* h, const uint32_t* id, const uint64_t* st
   if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
   cudaFree(buf);
   if (e != cudaSuccess) return fail(h, GCORECCD_ERR_CUDA, "debug_normals", e);
+  return GCORECCD_OK;
+}
+
+// ---------------------------------------------------------------------------- batched independent events
+int gcoreccd_load_events(gcoreccd_t* h, const float* xyz, const uint64_t* offsets, uint64_t n_events, int on_device) {
+  if (!h || !offsets || n_events == 0 || n_events > 0x7fffffffull) return GCORECCD_ERR_INVALID;
+  const uint64_t n = offsets[n_events];
+  if (offsets[0] != 0 || (!xyz && n)) return fail(h, GCORECCD_ERR_INVALID, "load_events: offsets[0] must be 0");
+  for (uint64_t e = 0; e < n_events; ++e) {
+    if (offsets[e + 1] < offsets[e]) return fail(h, GCORECCD_ERR_INVALID, "load_events: offsets must be non-decreasing");
+    if (offsets[e + 1] - offsets[e] > GCORECCD_EVENT_MAX_CARRIERS)
+      return fail(h, GCORECCD_ERR_CAPACITY, "load_events: an event exceeds GCORECCD_EVENT_MAX_CARRIERS");
+  }
+  if (n > h->p.max_carriers || h->n_loaded + n > 0xffffffffull) return fail(h, GCORECCD_ERR_CAPACITY, "load_events: capacity");
+  if (events_busy(h)) return fail(h, GCORECCD_ERR_STATE, "load_events: the previous batch is still drifting (run_events or reset first)");
+  DeviceGuard guard(h->device);
+  int rc = sync_ctrl(h);
+  if (rc) return rc;
+  if (h->h_ctrl->n_active) return fail(h, GCORECCD_ERR_STATE, "load_events: the handle holds a single event that is still drifting");
+
+  const float* src = xyz;
+  if (n) {
+    if (!on_device) {
+      GC_CUDA(h, cudaMemcpyAsync(h->Ep, xyz, n * 12, cudaMemcpyHostToDevice, h->stream));
+      src = h->Ep;
+    }
+    GC_CUDA(h, cudaMemsetAsync(&h->ctrl->invalid, 0, 4, h->stream));
+    k_validate<<<tiles_for(n), kTPB, 0, h->stream>>>(src, (uint32_t)n, h->ctrl, h->dp.thickness);
+    h->launches += 1;
+    rc = sync_ctrl(h);
+    if (rc) return rc;
+    if (h->h_ctrl->invalid) return fail(h, GCORECCD_ERR_INVALID, "load_events: non-finite coordinate or z > thickness");
+  }
+
+  drop_events(h);
+  auto& B = h->evb;
+  const size_t ne = (size_t)n_events;
+  const size_t b_off = align_up((ne + 1) * 4, 256), b_cnt = align_up(ne * 4, 256), b_ord = align_up(ne * 4, 256), b_q = 256,
+               b_step = align_up(ne * 8, 256);
+  cudaError_t e = cudaMalloc((void**)&B.d_buf, b_off + b_cnt + b_ord + b_q + b_step);
+  if (e != cudaSuccess) { B.d_buf = nullptr; return fail(h, e == cudaErrorMemoryAllocation ? GCORECCD_ERR_NOMEM : GCORECCD_ERR_CUDA, "load_events: cudaMalloc", e); }
+  B.d_off = (uint32_t*)B.d_buf;
+  B.d_cnt = (uint32_t*)(B.d_buf + b_off);
+  B.d_order = (uint32_t*)(B.d_buf + b_off + b_cnt);
+  B.d_queue = (uint32_t*)(B.d_buf + b_off + b_cnt + b_ord);
+  B.d_step = (uint64_t*)(B.d_buf + b_off + b_cnt + b_ord + b_q);
+  B.h_off = (uint32_t*)malloc((ne + 1) * 4);
+  B.h_cnt = (uint32_t*)malloc(ne * 4 + 4);
+  B.h_step = (uint64_t*)calloc(ne + 1, 8);
+  uint32_t* order = (uint32_t*)malloc(ne * 4 + 4);
+  if (!B.h_off || !B.h_cnt || !B.h_step || !order) { free(order); drop_events(h); return fail(h, GCORECCD_ERR_NOMEM, "load_events: host memory"); }
+  uint64_t left_events = 0;
+  for (size_t k = 0; k < ne; ++k) {
+    B.h_off[k] = (uint32_t)offsets[k];
+    B.h_cnt[k] = (uint32_t)(offsets[k + 1] - offsets[k]);
+    if (B.h_cnt[k]) left_events += 1;
+  }
+  B.h_off[ne] = (uint32_t)n;
+  // two queues, each largest event first (longest-processing-time order for the persistent grids)
+  uint32_t ns = 0;
+  for (size_t k = 0; k < ne; ++k) if (B.h_cnt[k] <= kEvCapSmall) order[ns++] = (uint32_t)k;
+  uint32_t nl = ns;
+  for (size_t k = 0; k < ne; ++k) if (B.h_cnt[k] > kEvCapSmall) order[nl++] = (uint32_t)k;
+  const uint32_t* cnt = B.h_cnt;
+  auto by_size = [cnt](uint32_t a, uint32_t b) { return cnt[a] != cnt[b] ? cnt[a] > cnt[b] : a < b; };
+  std::sort(order, order + ns, by_size);
+  std::sort(order + ns, order + ne, by_size);
+  B.n_small = ns; B.n_large = (uint32_t)ne - ns;
+  e = cudaMemcpyAsync(B.d_off, B.h_off, (ne + 1) * 4, cudaMemcpyHostToDevice, h->stream);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(B.d_cnt, B.h_cnt, ne * 4, cudaMemcpyHostToDevice, h->stream);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(B.d_order, order, ne * 4, cudaMemcpyHostToDevice, h->stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(B.d_step, 0, ne * 8, h->stream);
+  if (e == cudaSuccess && n) {
+    k_unpack_events<<<tiles_for(n), kTPB, 0, h->stream>>>(src, (uint32_t)n, h->A, (uint32_t)h->n_loaded);
+    h->launches += 1;
+    e = cudaGetLastError();
+  }
+  const uint64_t total_loaded = h->n_loaded + n;
+  if (e == cudaSuccess) e = cudaMemcpyAsync(&h->ctrl->n_loaded, &total_loaded, 8, cudaMemcpyHostToDevice, h->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+  free(order);
+  if (e != cudaSuccess) { drop_events(h); return fail(h, GCORECCD_ERR_CUDA, "load_events", e); }
+
+  // persistent grids: resident CTAs per SM x SM count
+  const size_t sm_small = event_smem_bytes(kEvCapSmall), sm_large = event_smem_bytes(kEvCapLarge);
+  int occ_s = 0, occ_l = 0;
+  e = cudaFuncSetAttribute(k_events<1, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_small);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_events<4, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_large);
+  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_s, k_events<1, 3>, kTPB, sm_small);
+  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_l, k_events<4, 1>, kTPB, sm_large);
+  if (e != cudaSuccess) { drop_events(h); return fail(h, GCORECCD_ERR_CUDA, "load_events: kernel attributes", e); }
+  B.grid_small = h->num_sms * (occ_s > 0 ? occ_s : 1);
+  B.grid_large = h->num_sms * (occ_l > 0 ? occ_l : 1);
+  B.loaded = true;
+  B.n_events = n_events; B.n_carriers = n;
+  B.events_left = left_events; B.carriers_left = n;
+  h->n_loaded = total_loaded;
+  return GCORECCD_OK;
+}
+
+int gcoreccd_run_events(gcoreccd_t* h, uint64_t max_steps, uint64_t* events_left, uint64_t* carriers_left) {
+  if (!h) return GCORECCD_ERR_INVALID;
+  auto& B = h->evb;
+  if (!B.loaded) return fail(h, GCORECCD_ERR_STATE, "run_events: no batch loaded");
+  DeviceGuard guard(h->device);
+  int ret = GCORECCD_OK;
+  if (B.carriers_left > 0) {
+    const EventTable tab{B.d_off, B.d_cnt, B.d_step};
+    GC_CUDA(h, cudaMemsetAsync(B.d_queue, 0, 8, h->stream));
+    // the large events first: they are the long poles; the small queue fills the SMs as they drain
+    if (B.n_large) {
+      const int g = (int)std::min<uint32_t>(B.n_large, (uint32_t)B.grid_large);
+      k_events<4, 1><<<g, kTPB, event_smem_bytes(kEvCapLarge), h->stream>>>(h->A, tab, B.d_order + B.n_small, B.n_large, B.d_queue + 1,
+                                                                          h->ctrl, h->image, h->dp, max_steps, kEvCapLarge);
+      h->launches += 1;
+    }
+    if (B.n_small) {
+      const int g = (int)std::min<uint32_t>(B.n_small, (uint32_t)B.grid_small);
+      k_events<1, 3><<<g, kTPB, event_smem_bytes(kEvCapSmall), h->stream>>>(h->A, tab, B.d_order, B.n_small, B.d_queue, h->ctrl,
+                                                                          h->image, h->dp, max_steps, kEvCapSmall);
+      h->launches += 1;
+    }
+    GC_CUDA(h, cudaGetLastError());
+    GC_CUDA(h, cudaMemcpyAsync(B.h_cnt, B.d_cnt, B.n_events * 4, cudaMemcpyDeviceToHost, h->stream));
+    GC_CUDA(h, cudaMemcpyAsync(B.h_step, B.d_step, B.n_events * 8, cudaMemcpyDeviceToHost, h->stream));
+    int rc = sync_ctrl(h);
+    if (rc) return rc;
+    uint64_t el = 0, cl = 0;
+    for (uint64_t k = 0; k < B.n_events; ++k) { if (B.h_cnt[k]) el += 1; cl += B.h_cnt[k]; }
+    B.events_left = el; B.carriers_left = cl;
+    h->n_bound = 0;
+    if (h->h_ctrl->nonfinite) return fail(h, GCORECCD_ERR_NONFINITE, "a carrier position became non-finite");
+  }
+  if (B.carriers_left > 0) ret = GCORECCD_MAX_STEPS;
+  if (events_left) *events_left = B.events_left;
+  if (carriers_left) *carriers_left = B.carriers_left;
+  return ret;
+}
+
+int gcoreccd_get_events(gcoreccd_t* h, uint64_t* n_active, uint64_t* step, uint64_t cap_events, uint64_t* n_events) {
+  if (!h) return GCORECCD_ERR_INVALID;
+  const auto& B = h->evb;
+  if (!B.loaded) return fail(h, GCORECCD_ERR_STATE, "get_events: no batch loaded");
+  if (n_events) *n_events = B.n_events;
+  if ((n_active || step) && cap_events < B.n_events) return fail(h, GCORECCD_ERR_CAPACITY, "get_events: buffer too small");
+  for (uint64_t k = 0; k < B.n_events; ++k) {
+    if (n_active) n_active[k] = B.h_cnt[k];
+    if (step) step[k] = B.h_step[k];
+  }
+  return GCORECCD_OK;
+}
+
+int gcoreccd_read_event_carriers(gcoreccd_t* h, uint64_t event, float* xyz, uint32_t* id, uint64_t cap, uint64_t* n) {
+  if (!h) return GCORECCD_ERR_INVALID;
+  const auto& B = h->evb;
+  if (!B.loaded) return fail(h, GCORECCD_ERR_STATE, "read_event_carriers: no batch loaded");
+  if (event >= B.n_events) return fail(h, GCORECCD_ERR_INVALID, "read_event_carriers: no such event");
+  const uint32_t cnt = B.h_cnt[event], off = B.h_off[event];
+  if (n) *n = cnt;
+  if ((xyz || id) && cap < cnt) return fail(h, GCORECCD_ERR_CAPACITY, "read_event_carriers: buffer too small");
+  if (cnt == 0 || (!xyz && !id)) return GCORECCD_OK;
+  DeviceGuard guard(h->device);
+  if (xyz) {
+    k_interleave_range<<<tiles_for(cnt), kTPB, 0, h->stream>>>(h->A, off, cnt, h->Ep);
+    h->launches += 1;
+    GC_CUDA(h, cudaMemcpyAsync(xyz, h->Ep, (size_t)cnt * 12, cudaMemcpyDeviceToHost, h->stream));
+  }
+  if (id) GC_CUDA(h, cudaMemcpyAsync(id, h->A.id + off, (size_t)cnt * 4, cudaMemcpyDeviceToHost, h->stream));
+  GC_CUDA(h, cudaGetLastError());
+  GC_CUDA(h, cudaStreamSynchronize(h->stream));
   return GCORECCD_OK;
 }
 

@@ -118,3 +118,25 @@ def make(config, seed=SEED, n=None):
     # keep the float32 state inside the slab (rounding can land exactly on the back surface; that is allowed)
     xyz[:, 2] = np.minimum(xyz[:, 2], np.float32(th))
     return dict(xyz=xyz, params=P, groups=groups, name=name, config=config)
+
+
+def make_events(sizes, seed=SEED, sigma_um=0.5, depth_range=(10.0, 665.0), half_window_um=400.0):
+    """A batch of INDEPENDENT X-ray events: event k is a Gaussian cloud of
+    sizes[k] holes (sigma_um) at a depth uniform in depth_range and a lateral centre uniform over the central
+    +-half_window_um of the 64x64-pixel window.  Holes of different events never interact.  Returns
+    dict(xyz float32 (N,3), offsets uint64 (n_events+1), params, name)."""
+    P = dict(COMMON)
+    P["seed"] = seed
+    P.update(img_nx=64, img_ny=64, img_x0_um=-480.0, img_y0_um=-480.0)
+    rng = _rng(seed, 0x45564E54)
+    parts, off = [], [0]
+    for s in sizes:
+        c = (rng.uniform(-half_window_um, half_window_um), rng.uniform(-half_window_um, half_window_um),
+             rng.uniform(depth_range[0], depth_range[1]))
+        parts.append(gaussian_cloud(rng, int(s), sigma_um, c))
+        off.append(off[-1] + int(s))
+    xyz = np.concatenate(parts) if parts else np.zeros((0, 3))
+    xyz = np.ascontiguousarray(xyz.astype(np.float32))
+    xyz[:, 2] = np.minimum(xyz[:, 2], np.float32(P["thickness_um"]))
+    return dict(xyz=xyz, offsets=np.asarray(off, dtype=np.uint64), params=P,
+                name="%d independent X-ray events, %d holes in total (sigma %.2g um)" % (len(sizes), off[-1], sigma_um))
