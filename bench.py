@@ -268,6 +268,36 @@ def run_ours(args):
         event = {"seconds": ev_s, "steps": done, "pair_interactions": st2["pair_interactions"],
                  "avg_G_pairs_per_s": st2["pair_interactions"] / ev_s / 1e9, "holes": n, "collected_in_window": int(img.sum())}
 
+    # ---- batched independent events (secondary numbers, not the headline): one CTA per event
+    batched = None
+    if not args.no_event and rank == 0:
+        batched = []
+        for sizes, what in (([2048] * 592, "592 X-ray events x 2,048 holes (7.5 keV-like clouds, sigma 0.5 um, depth U[10,665] um)"),
+                            ([26] * 44400, "44,400 X-ray events x 26 holes (100 eV, PAPER.md:106)")):
+            we = workloads.make_events(sizes)
+            ne = len(we["xyz"])
+            bs = binding.from_workload(we, max_carriers=ne, stream=stream)
+            hin = torch.from_numpy(we["xyz"]).pin_memory()
+            best = None
+            for _ in range(2):
+                bs.reset()
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                bs.load_events_ptr(hin.data_ptr(), we["offsets"])
+                ev_left, ca_left, rc = bs.run_events()
+                imgb, overb = bs.read_image()
+                dt_s = time.perf_counter() - t0
+                stb = bs.state()
+                assert ca_left == 0 and int(imgb.sum()) + overb == ne, "hole count not conserved (batch)"
+                if best is None or dt_s < best["seconds"]:
+                    best = {"workload": what, "seconds": dt_s, "events_per_s": len(sizes) / dt_s,
+                            "pair_interactions": stb["pair_interactions"],
+                            "G_pairs_per_s": stb["pair_interactions"] / dt_s / 1e9,
+                            "frac_of_fp32_peak": stb["pair_interactions"] * FLOP_PER_PAIR / dt_s / 1e12 / peak_tf,
+                            "timing": "wall clock: load_events(pinned host) + run_events to full collection + read_image"}
+            batched.append(best)
+            bs.close()
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -292,7 +322,7 @@ def run_ours(args):
             "clocks": clocks, "gpu_launches": launches,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": n * 12, "d2h_bytes_per_step": n * 12,
                     "what": "reset + load_carriers(pinned host) + step(1) + read_carriers(host), wall clock"},
-            "roofline": roofline, "cpu_baseline": cpu, "seconds_per_event": event}
+            "roofline": roofline, "cpu_baseline": cpu, "seconds_per_event": event, "batched_events": batched}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

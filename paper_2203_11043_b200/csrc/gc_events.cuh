@@ -10,7 +10,8 @@
 // the same packed inner loop as k_field — with zero launches and zero HBM round trips per step.
 //
 // Per step inside the CTA (PAPER.md:68 order, identical arithmetic to k_field / k_integrate / k_compact):
-//   field + integrate:  thread t owns targets {pass*2*NPACK*TPB + (p*TPB + t)*2 + {0,1}}; it sums eq. 6 over all
+//   field + integrate:  thread t owns targets {pass*2*NPACK*TPB + p*2*TPB + t + {0,hs}} (the two lanes of pack p; hs = TPB,
+//                       less in the last pack, see k_events); it sums eq. 6 over all
 //                       sources from shared memory (two-level FP32 accumulation: 256-source tile partials flushed
 //                       into a total), then advances each of its targets in FP64 (advance_carrier) into s_next;
 //   collect + compact:  each thread takes a contiguous run of s_next, bins the holes with z <= z_well into the
@@ -29,8 +30,10 @@ struct EventTable {            // device arrays, one entry per event
   uint64_t* step;              // steps taken so far = index of the event's next step (Philox counter)
 };
 
-constexpr uint32_t kEvCapSmall = 512;      // NPACK = 1 variant: one pass covers 512 targets, several CTAs per SM
-constexpr uint32_t kEvCapLarge = 4096;     // NPACK = 4 variant: 2,048 targets per pass, one CTA per SM
+// Three variants, chosen per event by its size at load:
+constexpr uint32_t kEvCapTiny  = 128;      // NPACK 1,  64 threads: one pass covers 128 targets, ~12 CTAs (events) per SM
+constexpr uint32_t kEvCapSmall = 512;      // NPACK 1, 256 threads: one pass covers 512 targets, 3 CTAs per SM
+constexpr uint32_t kEvCapLarge = 4096;     // NPACK 4, 256 threads: 2,048 targets per pass, one CTA per SM
 
 __host__ __device__ constexpr size_t event_smem_bytes(uint32_t cap) {
   // s_xy float4[cap+4] | s_next float4[cap] | s_z float2[cap+4] | s_id u32[cap]
@@ -38,18 +41,18 @@ __host__ __device__ constexpr size_t event_smem_bytes(uint32_t cap) {
 }
 
 // Field of NP packs of this thread against all n sources in shared memory; returns sum (r_s - r_t) w per target.
-template <int NP>
+template <int NP, int TPB>
 __device__ __forceinline__ void event_field(const float4* __restrict__ s_xy, const float2* __restrict__ s_z, uint32_t n,
-                                            uint32_t i_first, const float2 eps2v, float2 (&tx)[NP], float2 (&ty)[NP],
-                                            float2 (&tz)[NP]) {
+                                            uint32_t i_first, uint32_t p_last, uint32_t hs_last, const float2 eps2v,
+                                            float2 (&tx)[NP], float2 (&ty)[NP], float2 (&tz)[NP]) {
   float2 ntx[NP], nty[NP], ntz[NP];
 #pragma unroll
   for (int p = 0; p < NP; ++p) {
-    const uint32_t i0 = i_first + (uint32_t)p * (2u * kTPB);
+    const uint32_t i0 = i_first + (uint32_t)p * (2u * TPB), i1 = i0 + ((uint32_t)p == p_last ? hs_last : (uint32_t)TPB);
     // slots >= n hold sentinels or stale data: keep them out of the arithmetic (their result is never used)
-    const bool v0 = i0 < n, v1 = i0 + 1 < n;
-    const float4 a0 = s_xy[v0 ? i0 : 0], a1 = s_xy[v1 ? i0 + 1 : 0];
-    const float2 b0 = s_z[v0 ? i0 : 0], b1 = s_z[v1 ? i0 + 1 : 0];
+    const bool v0 = i0 < n, v1 = i1 < n;
+    const float4 a0 = s_xy[v0 ? i0 : 0], a1 = s_xy[v1 ? i1 : 0];
+    const float2 b0 = s_z[v0 ? i0 : 0], b1 = s_z[v1 ? i1 : 0];
     ntx[p] = make_float2(-a0.x, -a1.x); nty[p] = make_float2(-a0.z, -a1.z); ntz[p] = make_float2(-b0.x, -b1.x);
     tx[p] = make_float2(0.f, 0.f); ty[p] = tx[p]; tz[p] = tx[p];
   }
@@ -70,16 +73,17 @@ __device__ __forceinline__ void event_field(const float4* __restrict__ s_xy, con
 }
 
 // a2..a6 for the 2 NP targets of this thread, results into s_next (x', y', z', id).
-template <int NP>
+template <int NP, int TPB>
 __device__ __forceinline__ void event_advance(const float4* __restrict__ s_xy, const float2* __restrict__ s_z,
                                               const uint32_t* __restrict__ s_id, float4* __restrict__ s_next, uint32_t n,
-                                              uint32_t i_first, uint64_t step, const float2 (&tx)[NP], const float2 (&ty)[NP],
-                                              const float2 (&tz)[NP], const DevParams& P, uint32_t& nonfinite) {
+                                              uint32_t i_first, uint32_t p_last, uint32_t hs_last, uint64_t step,
+                                              const float2 (&tx)[NP], const float2 (&ty)[NP], const float2 (&tz)[NP],
+                                              const DevParams& P, uint32_t& nonfinite) {
 #pragma unroll
   for (int p = 0; p < NP; ++p) {
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
-      const uint32_t i = i_first + (uint32_t)p * (2u * kTPB) + (uint32_t)h;
+      const uint32_t i = i_first + (uint32_t)p * (2u * TPB) + (uint32_t)h * ((uint32_t)p == p_last ? hs_last : (uint32_t)TPB);
       if (i < n) {
         const float x = s_xy[i].x, y = s_xy[i].z, z = s_z[i].x;
         const uint32_t id = s_id[i];
@@ -94,23 +98,24 @@ __device__ __forceinline__ void event_advance(const float4* __restrict__ s_xy, c
   }
 }
 
-template <int NP>
+template <int NP, int TPB>
 __device__ __forceinline__ void event_pass(const float4* s_xy, const float2* s_z, const uint32_t* s_id, float4* s_next,
-                                           uint32_t n, uint32_t i_first, uint64_t step, const DevParams& P, uint32_t& nonfinite) {
+                                           uint32_t n, uint32_t i_first, uint32_t p_last, uint32_t hs_last, uint64_t step,
+                                           const DevParams& P, uint32_t& nonfinite) {
   float2 tx[NP], ty[NP], tz[NP];
   if (!(P.flags & 1u)) {                                     // GCORECCD_COULOMB_OFF
-    event_field<NP>(s_xy, s_z, n, i_first, make_float2(P.eps2, P.eps2), tx, ty, tz);
+    event_field<NP, TPB>(s_xy, s_z, n, i_first, p_last, hs_last, make_float2(P.eps2, P.eps2), tx, ty, tz);
   } else {
 #pragma unroll
     for (int p = 0; p < NP; ++p) { tx[p] = make_float2(0.f, 0.f); ty[p] = tx[p]; tz[p] = tx[p]; }
   }
-  event_advance<NP>(s_xy, s_z, s_id, s_next, n, i_first, step, tx, ty, tz, P, nonfinite);
+  event_advance<NP, TPB>(s_xy, s_z, s_id, s_next, n, i_first, p_last, hs_last, step, tx, ty, tz, P, nonfinite);
 }
 
 // Persistent grid; CTA loop: take the next event of `order[0..n_order)`, run it for up to max_steps more steps
 // (or to full collection), store the survivors back.  cap = holes the dynamic shared memory is sized for.
-template <int NPACK, int MINB>                 // NPACK is 1 (small events) or 4 (large events)
-__global__ void __launch_bounds__(kTPB, MINB)
+template <int NPACK, int TPB, int MINB>        // NPACK is 1 (tiny / small events) or 4 (large events)
+__global__ void __launch_bounds__(TPB, MINB)
 k_events(SoA A, EventTable ev, const uint32_t* __restrict__ order, uint32_t n_order, uint32_t* __restrict__ queue,
          Ctrl* __restrict__ ctrl, uint32_t* __restrict__ image, DevParams P, uint64_t max_steps, uint32_t cap) {
   extern __shared__ __align__(16) unsigned char smem[];
@@ -118,11 +123,11 @@ k_events(SoA A, EventTable ev, const uint32_t* __restrict__ order, uint32_t n_or
   float4* s_next = s_xy + (cap + 4);                                    // (x',y',z',id), cap entries
   float2* s_z = reinterpret_cast<float2*>(s_next + cap);                // (z,z), cap + 4 entries
   uint32_t* s_id = reinterpret_cast<uint32_t*>(s_z + (cap + 4));        // cap entries
-  __shared__ uint32_t s_warp[kTPB / 32];
+  __shared__ uint32_t s_warp[TPB / 32];
   __shared__ uint32_t s_ev, s_coll, s_over;
 
   const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
-  constexpr uint32_t kPass = 2u * NPACK * kTPB;                          // targets per pass
+  constexpr uint32_t kPass = 2u * NPACK * TPB;                          // targets per pass
   uint32_t nonfinite = 0;
 
   for (;;) {
@@ -135,7 +140,7 @@ k_events(SoA A, EventTable ev, const uint32_t* __restrict__ order, uint32_t n_or
     uint32_t n = ev.cnt[e];
     uint64_t step = ev.step[e];
     if (n == 0) continue;
-    for (uint32_t i = tid; i < n; i += kTPB)
+    for (uint32_t i = tid; i < n; i += TPB)
       s_next[i] = make_float4(A.x[off + i], A.y[off + i], A.z[off + i], __uint_as_float(A.id[off + i]));
     __syncthreads();
 
@@ -143,7 +148,7 @@ k_events(SoA A, EventTable ev, const uint32_t* __restrict__ order, uint32_t n_or
     bool first = true;
     for (;;) {
       // ---- a7 + a8: bin the holes that crossed z_well, compact the survivors (stable) into the field layout
-      const uint32_t per = (n + kTPB - 1) / kTPB;
+      const uint32_t per = (n + TPB - 1) / TPB;
       const uint32_t lo = min(tid * per, n), hi = min(lo + per, n);
       uint32_t keep = 0, coll = 0, over = 0;
       for (uint32_t i = lo; i < hi; ++i) {
@@ -159,7 +164,7 @@ k_events(SoA A, EventTable ev, const uint32_t* __restrict__ order, uint32_t n_or
       __syncthreads();
       uint32_t base = 0, total = 0;
 #pragma unroll
-      for (int w = 0; w < kTPB / 32; ++w) { const uint32_t v = s_warp[w]; if (w < (int)warp) base += v; total += v; }
+      for (int w = 0; w < TPB / 32; ++w) { const uint32_t v = s_warp[w]; if (w < (int)warp) base += v; total += v; }
       uint32_t o = base + incl - keep;
       for (uint32_t i = lo; i < hi; ++i) {
         const float4 c = s_next[i];
@@ -180,24 +185,30 @@ k_events(SoA A, EventTable ev, const uint32_t* __restrict__ order, uint32_t n_or
 
       // ---- a1..a6: field of every hole of the event, then its Euler-Maruyama update, into s_next
       for (uint32_t base_i = 0; base_i < n; base_i += kPass) {
-        const uint32_t i_first = base_i + tid * 2u;                     // pack p adds p * 2 * kTPB
-        const uint32_t w_first = base_i + warp * 64u;                   // first target of this warp in pack 0
-        if (w_first >= n) continue;                                     // warp-uniform
-        const uint32_t np = min((uint32_t)NPACK, (n - w_first + 2u * kTPB - 1u) / (2u * kTPB));   // packs with a live target
+        // Pack p covers targets [base_i + p 2TPB, +2TPB): thread t takes t and t + hs of it.  hs = TPB except in the
+        // last live pack, where it shrinks to half the remaining targets (rounded up to a warp), so that both lanes
+        // of the packed arithmetic stay busy and an event of <= 32 holes puts one hole on each thread of one warp.
+        const uint32_t i_first = base_i + tid;
+        const uint32_t m = min(n - base_i, kPass);
+        const uint32_t p_last = (m - 1u) / (2u * TPB);
+        const uint32_t m_last = m - p_last * (2u * TPB);
+        const uint32_t hs_last = min((uint32_t)TPB, max(32u, (((m_last + 1u) >> 1) + 31u) & ~31u));
+        const uint32_t np = p_last + ((warp * 32u < hs_last) ? 1u : 0u);   // packs with a live target in this warp (uniform)
+        if (np == 0) continue;
         if constexpr (NPACK == 1) {
-          event_pass<1>(s_xy, s_z, s_id, s_next, n, i_first, step, P, nonfinite);
+          event_pass<1, TPB>(s_xy, s_z, s_id, s_next, n, i_first, p_last, hs_last, step, P, nonfinite);
         } else {
-          if (np == 1) event_pass<1>(s_xy, s_z, s_id, s_next, n, i_first, step, P, nonfinite);
-          else if (np == 2) event_pass<2>(s_xy, s_z, s_id, s_next, n, i_first, step, P, nonfinite);
-          else if (np == 3) event_pass<3>(s_xy, s_z, s_id, s_next, n, i_first, step, P, nonfinite);
-          else event_pass<4>(s_xy, s_z, s_id, s_next, n, i_first, step, P, nonfinite);
+          if (np == 1) event_pass<1, TPB>(s_xy, s_z, s_id, s_next, n, i_first, p_last, hs_last, step, P, nonfinite);
+          else if (np == 2) event_pass<2, TPB>(s_xy, s_z, s_id, s_next, n, i_first, p_last, hs_last, step, P, nonfinite);
+          else if (np == 3) event_pass<3, TPB>(s_xy, s_z, s_id, s_next, n, i_first, p_last, hs_last, step, P, nonfinite);
+          else event_pass<4, TPB>(s_xy, s_z, s_id, s_next, n, i_first, p_last, hs_last, step, P, nonfinite);
         }
       }
       __syncthreads();
     }
 
     // ---- retire: survivors (if max_steps stopped the event early) back to the state arrays, counters out
-    for (uint32_t i = tid; i < n; i += kTPB) {
+    for (uint32_t i = tid; i < n; i += TPB) {
       A.x[off + i] = s_xy[i].x; A.y[off + i] = s_xy[i].z; A.z[off + i] = s_z[i].x; A.id[off + i] = s_id[i];
     }
     if (tid == 0) {
@@ -217,6 +228,20 @@ k_interleave_range(SoA A, uint32_t off, uint32_t n, float* __restrict__ xyz) {
   const uint32_t i = blockIdx.x * kTPB + threadIdx.x;
   if (i >= n) return;
   xyz[3 * (size_t)i] = A.x[off + i]; xyz[3 * (size_t)i + 1] = A.y[off + i]; xyz[3 * (size_t)i + 2] = A.z[off + i];
+}
+
+// Scheduling hint only (never enters the physics): mean depth of each event, one warp per event.  The host orders
+// every queue by the estimated work n^2 x (steps to drift home from that depth), longest first.
+__global__ void __launch_bounds__(kTPB)
+k_event_depth(SoA A, const uint32_t* __restrict__ off, const uint32_t* __restrict__ cnt, uint32_t n_events,
+              float* __restrict__ zmean) {
+  const uint32_t e = (blockIdx.x * kTPB + threadIdx.x) >> 5, lane = threadIdx.x & 31u;
+  if (e >= n_events) return;
+  const uint32_t o = off[e], n = cnt[e];
+  float s = 0.f;
+  for (uint32_t i = lane; i < n; i += 32) s += A.z[o + i];
+  for (int k = 16; k > 0; k >>= 1) s += __shfl_xor_sync(0xffffffffu, s, k);
+  if (lane == 0) zmean[e] = n ? s / (float)n : 0.f;
 }
 
 // Load path of the batch: interleaved xyz -> state arrays at the same index, ids id_base + index.

@@ -42,9 +42,13 @@ __device__ __forceinline__ void philox_normals(uint32_t seed_lo, uint32_t seed_h
   if (words) *words = w;
 }
 
-// eq. 2 with the temperature terms folded on the host: mu = mu0 / (1 + (E/Ec)^beta)^(1/beta)
+// eq. 2 with the temperature terms folded on the host: mu = mu0 / (1 + (E/Ec)^beta)^(1/beta), evaluated as
+// mu0 exp(-log1p(exp(beta log(E/Ec))) / beta): relative error ~1e-15 (FP64 log/exp), ten orders below what the
+// FP32 state can resolve, at a third of the dependent-instruction chain of two pow() calls (the per-carrier
+// chain is what bounds a small event's step, gc_events.cuh).  E = 0 gives log = -inf, exp = 0, mu = mu0.
 __device__ __forceinline__ double mobility(double E, const DevParams& P) {
-  return P.mu0 / pow(1.0 + pow(E * P.inv_Ec, P.beta), P.inv_beta);
+  const double t = exp(P.beta * log(E * P.inv_Ec));
+  return P.mu0 * exp(-P.inv_beta * log1p(t));
 }
 
 // a7: half-open pixel bins, floor, in FP64 on the stored FP32 position (exactly reproducible).

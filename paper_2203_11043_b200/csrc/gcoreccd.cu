@@ -79,13 +79,15 @@ struct gcoreccd {
     bool loaded;
     uint64_t n_events, n_carriers;        // as loaded
     uint64_t events_left, carriers_left;  // after the last run_events
-    uint32_t n_small, n_large;            // events per queue (order = [small..., large...], each largest first)
+    uint32_t n_q[3];                      // events per queue: tiny, small, large (order = [tiny..., small..., large...])
     char* d_buf;                          // one allocation: off | cnt | order | queue | step
     uint32_t *d_off, *d_cnt, *d_order, *d_queue;
     uint64_t* d_step;
     uint32_t *h_off, *h_cnt;              // host mirrors
     uint64_t* h_step;
-    int grid_small, grid_large;
+    int grid_q[3];
+    cudaStream_t aux[2];                  // the small and tiny queues run beside the large one
+    cudaEvent_t fork, join[2];
   } evb;
 };
 
@@ -223,6 +225,11 @@ int enqueue_steps(gcoreccd_t* h, uint64_t n_steps) {
 
 void drop_events(gcoreccd_t* h) {
   if (h->evb.d_buf) cudaFree(h->evb.d_buf);
+  for (int k = 0; k < 2; ++k) {
+    if (h->evb.aux[k]) cudaStreamDestroy(h->evb.aux[k]);
+    if (h->evb.join[k]) cudaEventDestroy(h->evb.join[k]);
+  }
+  if (h->evb.fork) cudaEventDestroy(h->evb.fork);
   free(h->evb.h_off); free(h->evb.h_cnt); free(h->evb.h_step);
   memset(&h->evb, 0, sizeof(h->evb));
 }
@@ -644,19 +651,8 @@ int gcoreccd_load_events(gcoreccd_t* h, const float* xyz, const uint64_t* offset
     if (B.h_cnt[k]) left_events += 1;
   }
   B.h_off[ne] = (uint32_t)n;
-  // two queues, each largest event first (longest-processing-time order for the persistent grids)
-  uint32_t ns = 0;
-  for (size_t k = 0; k < ne; ++k) if (B.h_cnt[k] <= kEvCapSmall) order[ns++] = (uint32_t)k;
-  uint32_t nl = ns;
-  for (size_t k = 0; k < ne; ++k) if (B.h_cnt[k] > kEvCapSmall) order[nl++] = (uint32_t)k;
-  const uint32_t* cnt = B.h_cnt;
-  auto by_size = [cnt](uint32_t a, uint32_t b) { return cnt[a] != cnt[b] ? cnt[a] > cnt[b] : a < b; };
-  std::sort(order, order + ns, by_size);
-  std::sort(order + ns, order + ne, by_size);
-  B.n_small = ns; B.n_large = (uint32_t)ne - ns;
   e = cudaMemcpyAsync(B.d_off, B.h_off, (ne + 1) * 4, cudaMemcpyHostToDevice, h->stream);
   if (e == cudaSuccess) e = cudaMemcpyAsync(B.d_cnt, B.h_cnt, ne * 4, cudaMemcpyHostToDevice, h->stream);
-  if (e == cudaSuccess) e = cudaMemcpyAsync(B.d_order, order, ne * 4, cudaMemcpyHostToDevice, h->stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(B.d_step, 0, ne * 8, h->stream);
   if (e == cudaSuccess && n) {
     k_unpack_events<<<tiles_for(n), kTPB, 0, h->stream>>>(src, (uint32_t)n, h->A, (uint32_t)h->n_loaded);
@@ -665,20 +661,61 @@ int gcoreccd_load_events(gcoreccd_t* h, const float* xyz, const uint64_t* offset
   }
   const uint64_t total_loaded = h->n_loaded + n;
   if (e == cudaSuccess) e = cudaMemcpyAsync(&h->ctrl->n_loaded, &total_loaded, 8, cudaMemcpyHostToDevice, h->stream);
+  // scheduling hint: mean depth per event (d_order doubles as the float scratch until the order is uploaded)
+  float* zmean = (float*)malloc(ne * 4 + 4);
+  if (!zmean) { free(order); drop_events(h); return fail(h, GCORECCD_ERR_NOMEM, "load_events: host memory"); }
+  if (e == cudaSuccess) {
+    k_event_depth<<<(unsigned)((ne * 32 + kTPB - 1) / kTPB), kTPB, 0, h->stream>>>(h->A, B.d_off, B.d_cnt, (uint32_t)ne, (float*)B.d_order);
+    h->launches += 1;
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess) e = cudaMemcpyAsync(zmean, B.d_order, ne * 4, cudaMemcpyDeviceToHost, h->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+  if (e != cudaSuccess) { free(order); free(zmean); drop_events(h); return fail(h, GCORECCD_ERR_CUDA, "load_events", e); }
+  // three queues (one per kernel variant), each in longest-processing-time-first order
+  // estimated work of an event = n^2 x steps, steps ~ the low-field drift time from its mean depth,
+  // ln(a2 / (a2 - a1 z)) (eq. 1 with constant mobility); plain z where that is undefined.  Order only: never physics.
+  const uint32_t* cnt = B.h_cnt;
+  const double a1u = h->dp.a1_um, a2 = h->dp.a2;
+  const bool lin = (h->dp.flags & GCORECCD_DEPLETION_OFF) || !(a1u > 0.0) || !(a2 > 0.0);
+  for (size_t k = 0; k < ne; ++k) {
+    const double z = zmean[k] > 0.f ? (double)zmean[k] : 0.0;
+    const double r = lin ? 0.0 : std::min(a1u * z / a2, 0.98);
+    const double steps = lin ? z : -std::log1p(-r);
+    zmean[k] = (float)((double)cnt[k] * (double)cnt[k] * (steps + 1e-3));
+  }
+  const float* cost = zmean;
+  auto by_size = [cost](uint32_t a, uint32_t b) { return cost[a] != cost[b] ? cost[a] > cost[b] : a < b; };
+  const uint32_t lim[4] = {0u, kEvCapTiny, kEvCapSmall, kEvCapLarge};
+  uint32_t filled = 0;
+  for (int q = 0; q < 3; ++q) {
+    const uint32_t first = filled;
+    for (size_t k = 0; k < ne; ++k)
+      if ((q == 0 ? true : B.h_cnt[k] > lim[q]) && B.h_cnt[k] <= lim[q + 1]) order[filled++] = (uint32_t)k;
+    std::sort(order + first, order + filled, by_size);
+    B.n_q[q] = filled - first;
+  }
+  free(zmean);
+  e = cudaMemcpyAsync(B.d_order, order, ne * 4, cudaMemcpyHostToDevice, h->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
   free(order);
   if (e != cudaSuccess) { drop_events(h); return fail(h, GCORECCD_ERR_CUDA, "load_events", e); }
 
   // persistent grids: resident CTAs per SM x SM count
-  const size_t sm_small = event_smem_bytes(kEvCapSmall), sm_large = event_smem_bytes(kEvCapLarge);
-  int occ_s = 0, occ_l = 0;
-  e = cudaFuncSetAttribute(k_events<1, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_small);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_events<4, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_large);
-  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_s, k_events<1, 3>, kTPB, sm_small);
-  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_l, k_events<4, 1>, kTPB, sm_large);
+  const size_t smem[3] = {event_smem_bytes(kEvCapTiny), event_smem_bytes(kEvCapSmall), event_smem_bytes(kEvCapLarge)};
+  int occ[3] = {0, 0, 0};
+  e = cudaFuncSetAttribute(k_events<4, 256, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem[2]);
+  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[0], k_events<1, 64, 12>, 64, smem[0]);
+  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[1], k_events<1, 256, 3>, 256, smem[1]);
+  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[2], k_events<4, 256, 1>, 256, smem[2]);
   if (e != cudaSuccess) { drop_events(h); return fail(h, GCORECCD_ERR_CUDA, "load_events: kernel attributes", e); }
-  B.grid_small = h->num_sms * (occ_s > 0 ? occ_s : 1);
-  B.grid_large = h->num_sms * (occ_l > 0 ? occ_l : 1);
+  for (int q = 0; q < 3; ++q) B.grid_q[q] = h->num_sms * (occ[q] > 0 ? occ[q] : 1);
+  e = cudaEventCreateWithFlags(&B.fork, cudaEventDisableTiming);
+  for (int k = 0; k < 2 && e == cudaSuccess; ++k) {
+    e = cudaStreamCreateWithFlags(&B.aux[k], cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&B.join[k], cudaEventDisableTiming);
+  }
+  if (e != cudaSuccess) { drop_events(h); return fail(h, GCORECCD_ERR_CUDA, "load_events: streams", e); }
   B.loaded = true;
   B.n_events = n_events; B.n_carriers = n;
   B.events_left = left_events; B.carriers_left = n;
@@ -694,19 +731,33 @@ int gcoreccd_run_events(gcoreccd_t* h, uint64_t max_steps, uint64_t* events_left
   int ret = GCORECCD_OK;
   if (B.carriers_left > 0) {
     const EventTable tab{B.d_off, B.d_cnt, B.d_step};
-    GC_CUDA(h, cudaMemsetAsync(B.d_queue, 0, 8, h->stream));
-    // the large events first: they are the long poles; the small queue fills the SMs as they drain
-    if (B.n_large) {
-      const int g = (int)std::min<uint32_t>(B.n_large, (uint32_t)B.grid_large);
-      k_events<4, 1><<<g, kTPB, event_smem_bytes(kEvCapLarge), h->stream>>>(h->A, tab, B.d_order + B.n_small, B.n_large, B.d_queue + 1,
-                                                                          h->ctrl, h->image, h->dp, max_steps, kEvCapLarge);
+    GC_CUDA(h, cudaMemsetAsync(B.d_queue, 0, 12, h->stream));
+    // one kernel per queue, forked onto side streams so that the small events fill the SMs the large ones leave
+    const uint32_t first[3] = {0u, B.n_q[0], B.n_q[0] + B.n_q[1]};
+    GC_CUDA(h, cudaEventRecord(B.fork, h->stream));
+    if (B.n_q[2]) {
+      const int g = (int)std::min<uint32_t>(B.n_q[2], (uint32_t)B.grid_q[2]);
+      k_events<4, 256, 1><<<g, 256, event_smem_bytes(kEvCapLarge), h->stream>>>(h->A, tab, B.d_order + first[2], B.n_q[2], B.d_queue + 2,
+                                                                              h->ctrl, h->image, h->dp, max_steps, kEvCapLarge);
       h->launches += 1;
     }
-    if (B.n_small) {
-      const int g = (int)std::min<uint32_t>(B.n_small, (uint32_t)B.grid_small);
-      k_events<1, 3><<<g, kTPB, event_smem_bytes(kEvCapSmall), h->stream>>>(h->A, tab, B.d_order, B.n_small, B.d_queue, h->ctrl,
-                                                                          h->image, h->dp, max_steps, kEvCapSmall);
+    if (B.n_q[1]) {
+      GC_CUDA(h, cudaStreamWaitEvent(B.aux[0], B.fork, 0));
+      const int g = (int)std::min<uint32_t>(B.n_q[1], (uint32_t)B.grid_q[1]);
+      k_events<1, 256, 3><<<g, 256, event_smem_bytes(kEvCapSmall), B.aux[0]>>>(h->A, tab, B.d_order + first[1], B.n_q[1], B.d_queue + 1,
+                                                                             h->ctrl, h->image, h->dp, max_steps, kEvCapSmall);
       h->launches += 1;
+      GC_CUDA(h, cudaEventRecord(B.join[0], B.aux[0]));
+      GC_CUDA(h, cudaStreamWaitEvent(h->stream, B.join[0], 0));
+    }
+    if (B.n_q[0]) {
+      GC_CUDA(h, cudaStreamWaitEvent(B.aux[1], B.fork, 0));
+      const int g = (int)std::min<uint32_t>(B.n_q[0], (uint32_t)B.grid_q[0]);
+      k_events<1, 64, 12><<<g, 64, event_smem_bytes(kEvCapTiny), B.aux[1]>>>(h->A, tab, B.d_order, B.n_q[0], B.d_queue, h->ctrl,
+                                                                           h->image, h->dp, max_steps, kEvCapTiny);
+      h->launches += 1;
+      GC_CUDA(h, cudaEventRecord(B.join[1], B.aux[1]));
+      GC_CUDA(h, cudaStreamWaitEvent(h->stream, B.join[1], 0));
     }
     GC_CUDA(h, cudaGetLastError());
     GC_CUDA(h, cudaMemcpyAsync(B.h_cnt, B.d_cnt, B.n_events * 4, cudaMemcpyDeviceToHost, h->stream));
