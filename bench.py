@@ -152,7 +152,7 @@ def run_reference(args):
 def run_ours(args):
     import torch
     import torch.distributed as dist
-    from paper_2203_11043_b200 import binding, workloads
+    from paper_2203_11043_b200 import binding, replicas, workloads
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -164,7 +164,7 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     peaks, peak_src = measured_peaks()
 
-    w = workloads.make(WORKLOAD_CFG, seed=workloads.SEED + rank)       # replicas: one independent event per rank
+    w = workloads.make(WORKLOAD_CFG, seed=replicas.rank_seed(workloads.SEED, rank))   # replicas: one event per rank
     P, xyz = w["params"], w["xyz"]
     n = len(xyz)
     stream = torch.cuda.Stream()                                       # the handle, the flush and the events share it
@@ -201,12 +201,7 @@ def run_ours(args):
     launches = sim.kernel_launches() - l0
     st = sim.state()
     pairs = st["pair_interactions"] - p0
-    tms = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    tp = torch.tensor([float(pairs)], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
-        dist.all_reduce(tp, op=dist.ReduceOp.SUM)
-    ms_max, pairs_all = float(tms.item()), float(tp.item())
+    ms_max, pairs_all = replicas.aggregate(ms, pairs, device="cuda")     # max over ranks of the device time, summed work
     value = pairs_all / (ms_max * 1e-3) / 1e9
 
     # ---- roofline of the dominant kernel (field), CUDA events inside the library on its launching stream
@@ -247,10 +242,8 @@ def run_ours(args):
         assert got <= n
     barrier()
     e2e_s = time.perf_counter() - t0
-    te = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_value = world * e2e_pairs / float(te.item()) / 1e9
+    e2e_ms, e2e_pairs_all = replicas.aggregate(e2e_s * 1e3, e2e_pairs, device="cuda")
+    e2e_value = e2e_pairs_all / (e2e_ms * 1e-3) / 1e9
 
     # ---- seconds per 131k-hole event (second half of BASELINE.json's metric): load -> full collection
     event = None
