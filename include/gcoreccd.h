@@ -122,6 +122,13 @@ int gcoreccd_get_state(gcoreccd_t* h, uint64_t* step, uint64_t* n_active, uint64
  * may be NULL.  *n receives the active count; fails with CAPACITY if cap < count.  Same on_device flag for both. */
 int gcoreccd_read_carriers(gcoreccd_t* h, float* xyz_um, uint32_t* id, uint64_t cap, uint64_t* n, int on_device);
 
+/* Final positions (the image is "the histogram of the output positions"; "save the final
+ * results"): for every carrier id < min(n_loaded, max_carriers), its x,y,z (um) after the step in which it crossed
+ * z_well and the index of that step (the current step index for holes collected at load); NaN / 0xFFFFFFFF while it is
+ * still drifting.  Host buffers of cap entries (3 floats / 1 uint32 per id), both or neither; *n receives the count.
+ * Step indices are recorded modulo 2^32. */
+int gcoreccd_read_collected(gcoreccd_t* h, float* xyz_um_host, uint32_t* step_host, uint64_t cap, uint64_t* n);
+
 /* Coulomb field (eq. 6, V/cm) of the current snapshot, interleaved Ex,Ey,Ez in read_carriers order;
  * does not advance the simulation.  cap = number of carriers the buffer holds. */
 int gcoreccd_eval_field(gcoreccd_t* h, float* Exyz_V_per_cm, uint64_t cap, int on_device);

@@ -18,7 +18,7 @@ COULOMB_OFF, DIFFUSION_OFF, DEPLETION_OFF = 1, 2, 4
 
 EXPORTS = ["gcoreccd_workspace_size", "gcoreccd_create", "gcoreccd_destroy", "gcoreccd_reset",
            "gcoreccd_load_carriers", "gcoreccd_load_snapshot", "gcoreccd_step", "gcoreccd_run_to_collection",
-           "gcoreccd_read_image", "gcoreccd_get_state", "gcoreccd_read_carriers", "gcoreccd_eval_field",
+           "gcoreccd_read_image", "gcoreccd_get_state", "gcoreccd_read_carriers", "gcoreccd_read_collected", "gcoreccd_eval_field",
            "gcoreccd_load_events", "gcoreccd_run_events", "gcoreccd_get_events", "gcoreccd_read_event_carriers",
            "gcoreccd_profile_step", "gcoreccd_kernel_launches", "gcoreccd_debug_normals", "gcoreccd_strerror",
            "gcoreccd_last_error", "gcoreccd_version"]
@@ -80,6 +80,8 @@ def lib():
     L.gcoreccd_get_state.argtypes = [vp, u64p, u64p, u64p, u64p, u64p, u64p]
     L.gcoreccd_read_carriers.restype = C.c_int
     L.gcoreccd_read_carriers.argtypes = [vp, vp, vp, C.c_uint64, u64p, C.c_int]
+    L.gcoreccd_read_collected.restype = C.c_int
+    L.gcoreccd_read_collected.argtypes = [vp, vp, vp, C.c_uint64, u64p]
     L.gcoreccd_eval_field.restype = C.c_int
     L.gcoreccd_eval_field.argtypes = [vp, vp, C.c_uint64, C.c_int]
     L.gcoreccd_load_events.restype = C.c_int
@@ -292,6 +294,18 @@ class Gcoreccd:
             self._check(lib().gcoreccd_read_carriers(self._h, C.c_void_p(xyz.ctypes.data), C.c_void_p(ids.ctypes.data),
                                                      k, C.byref(n), 0), "gcoreccd_read_carriers")
         return xyz, ids
+
+    def read_collected(self):
+        """(xyz float32 (n,3), step uint32 (n,)) indexed by carrier id; NaN / 0xFFFFFFFF while still drifting."""
+        n = C.c_uint64()
+        self._check(lib().gcoreccd_read_collected(self._h, None, None, 0, C.byref(n)), "gcoreccd_read_collected")
+        k = int(n.value)
+        xyz = np.zeros((k, 3), dtype=np.float32)
+        st = np.zeros(k, dtype=np.uint32)
+        if k:
+            self._check(lib().gcoreccd_read_collected(self._h, C.c_void_p(xyz.ctypes.data), C.c_void_p(st.ctypes.data), k,
+                                                      C.byref(n)), "gcoreccd_read_collected")
+        return xyz, st
 
     def read_carriers_into(self, host_ptr_xyz, cap):
         n = C.c_uint64()

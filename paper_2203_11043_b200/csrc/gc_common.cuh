@@ -64,6 +64,12 @@ struct DevParams {            // constants uploaded by value with every launch
   int32_t nx, ny;
 };
 
+struct Sink {                 // where a collected hole goes (a7)
+  uint32_t* image;            // [ny][nx] integer pixel histogram
+  float4* fin;                // per-id record (x, y, z at collection, bits(step index)); all-ones = still drifting
+  uint32_t fin_cap;           // ids >= fin_cap are binned but not recorded
+};
+
 struct PlanArgs { uint32_t IB; uint32_t grid; uint32_t part_cap_entries; };
 
 #ifdef __CUDACC__

@@ -117,7 +117,7 @@ __device__ __forceinline__ void event_pass(const float4* s_xy, const float2* s_z
 template <int NPACK, int TPB, int MINB>        // NPACK is 1 (tiny / small events) or 4 (large events)
 __global__ void __launch_bounds__(TPB, MINB)
 k_events(SoA A, EventTable ev, const uint32_t* __restrict__ order, uint32_t n_order, uint32_t* __restrict__ queue,
-         Ctrl* __restrict__ ctrl, uint32_t* __restrict__ image, DevParams P, uint64_t max_steps, uint32_t cap) {
+         Ctrl* __restrict__ ctrl, Sink sink, DevParams P, uint64_t max_steps, uint32_t cap) {
   extern __shared__ __align__(16) unsigned char smem[];
   float4* s_xy = reinterpret_cast<float4*>(smem);                       // (x,x,y,y), cap + 4 entries
   float4* s_next = s_xy + (cap + 4);                                    // (x',y',z',id), cap entries
@@ -153,7 +153,7 @@ k_events(SoA A, EventTable ev, const uint32_t* __restrict__ order, uint32_t n_or
       uint32_t keep = 0, coll = 0, over = 0;
       for (uint32_t i = lo; i < hi; ++i) {
         const float4 c = s_next[i];
-        if ((double)c.z <= P.z_well) { coll += 1; collect(c.x, c.y, P, image, over); }
+        if ((double)c.z <= P.z_well) { coll += 1; collect(c.x, c.y, c.z, __float_as_uint(c.w), step, P, sink, over); }
         else keep += 1;
       }
       uint32_t incl = keep;                                             // block exclusive scan of the survivor counts

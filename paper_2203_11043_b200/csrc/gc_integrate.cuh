@@ -51,14 +51,17 @@ __device__ __forceinline__ double mobility(double E, const DevParams& P) {
   return P.mu0 * exp(-P.inv_beta * log1p(t));
 }
 
-// a7: half-open pixel bins, floor, in FP64 on the stored FP32 position (exactly reproducible).
-__device__ __forceinline__ void collect(float x, float y, const DevParams& P, uint32_t* image, uint32_t& n_over) {
+// a7: half-open pixel bins, floor, in FP64 on the stored FP32 position (exactly reproducible); the final position
+// and the index of the crossing step are recorded per carrier id ("output positions").
+__device__ __forceinline__ void collect(float x, float y, float z, uint32_t id, uint64_t step, const DevParams& P,
+                                        const Sink& sink, uint32_t& n_over) {
   const double fx = floor(((double)x - P.x0) / P.pitch);
   const double fy = floor(((double)y - P.y0) / P.pitch);
   if (fx >= 0.0 && fx < (double)P.nx && fy >= 0.0 && fy < (double)P.ny)
-    atomicAdd(image + (size_t)fy * (size_t)P.nx + (size_t)fx, 1u);
+    atomicAdd(sink.image + (size_t)fy * (size_t)P.nx + (size_t)fx, 1u);
   else
     n_over += 1u;
+  if (id < sink.fin_cap) sink.fin[id] = make_float4(x, y, z, __uint_as_float((uint32_t)step));
 }
 
 // Sum of the S column-chunk partials of one target, in FP64 and in fixed (ascending chunk) order.  The loads of
@@ -128,7 +131,7 @@ __device__ __forceinline__ void tally(uint32_t coll, uint32_t over, uint32_t kee
 // the tile's survivor count.  Grid is sized from the host's upper bound on n_active; surplus CTAs exit.
 __global__ void __launch_bounds__(kTPB, 4)      // 64 registers: 4 CTAs/SM, 151,552 carriers in one wave on 148 SMs
 k_integrate(SoA A, SoA B, Ctrl* __restrict__ ctrl, const float* __restrict__ Ep, uint32_t part_cap,
-            uint32_t* __restrict__ image, uint32_t* __restrict__ tile_count, DevParams P) {
+            Sink sink, uint32_t* __restrict__ tile_count, DevParams P) {
   const uint32_t n = ctrl->n_active;
   const uint32_t i = blockIdx.x * kTPB + threadIdx.x;
   if (blockIdx.x * kTPB >= n) return;
@@ -145,7 +148,7 @@ k_integrate(SoA A, SoA B, Ctrl* __restrict__ ctrl, const float* __restrict__ Ep,
     float xf, yf, zf;
     if (!advance_carrier(x, y, z, id, step, Ex, Ey, Ez, P, xf, yf, zf)) atomicOr(&ctrl->nonfinite, 1u);
     B.x[i] = xf; B.y[i] = yf; B.z[i] = zf; B.id[i] = id;
-    if ((double)zf <= P.z_well) { coll = 1; uint32_t o = 0; collect(xf, yf, P, image, o); over = o; }
+    if ((double)zf <= P.z_well) { coll = 1; uint32_t o = 0; collect(xf, yf, zf, id, step, P, sink, o); over = o; }
     else keep = 1;
   }
   tally(coll, over, keep, ctrl, tile_count);
@@ -154,13 +157,14 @@ k_integrate(SoA A, SoA B, Ctrl* __restrict__ ctrl, const float* __restrict__ Ep,
 // Load path: unpack interleaved xyz into state B at [0,n), assign ids n_loaded + k, collect z <= z_well.
 __global__ void __launch_bounds__(kTPB)
 k_unpack(const float* __restrict__ xyz, uint32_t n, SoA B, Ctrl* __restrict__ ctrl, uint32_t id_base,
-         uint32_t* __restrict__ image, uint32_t* __restrict__ tile_count, DevParams P) {
+         Sink sink, uint32_t* __restrict__ tile_count, DevParams P) {
   const uint32_t i = blockIdx.x * kTPB + threadIdx.x;
   uint32_t coll = 0, over = 0, keep = 0;
+  const uint64_t step = ctrl->step;
   if (i < n) {
     const float x = xyz[3 * (size_t)i], y = xyz[3 * (size_t)i + 1], z = xyz[3 * (size_t)i + 2];
     B.x[i] = x; B.y[i] = y; B.z[i] = z; B.id[i] = id_base + i;
-    if ((double)z <= P.z_well) { coll = 1; uint32_t o = 0; collect(x, y, P, image, o); over = o; }
+    if ((double)z <= P.z_well) { coll = 1; uint32_t o = 0; collect(x, y, z, id_base + i, step, P, sink, o); over = o; }
     else keep = 1;
   }
   tally(coll, over, keep, ctrl, tile_count);
@@ -194,6 +198,16 @@ k_interleave(SoA A, const Ctrl* __restrict__ ctrl, float* __restrict__ xyz) {
   const uint32_t i = blockIdx.x * kTPB + threadIdx.x;
   if (i >= n) return;
   xyz[3 * (size_t)i] = A.x[i]; xyz[3 * (size_t)i + 1] = A.y[i]; xyz[3 * (size_t)i + 2] = A.z[i];
+}
+
+// read_collected: per-id records -> interleaved xyz (NaN while drifting) and the crossing step (all-ones likewise)
+__global__ void __launch_bounds__(kTPB)
+k_read_final(const float4* __restrict__ fin, uint32_t n, float* __restrict__ xyz, uint32_t* __restrict__ step) {
+  const uint32_t i = blockIdx.x * kTPB + threadIdx.x;
+  if (i >= n) return;
+  const float4 f = fin[i];
+  xyz[3 * (size_t)i] = f.x; xyz[3 * (size_t)i + 1] = f.y; xyz[3 * (size_t)i + 2] = f.z;
+  step[i] = __float_as_uint(f.w);
 }
 
 // load_snapshot: replace the active set

@@ -26,7 +26,7 @@ constexpr int kGraphSteps = 8;                        // steps per CUDA-graph la
 
 struct Layout {
   uint64_t cap_pad, part_cap, n_tiles;
-  uint64_t off_ctrl, off_A, off_B, off_Ep, off_tiles, off_image, total;
+  uint64_t off_ctrl, off_A, off_B, off_Ep, off_tiles, off_image, off_fin, total;
 };
 
 inline uint64_t align_up(uint64_t v, uint64_t a) { return (v + a - 1) / a * a; }
@@ -43,6 +43,7 @@ Layout make_layout(uint64_t max_carriers, int32_t nx, int32_t ny) {
   L.off_Ep = o;    o += align_up(3 * L.part_cap * 4, 256);
   L.off_tiles = o; o += align_up(L.n_tiles * 4, 256);
   L.off_image = o; o += align_up((uint64_t)nx * (uint64_t)ny * 4, 256);
+  L.off_fin = o;   o += align_up(L.cap_pad * 16, 256);
   L.total = o;
   return L;
 }
@@ -64,6 +65,8 @@ struct gcoreccd {
   float* Ep;
   uint32_t* tile_count;
   uint32_t* image;
+  float4* fin;                  // per-id collection records
+  Sink sink;
   uint64_t n_loaded;            // host copy (ids continue)
   uint64_t n_bound;             // host upper bound on n_active
   int variant;                  // current field variant (-1 = none yet)
@@ -156,7 +159,7 @@ int launch_field(gcoreccd_t* h, int v) {
 void enqueue_step(gcoreccd_t* h, uint32_t tiles) {
   const bool coulomb = !(h->dp.flags & GCORECCD_COULOMB_OFF);
   if (coulomb) launch_field(h, h->variant);
-  k_integrate<<<tiles, kTPB, 0, h->stream>>>(h->A, h->B, h->ctrl, h->Ep, (uint32_t)h->L.part_cap, h->image,
+  k_integrate<<<tiles, kTPB, 0, h->stream>>>(h->A, h->B, h->ctrl, h->Ep, (uint32_t)h->L.part_cap, h->sink,
                                              h->tile_count, h->dp);
   k_compact<<<tiles, kTPB, 0, h->stream>>>(h->B, h->A, h->ctrl, h->tile_count, 0u, 0u, 0, h->dp.z_well,
                                            coulomb ? 1u : 0u, plan_args(h, h->variant));
@@ -310,6 +313,8 @@ int gcoreccd_create(const gcoreccd_params* p, gcoreccd_t** out) {
   h->Ep = (float*)(h->ws + h->L.off_Ep);
   h->tile_count = (uint32_t*)(h->ws + h->L.off_tiles);
   h->image = (uint32_t*)(h->ws + h->L.off_image);
+  h->fin = (float4*)(h->ws + h->L.off_fin);
+  h->sink = Sink{h->image, h->fin, (uint32_t)std::min<uint64_t>(p->max_carriers, 0xffffffffull)};
 
   // constants (eq. 2 temperature terms, K', thermal voltage) folded on the host in FP64
   const double q = 1.602176634e-19, kB = 1.380649e-23, eps0 = 8.8541878128e-12, pi = 3.14159265358979323846;
@@ -367,6 +372,7 @@ int gcoreccd_reset(gcoreccd_t* h) {
   DeviceGuard guard(h->device);
   GC_CUDA(h, cudaMemsetAsync(h->ctrl, 0, sizeof(Ctrl), h->stream));
   GC_CUDA(h, cudaMemsetAsync(h->image, 0, (size_t)h->p.img_nx * h->p.img_ny * 4, h->stream));
+  GC_CUDA(h, cudaMemsetAsync(h->fin, 0xff, (size_t)h->L.cap_pad * 16, h->stream));     // NaN / all-ones = still drifting
   GC_CUDA(h, cudaStreamSynchronize(h->stream));
   drop_events(h);
   h->n_loaded = 0;
@@ -400,7 +406,7 @@ int gcoreccd_load_carriers(gcoreccd_t* h, const float* xyz, uint64_t n, int on_d
   // the plan stored with the new n_active must match the variant the next step will use
   const int v = pick_variant(n_act + n);
   h->variant = v;
-  k_unpack<<<tiles, kTPB, 0, h->stream>>>(src, (uint32_t)n, h->B, h->ctrl, (uint32_t)h->n_loaded, h->image,
+  k_unpack<<<tiles, kTPB, 0, h->stream>>>(src, (uint32_t)n, h->B, h->ctrl, (uint32_t)h->n_loaded, h->sink,
                                           h->tile_count, h->dp);
   k_compact<<<tiles, kTPB, 0, h->stream>>>(h->B, h->A, h->ctrl, h->tile_count, (uint32_t)n, (uint32_t)n_act, 1,
                                            h->dp.z_well, 0u, plan_args(h, v));
@@ -519,6 +525,26 @@ int gcoreccd_read_carriers(gcoreccd_t* h, float* xyz, uint32_t* id, uint64_t cap
   return GCORECCD_OK;
 }
 
+int gcoreccd_read_collected(gcoreccd_t* h, float* xyz, uint32_t* step, uint64_t cap, uint64_t* n) {
+  if (!h) return GCORECCD_ERR_INVALID;
+  const uint64_t m = std::min<uint64_t>(h->n_loaded, h->sink.fin_cap);
+  if (n) *n = m;
+  if (!xyz && !step) return GCORECCD_OK;
+  if (!xyz || !step) return fail(h, GCORECCD_ERR_INVALID, "read_collected: pass both buffers or neither");
+  if (cap < m) return fail(h, GCORECCD_ERR_CAPACITY, "read_collected: buffer too small");
+  if (m == 0) return GCORECCD_OK;
+  DeviceGuard guard(h->device);
+  float* st_xyz = h->Ep;                                   // partials are scratch between steps
+  uint32_t* st_step = (uint32_t*)(h->Ep + 3 * h->L.cap_pad);
+  k_read_final<<<tiles_for(m), kTPB, 0, h->stream>>>(h->fin, (uint32_t)m, st_xyz, st_step);
+  h->launches += 1;
+  GC_CUDA(h, cudaGetLastError());
+  GC_CUDA(h, cudaMemcpyAsync(xyz, st_xyz, m * 12, cudaMemcpyDeviceToHost, h->stream));
+  GC_CUDA(h, cudaMemcpyAsync(step, st_step, m * 4, cudaMemcpyDeviceToHost, h->stream));
+  GC_CUDA(h, cudaStreamSynchronize(h->stream));
+  return GCORECCD_OK;
+}
+
 int gcoreccd_eval_field(gcoreccd_t* h, float* E, uint64_t cap, int on_device) {
   if (!h || !E) return GCORECCD_ERR_INVALID;
   DeviceGuard guard(h->device);
@@ -551,7 +577,7 @@ int gcoreccd_profile_step(gcoreccd_t* h, float ms[4]) {
   GC_CUDA(h, cudaEventRecord(h->ev[0], h->stream));
   if (coulomb) launch_field(h, h->variant);
   GC_CUDA(h, cudaEventRecord(h->ev[1], h->stream));
-  k_integrate<<<tiles, kTPB, 0, h->stream>>>(h->A, h->B, h->ctrl, h->Ep, (uint32_t)h->L.part_cap, h->image,
+  k_integrate<<<tiles, kTPB, 0, h->stream>>>(h->A, h->B, h->ctrl, h->Ep, (uint32_t)h->L.part_cap, h->sink,
                                              h->tile_count, h->dp);
   GC_CUDA(h, cudaEventRecord(h->ev[2], h->stream));
   k_compact<<<tiles, kTPB, 0, h->stream>>>(h->B, h->A, h->ctrl, h->tile_count, 0u, 0u, 0, h->dp.z_well,
@@ -738,14 +764,14 @@ int gcoreccd_run_events(gcoreccd_t* h, uint64_t max_steps, uint64_t* events_left
     if (B.n_q[2]) {
       const int g = (int)std::min<uint32_t>(B.n_q[2], (uint32_t)B.grid_q[2]);
       k_events<4, 256, 1><<<g, 256, event_smem_bytes(kEvCapLarge), h->stream>>>(h->A, tab, B.d_order + first[2], B.n_q[2], B.d_queue + 2,
-                                                                              h->ctrl, h->image, h->dp, max_steps, kEvCapLarge);
+                                                                              h->ctrl, h->sink, h->dp, max_steps, kEvCapLarge);
       h->launches += 1;
     }
     if (B.n_q[1]) {
       GC_CUDA(h, cudaStreamWaitEvent(B.aux[0], B.fork, 0));
       const int g = (int)std::min<uint32_t>(B.n_q[1], (uint32_t)B.grid_q[1]);
       k_events<1, 256, 3><<<g, 256, event_smem_bytes(kEvCapSmall), B.aux[0]>>>(h->A, tab, B.d_order + first[1], B.n_q[1], B.d_queue + 1,
-                                                                             h->ctrl, h->image, h->dp, max_steps, kEvCapSmall);
+                                                                             h->ctrl, h->sink, h->dp, max_steps, kEvCapSmall);
       h->launches += 1;
       GC_CUDA(h, cudaEventRecord(B.join[0], B.aux[0]));
       GC_CUDA(h, cudaStreamWaitEvent(h->stream, B.join[0], 0));
@@ -754,7 +780,7 @@ int gcoreccd_run_events(gcoreccd_t* h, uint64_t max_steps, uint64_t* events_left
       GC_CUDA(h, cudaStreamWaitEvent(B.aux[1], B.fork, 0));
       const int g = (int)std::min<uint32_t>(B.n_q[0], (uint32_t)B.grid_q[0]);
       k_events<1, 64, 12><<<g, 64, event_smem_bytes(kEvCapTiny), B.aux[1]>>>(h->A, tab, B.d_order, B.n_q[0], B.d_queue, h->ctrl,
-                                                                           h->image, h->dp, max_steps, kEvCapTiny);
+                                                                           h->sink, h->dp, max_steps, kEvCapTiny);
       h->launches += 1;
       GC_CUDA(h, cudaEventRecord(B.join[1], B.aux[1]));
       GC_CUDA(h, cudaStreamWaitEvent(h->stream, B.join[1], 0));

@@ -225,3 +225,28 @@ def test_batch_edge_cases_and_error_codes():
     with pytest.raises(binding.GcoreccdError):
         sim.events()
     sim.close()
+
+
+def test_batch_records_final_positions_per_id():
+    sizes = [40, 300, 0, 900]
+    w = workloads.make_events(sizes, seed=5, depth_range=(20.0, 60.0))
+    n = len(w["xyz"])
+    sim = gpu_sim(w, max_carriers=n)
+    sim.load_events(w["xyz"], w["offsets"])
+    sim.run_events()
+    fin, st = sim.read_collected()
+    act, stp = sim.events()
+    assert len(fin) == n and not np.isnan(fin).any() and (fin[:, 2] <= 0.0).all()
+    for e in range(len(sizes)):
+        lo, hi = int(w["offsets"][e]), int(w["offsets"][e + 1])
+        if hi > lo:
+            assert st[lo:hi].max() == stp[e] - 1                               # the event ended with its last hole
+            o, _ = _oracle_event(w, e, 0)
+            o.run()
+            ofin, ost = o.collected()
+            # statistical agreement of the collected cloud (chaotic run): centroid and rms radius
+            c, oc = fin[lo:hi, :2].astype(np.float64), ofin[lo:hi, :2]
+            r, ro = np.sqrt(c.var(axis=0).sum()), np.sqrt(oc.var(axis=0).sum())
+            assert np.linalg.norm(c.mean(axis=0) - oc.mean(axis=0)) <= 4.0 * ro / np.sqrt(hi - lo) + 1e-3
+            assert abs(r - ro) <= max(0.05 * ro, 4.0 * ro / np.sqrt(2.0 * (hi - lo)))
+    sim.close()

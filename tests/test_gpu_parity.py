@@ -328,3 +328,44 @@ def test_device_pointer_load_and_library_owned_workspace():
     dimg, _ = s.read_image(device=True)
     assert dimg.is_cuda and int(dimg.sum()) == int(s.read_image()[0].sum())
     a.close(); s.close()
+
+
+# ------------------------------------------------------------------ final positions ("output positions")
+def test_collected_positions_and_steps_match_the_oracle():
+    w = workloads.make(0, n=900)
+    xyz = w["xyz"].copy()
+    xyz[:, 2] = np.abs(xyz[:, 2] - 200.0) * 4.0 + 0.5          # 0.5 .. ~15 um above the collection plane
+    xyz[:7, 2] = [0.0, -0.5, 0.0, -2.0, 0.0, 0.0, -1e-3]       # collected at load, recorded with step 0
+    sim = gpu_sim(w)
+    sim.load_carriers(xyz)
+    o = oracle_sim(w, flags=g.FP32_STATE)
+    o.load(xyz)
+    sim.step(10)
+    o.step(10)
+    fin, st = sim.read_collected()
+    ofin, ost = o.collected()
+    assert len(fin) == len(ofin) == 900
+    got, ref = st != 0xFFFFFFFF, ost != np.iinfo(np.uint64).max
+    assert got[:7].all() and (st[:7] == 0).all() and np.array_equal(fin[:7], xyz[:7])
+    assert np.isnan(fin[~got]).all()
+    both = got & ref
+    assert both.sum() > 300 and (got != ref).sum() <= 4          # retire-flag mismatches only at the plane
+    assert np.array_equal(st[both].astype(np.uint64), ost[both]) or (st[both] != ost[both]).sum() <= 2
+    same = both & (st.astype(np.uint64) == ost)
+    d = np.abs(fin[same].astype(np.float64) - ofin[same]).max(axis=1)
+    assert np.quantile(d, 0.98) <= 2e-4 and (d > TRAJ_TOL).mean() <= 0.02, d.max()
+    # the image is the histogram of exactly these positions (a7), and every hole is accounted for
+    sim.run_to_collection()
+    fin, st = sim.read_collected()
+    img, over = sim.read_image()
+    P = w["params"]
+    ix = np.floor((fin[:, 0].astype(np.float64) - P["img_x0_um"]) / P["pixel_pitch_um"]).astype(np.int64)
+    iy = np.floor((fin[:, 1].astype(np.float64) - P["img_y0_um"]) / P["pixel_pitch_um"]).astype(np.int64)
+    ok = (ix >= 0) & (ix < P["img_nx"]) & (iy >= 0) & (iy < P["img_ny"])
+    hist = np.zeros_like(img)
+    np.add.at(hist, (iy[ok], ix[ok]), 1)
+    assert np.array_equal(hist, img) and int((~ok).sum()) == over
+    assert (fin[:, 2] <= P["z_well_um"]).all() and st.max() == sim.state()["step"] - 1
+    sim.reset()
+    assert len(sim.read_collected()[0]) == 0
+    sim.close()
