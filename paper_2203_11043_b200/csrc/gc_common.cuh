@@ -40,7 +40,7 @@ struct Ctrl {                 // lives in device memory; only kernels write it (
   uint32_t nonfinite;         // sticky flag
   uint32_t invalid;           // load validation flag
   uint32_t blocks_done;       // "last block finishes" counter of the compactor
-  uint32_t pad_;
+  uint32_t multi_steps;       // scratch of the Coulomb-off multi-step kernel: steps the longest-lived carrier took
   FieldPlan plan;             // valid for (n_active, current field variant)
   uint32_t pad2_[2];
 };

@@ -12,14 +12,15 @@ namespace gc {
 
 // src: m entries of state B (m = n_active for a step, = n for a load); survivors (z > z_well) are appended to
 // dst (state A) starting at dst_off.  mode 0: time step (m read from ctrl->n_active, dst_off = 0, step += 1,
-// pairs += m^2 unless Coulomb is off);  mode 1: load (m, dst_off given; n_loaded += m).
+// pairs += m^2 unless Coulomb is off);  mode 1: load (m, dst_off given; n_loaded += m);  mode 2: as mode 0 after
+// k_drift_multi (step += ctrl->multi_steps, which is cleared).
 __global__ void __launch_bounds__(kTPB)
 k_compact(SoA B, SoA A, Ctrl* __restrict__ ctrl, const uint32_t* __restrict__ tile_count, uint32_t m_arg,
           uint32_t dst_off_arg, int mode, double z_well, uint32_t count_pairs, PlanArgs pa) {
   __shared__ uint32_t s_red[kTPB / 32];
   __shared__ uint32_t s_base, s_last;
-  const uint32_t m = mode == 0 ? ctrl->n_active : m_arg;
-  const uint32_t dst_off = mode == 0 ? 0u : dst_off_arg;
+  const uint32_t m = mode != 1 ? ctrl->n_active : m_arg;
+  const uint32_t dst_off = mode != 1 ? 0u : dst_off_arg;
   if (m == 0) return;                                     // uniform: every CTA sees the same m; no step is taken
   const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
   const uint32_t t = blockIdx.x;
@@ -83,6 +84,9 @@ k_compact(SoA B, SoA A, Ctrl* __restrict__ ctrl, const uint32_t* __restrict__ ti
       if (mode == 0) {
         ctrl->step += 1;
         if (count_pairs) ctrl->pairs += (uint64_t)m * (uint64_t)m;
+      } else if (mode == 2) {
+        ctrl->step += ctrl->multi_steps;
+        ctrl->multi_steps = 0;
       } else {
         ctrl->n_loaded += m;
       }

@@ -154,6 +154,39 @@ k_integrate(SoA A, SoA B, Ctrl* __restrict__ ctrl, const float* __restrict__ Ep,
   tally(coll, over, keep, ctrl, tile_count);
 }
 
+// Coulomb OFF (the O(N) mode): without eq. 6 the carriers are independent, so one launch takes
+// every carrier through up to n_steps steps (or to collection) instead of one launch train per step.  Same
+// advance_carrier, same Philox counters (id, step): bit-identical to n_steps single steps.  The step index advances
+// by the steps the longest-lived carrier needed (a step with nobody drifting is a no-op), via ctrl->multi_steps.
+__global__ void __launch_bounds__(kTPB, 4)
+k_drift_multi(SoA A, SoA B, Ctrl* __restrict__ ctrl, Sink sink, uint32_t* __restrict__ tile_count, DevParams P,
+              uint32_t n_steps) {
+  const uint32_t n = ctrl->n_active;
+  const uint32_t i = blockIdx.x * kTPB + threadIdx.x;
+  if (blockIdx.x * kTPB >= n) return;
+  const uint64_t step0 = ctrl->step;
+  uint32_t coll = 0, over = 0, keep = 0, taken = 0;
+  if (i < n) {
+    float x = A.x[i], y = A.y[i], z = A.z[i];
+    const uint32_t id = A.id[i];
+    bool bad = false;
+    for (uint32_t k = 0; k < n_steps; ++k) {
+      float xf, yf, zf;
+      if (!advance_carrier(x, y, z, id, step0 + k, 0.0, 0.0, 0.0, P, xf, yf, zf)) bad = true;
+      x = xf; y = yf; z = zf;
+      taken = k + 1;
+      if ((double)z <= P.z_well) { coll = 1; uint32_t o = 0; collect(x, y, z, id, step0 + k, P, sink, o); over = o; break; }
+      if (bad) break;                                        // non-finite: stop here, the flag below reports it
+    }
+    if (bad) atomicOr(&ctrl->nonfinite, 1u);
+    B.x[i] = x; B.y[i] = y; B.z[i] = z; B.id[i] = id;
+    keep = coll ? 0u : 1u;
+  }
+  const uint32_t wmax = __reduce_max_sync(0xffffffffu, taken);
+  if ((threadIdx.x & 31u) == 0 && wmax) atomicMax(&ctrl->multi_steps, wmax);
+  tally(coll, over, keep, ctrl, tile_count);
+}
+
 // Load path: unpack interleaved xyz into state B at [0,n), assign ids n_loaded + k, collect z <= z_well.
 __global__ void __launch_bounds__(kTPB)
 k_unpack(const float* __restrict__ xyz, uint32_t n, SoA B, Ctrl* __restrict__ ctrl, uint32_t id_base,

@@ -211,6 +211,19 @@ int enqueue_steps(gcoreccd_t* h, uint64_t n_steps) {
   int rc = ensure_variant(h);
   if (rc) return rc;
   const uint32_t tiles = bucket_tiles(tiles_for(h->n_bound));
+  if (h->dp.flags & GCORECCD_COULOMB_OFF) {
+    // independent carriers: one launch pair for the whole batch of steps (gc_integrate.cuh: k_drift_multi)
+    while (n_steps > 0) {
+      const uint32_t chunk = (uint32_t)std::min<uint64_t>(n_steps, 1u << 30);
+      k_drift_multi<<<tiles, kTPB, 0, h->stream>>>(h->A, h->B, h->ctrl, h->sink, h->tile_count, h->dp, chunk);
+      k_compact<<<tiles, kTPB, 0, h->stream>>>(h->B, h->A, h->ctrl, h->tile_count, 0u, 0u, 2, h->dp.z_well, 0u,
+                                               plan_args(h, h->variant));
+      h->launches += 2;
+      n_steps -= chunk;
+    }
+    GC_CUDA(h, cudaGetLastError());
+    return 0;
+  }
   const uint32_t per_step = (h->dp.flags & GCORECCD_COULOMB_OFF) ? 2u : 3u;
   // stream capture is not permitted on the legacy / per-thread default streams: plain launches there
   const bool can_graph = h->stream != cudaStreamLegacy && h->stream != cudaStreamPerThread && h->stream != nullptr;
@@ -461,7 +474,7 @@ int gcoreccd_run_to_collection(gcoreccd_t* h, uint64_t max_steps, uint64_t* step
   int ret = GCORECCD_OK;
   while (h->h_ctrl->n_active > 0) {
     if (done >= max_steps) { ret = GCORECCD_MAX_STEPS; break; }
-    uint64_t batch = 4 * kGraphSteps;
+    uint64_t batch = (h->dp.flags & GCORECCD_COULOMB_OFF) ? (1ull << 20) : 4 * kGraphSteps;
     if (batch > max_steps - done) batch = max_steps - done;
     rc = enqueue_steps(h, batch);
     if (rc) return rc;

@@ -369,3 +369,39 @@ def test_collected_positions_and_steps_match_the_oracle():
     sim.reset()
     assert len(sim.read_collected()[0]) == 0
     sim.close()
+
+
+# ------------------------------------------------------------------ Coulomb off: one launch for many steps
+def test_coulomb_off_multi_step_launch_is_bit_identical_to_single_steps():
+    from paper_2203_11043_b200 import binding as b
+    w = workloads.make(0, n=3000)
+    xyz = w["xyz"].copy()
+    xyz[:, 2] = np.linspace(0.5, 60.0, len(xyz), dtype=np.float32)             # collections spread over the window
+    multi, single = gpu_sim(w, flags=b.COULOMB_OFF), gpu_sim(w, flags=b.COULOMB_OFF)
+    multi.load_carriers(xyz)
+    single.load_carriers(xyz)
+    for chunk in (1, 7, 30):
+        multi.step(chunk)                                                      # k_drift_multi: one launch pair
+        for _ in range(chunk):
+            single.profile_step()                                              # k_integrate + k_compact per step
+        (xa, ia), (xb, ib) = multi.read_carriers(), single.read_carriers()
+        assert np.array_equal(ia, ib) and np.array_equal(xa, xb)
+        sa, sb = multi.state(), single.state()
+        assert sa == sb and sa["pair_interactions"] == 0
+    assert np.array_equal(multi.read_image()[0], single.read_image()[0])
+    fa, fb = multi.read_collected(), single.read_collected()
+    assert np.array_equal(fa[1], fb[1]) and np.array_equal(fa[0], fb[0], equal_nan=True)
+    # to full collection: the step index stops at the last hole's crossing, as with single steps
+    done, left, rc = multi.run_to_collection()
+    while single.state()["n_active"]:
+        single.profile_step()
+    assert left == 0 and multi.state() == single.state()
+    assert np.array_equal(multi.read_image()[0], single.read_image()[0])
+    # and the oracle agrees on that trajectory (Coulomb off, FP32 state): same step count, same image
+    o = oracle_sim(w, flags=g.COULOMB_OFF | g.FP32_STATE)
+    o.load(xyz)
+    o.run()
+    assert o.state()["step"] == multi.state()["step"]
+    assert np.abs(o.image().astype(np.int64) - multi.read_image()[0].astype(np.int64)).sum() <= 4
+    multi.close()
+    single.close()
