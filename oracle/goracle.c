@@ -93,6 +93,39 @@ void goracle_normals(uint64_t seed, uint32_t id, uint64_t step, double n[3], uin
   if (words) { words[0] = w[0]; words[1] = w[1]; words[2] = w[2]; words[3] = w[3]; }
 }
 
+/* ------------------------------------------------------------------ X-ray initial cloud (front end) */
+/* "N = E_e / w_e", w_e = 3.77 eV at 140 K; a fraction of a pair is not a carrier: floor. */
+uint64_t goracle_xray_hole_count(double E_e_eV, double w_eV) {
+  if (!(E_e_eV > 0.0) || !(w_eV > 0.0)) return 0;
+  return (uint64_t)floor(E_e_eV / w_eV);
+}
+
+/* "the initial cloud ... 3D Gaussian distribution with standard deviation depending solely on
+ * E_e" (the sigma(E_e) model is in the paper's refs [11-13], not in its text: sigma is an input here).
+ * Hole k = first_index + i gets centre + sigma * n_k, n_k the Box-Muller triple of
+ * Philox4x32-10(ctr = (k_lo, 'XRAY', k_hi, 0), key = gen_seed) with the uniform mapping of goracle_normals;
+ * z above the back surface is mirrored (R12); the result is rounded to FP32. */
+void goracle_xray_cloud(uint64_t gen_seed, uint64_t first_index, uint64_t n, const double centre_um[3],
+                        double sigma_um, double thickness_um, float* xyz) {
+  uint32_t key[2] = { (uint32_t)(gen_seed & 0xffffffffu), (uint32_t)(gen_seed >> 32) };
+  for (uint64_t i = 0; i < n; ++i) {
+    const uint64_t k = first_index + i;
+    uint32_t ctr[4] = { (uint32_t)(k & 0xffffffffu), 0x58524159u, (uint32_t)(k >> 32), 0u };
+    uint32_t w[4];
+    goracle_philox4x32_10(ctr, key, w);
+    double ua = ((double)(w[0] >> 9) + 0.5) * (1.0 / 8388608.0);
+    double fa = (double)(w[1] >> 8) * (1.0 / 16777216.0);
+    double ub = ((double)(w[2] >> 9) + 0.5) * (1.0 / 8388608.0);
+    double fb = (double)(w[3] >> 8) * (1.0 / 16777216.0);
+    double Ra = sqrt(-2.0 * log(ua)), Rb = sqrt(-2.0 * log(ub));
+    double x = centre_um[0] + sigma_um * (Ra * cos(2.0 * GO_PI * fa));
+    double y = centre_um[1] + sigma_um * (Ra * sin(2.0 * GO_PI * fa));
+    double z = centre_um[2] + sigma_um * (Rb * cos(2.0 * GO_PI * fb));
+    if (z > thickness_um) z = 2.0 * thickness_um - z;
+    xyz[3 * i] = (float)x; xyz[3 * i + 1] = (float)y; xyz[3 * i + 2] = (float)z;
+  }
+}
+
 /* ------------------------------------------------------------------ eq. 6 */
 /* PAPER.md:78  E_j = K sum_{i=1..N} r_ij / (|r_ij|^2 + eps^2)^{3/2},  r_ij = r_j - r_i.
  * The i = j term is included and is exactly zero (r_jj = 0). */

@@ -64,6 +64,10 @@ double goracle_coulomb_constant(double eps_si);                             /* K
 /* ---- counter-based RNG ---- */
 void goracle_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
 void goracle_normals(uint64_t seed, uint32_t id, uint64_t step, double n[3], uint32_t words[4]);
+/* X-ray front end: hole count N = floor(E_e / w) and the seeded 3-D Gaussian initial cloud */
+uint64_t goracle_xray_hole_count(double E_e_eV, double w_eV);
+void goracle_xray_cloud(uint64_t gen_seed, uint64_t first_index, uint64_t n, const double centre_um[3],
+                        double sigma_um, double thickness_um, float* xyz);
 
 /* ---- eq. 6: literal double loop.  Targets j = tgt[0..m) (or all if tgt==NULL, m==n);
  *      sources i = 0..n-1.  Output E in V/cm. ---- */

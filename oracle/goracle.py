@@ -62,6 +62,10 @@ def lib():
     L.goracle_philox4x32_10.argtypes = [u32p, u32p, u32p]
     L.goracle_normals.restype = None
     L.goracle_normals.argtypes = [C.c_uint64, C.c_uint32, C.c_uint64, dp, u32p]
+    L.goracle_xray_hole_count.restype = C.c_uint64
+    L.goracle_xray_hole_count.argtypes = [C.c_double, C.c_double]
+    L.goracle_xray_cloud.restype = None
+    L.goracle_xray_cloud.argtypes = [C.c_uint64, C.c_uint64, C.c_uint64, dp, C.c_double, C.c_double, C.POINTER(C.c_float)]
     L.goracle_coulomb_field.restype = None
     L.goracle_coulomb_field.argtypes = [dp, dp, dp, C.c_uint64, u64p, C.c_uint64, C.c_double, C.c_double, dp, dp, dp]
     L.goracle_advance.restype = C.c_int
@@ -121,6 +125,20 @@ def diffusion_sigma(mu, T, dt_ns):
 
 def coulomb_constant(eps_si=11.7):
     return lib().goracle_coulomb_constant(float(eps_si))
+
+
+def xray_hole_count(E_e_eV, w_eV=3.77):
+    """N = E_e / w_e (3.77 eV at 140 K), floored."""
+    return int(lib().goracle_xray_hole_count(float(E_e_eV), float(w_eV)))
+
+
+def xray_cloud(gen_seed, n, centre_um, sigma_um, thickness_um=675.0, first_index=0):
+    """seeded 3-D Gaussian initial cloud, float32 (n,3)."""
+    out = np.empty((int(n), 3), dtype=np.float32)
+    c = np.ascontiguousarray(centre_um, dtype=np.float64)
+    lib().goracle_xray_cloud(int(gen_seed), int(first_index), int(n), _dp(c), float(sigma_um), float(thickness_um),
+                             out.ctypes.data_as(C.POINTER(C.c_float)))
+    return out
 
 
 def philox4x32_10(ctr, key):
