@@ -164,6 +164,36 @@ int gcoreccd_get_events(gcoreccd_t* h, uint64_t* n_active_host, uint64_t* step_h
 int gcoreccd_read_event_carriers(gcoreccd_t* h, uint64_t event, float* xyz_um_host, uint32_t* id_host, uint64_t cap,
                                  uint64_t* n);
 
+/* ---- Workload front end ---------------------------------------------------------------
+ * X-rays: a photo-electron of energy E_e makes N = E_e / w_e holes (w_e = 3.77 eV at 140 K),
+ * initially a 3-D Gaussian cloud around the interaction point whose standard deviation depends on E_e (that model
+ * is in the paper's references, not its text: sigma is an input here).
+ *
+ * xray_hole_count: floor(E_e_eV / w_eV); 0 if either is not positive.  Pure host arithmetic.
+ * generate_cloud: draws n holes ~ N(centre, sigma^2 I) ON THE GPU and appends them exactly as load_carriers would
+ *   (ids continue, z <= z_well collected at once).  Hole i uses generator index first_index + i: Box-Muller of
+ *   Philox4x32-10(counter (index_lo, 'XRAY', index_hi, 0), key gen_seed), FP64, z above the back surface mirrored,
+ *   rounded to FP32 — so chunked calls with consecutive indices equal one call.  centre_um: 3 host doubles.
+ *   sigma_um >= 0.  Errors as load_carriers (INVALID also if the centre is outside (-inf, thickness]).
+ * generate_xray_events: one batch of n_events independent clouds for run_events (replaces load_events):
+ *   event e gets floor(E_e_eV[e] / w_eV) holes around centre_um[3e..3e+2] with sigma_um[e]; all arrays are HOST
+ *   arrays; generator index = first_index + position of the hole in the batch.  counts_out (host, n_events entries,
+ *   may be NULL) receives the hole count per event.  Errors as load_events.
+ * load_carriers_file: text file, one hole per line "x y z" in um separated by blanks, tabs, commas or semicolons;
+ *   empty lines and lines starting with '#' are skipped ("load the charge positions ... from an
+ *   external file"; the paper does not give its format).  Appends like load_carriers; *n_read (host, may be NULL)
+ *   receives the holes read.  INVALID on an unreadable file or a malformed line (nothing is loaded).
+ * save_collected_file: writes "id x y z step" per collected hole, ascending id, with a '#' header line
+ *   ("whether final results should be saved to a file"); *n_written may be NULL. */
+uint64_t gcoreccd_xray_hole_count(double E_e_eV, double w_eV);
+int gcoreccd_generate_cloud(gcoreccd_t* h, uint64_t n, const double* centre_um_host, double sigma_um, uint64_t gen_seed,
+                            uint64_t first_index);
+int gcoreccd_generate_xray_events(gcoreccd_t* h, uint64_t n_events, const double* E_e_eV_host, const double* centre_um_host,
+                                  const double* sigma_um_host, double w_eV, uint64_t gen_seed, uint64_t first_index,
+                                  uint64_t* counts_out_host);
+int gcoreccd_load_carriers_file(gcoreccd_t* h, const char* path, uint64_t* n_read);
+int gcoreccd_save_collected_file(gcoreccd_t* h, const char* path, uint64_t* n_written);
+
 /* Run ONE step with CUDA events between its kernels (on the handle's stream) and return the device time of
  * each in milliseconds: ms[0] field, ms[1] integrate+collect, ms[2] compact, ms[3] whole step.  Synchronous. */
 int gcoreccd_profile_step(gcoreccd_t* h, float ms_host[4]);

@@ -20,6 +20,8 @@ EXPORTS = ["gcoreccd_workspace_size", "gcoreccd_create", "gcoreccd_destroy", "gc
            "gcoreccd_load_carriers", "gcoreccd_load_snapshot", "gcoreccd_step", "gcoreccd_run_to_collection",
            "gcoreccd_read_image", "gcoreccd_get_state", "gcoreccd_read_carriers", "gcoreccd_read_collected", "gcoreccd_eval_field",
            "gcoreccd_load_events", "gcoreccd_run_events", "gcoreccd_get_events", "gcoreccd_read_event_carriers",
+           "gcoreccd_xray_hole_count", "gcoreccd_generate_cloud", "gcoreccd_generate_xray_events",
+           "gcoreccd_load_carriers_file", "gcoreccd_save_collected_file",
            "gcoreccd_profile_step", "gcoreccd_kernel_launches", "gcoreccd_debug_normals", "gcoreccd_strerror",
            "gcoreccd_last_error", "gcoreccd_version"]
 
@@ -92,6 +94,17 @@ def lib():
     L.gcoreccd_get_events.argtypes = [vp, u64p, u64p, C.c_uint64, u64p]
     L.gcoreccd_read_event_carriers.restype = C.c_int
     L.gcoreccd_read_event_carriers.argtypes = [vp, C.c_uint64, vp, vp, C.c_uint64, u64p]
+    dbl = C.POINTER(C.c_double)
+    L.gcoreccd_xray_hole_count.restype = C.c_uint64
+    L.gcoreccd_xray_hole_count.argtypes = [C.c_double, C.c_double]
+    L.gcoreccd_generate_cloud.restype = C.c_int
+    L.gcoreccd_generate_cloud.argtypes = [vp, C.c_uint64, dbl, C.c_double, C.c_uint64, C.c_uint64]
+    L.gcoreccd_generate_xray_events.restype = C.c_int
+    L.gcoreccd_generate_xray_events.argtypes = [vp, C.c_uint64, dbl, dbl, dbl, C.c_double, C.c_uint64, C.c_uint64, u64p]
+    L.gcoreccd_load_carriers_file.restype = C.c_int
+    L.gcoreccd_load_carriers_file.argtypes = [vp, C.c_char_p, u64p]
+    L.gcoreccd_save_collected_file.restype = C.c_int
+    L.gcoreccd_save_collected_file.argtypes = [vp, C.c_char_p, u64p]
     L.gcoreccd_profile_step.restype = C.c_int
     L.gcoreccd_profile_step.argtypes = [vp, fp]
     L.gcoreccd_kernel_launches.restype = C.c_uint64
@@ -114,6 +127,10 @@ def strerror(code):
 
 def version():
     return lib().gcoreccd_version().decode()
+
+
+def xray_hole_count(E_e_eV, w_eV=3.77):
+    return int(lib().gcoreccd_xray_hole_count(float(E_e_eV), float(w_eV)))
 
 
 def workspace_size(max_carriers, img_nx, img_ny):
@@ -227,6 +244,36 @@ class Gcoreccd:
             rc = lib().gcoreccd_read_image(self._h, C.c_void_p(out.ctypes.data), out.size, C.byref(over), 0)
         self._check(rc, "gcoreccd_read_image")
         return out, int(over.value)
+
+    # ---- workload front end
+    def generate_cloud(self, n, centre_um, sigma_um, gen_seed, first_index=0):
+        c = (C.c_double * 3)(*[float(v) for v in centre_um])
+        return self._check(lib().gcoreccd_generate_cloud(self._h, int(n), c, float(sigma_um), int(gen_seed), int(first_index)),
+                           "gcoreccd_generate_cloud")
+
+    def generate_xray_events(self, E_e_eV, centres_um, sigmas_um, gen_seed, w_eV=3.77, first_index=0):
+        """Returns the hole count per event."""
+        E = np.ascontiguousarray(E_e_eV, dtype=np.float64).reshape(-1)
+        c = np.ascontiguousarray(centres_um, dtype=np.float64).reshape(-1, 3)
+        sg = np.ascontiguousarray(sigmas_um, dtype=np.float64).reshape(-1)
+        assert len(c) == len(E) == len(sg)
+        counts = np.zeros(len(E), dtype=np.uint64)
+        dbl = C.POINTER(C.c_double)
+        rc = lib().gcoreccd_generate_xray_events(self._h, len(E), E.ctypes.data_as(dbl), c.ctypes.data_as(dbl), sg.ctypes.data_as(dbl),
+                                                 float(w_eV), int(gen_seed), int(first_index),
+                                                 counts.ctypes.data_as(C.POINTER(C.c_uint64)))
+        self._check(rc, "gcoreccd_generate_xray_events")
+        return counts
+
+    def load_carriers_file(self, path):
+        n = C.c_uint64()
+        self._check(lib().gcoreccd_load_carriers_file(self._h, os.fsencode(path), C.byref(n)), "gcoreccd_load_carriers_file")
+        return int(n.value)
+
+    def save_collected_file(self, path):
+        n = C.c_uint64()
+        self._check(lib().gcoreccd_save_collected_file(self._h, os.fsencode(path), C.byref(n)), "gcoreccd_save_collected_file")
+        return int(n.value)
 
     # ---- batched independent events (one thread block per event)
     def load_events(self, xyz, offsets):

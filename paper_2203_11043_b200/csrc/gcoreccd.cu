@@ -9,11 +9,13 @@
 #include <new>
 #include <algorithm>
 #include <cstdlib>
+#include <vector>
 
 #include "gc_common.cuh"
 #include "gc_compact.cuh"
 #include "gc_events.cuh"
 #include "gc_field.cuh"
+#include "gc_frontend.cuh"
 #include "gc_integrate.cuh"
 
 using namespace gc;
@@ -847,6 +849,126 @@ int gcoreccd_read_event_carriers(gcoreccd_t* h, uint64_t event, float* xyz, uint
   GC_CUDA(h, cudaGetLastError());
   GC_CUDA(h, cudaStreamSynchronize(h->stream));
   return GCORECCD_OK;
+}
+
+// ---------------------------------------------------------------------------- workload front end
+uint64_t gcoreccd_xray_hole_count(double E_e_eV, double w_eV) {
+  if (!(E_e_eV > 0.0) || !(w_eV > 0.0)) return 0;
+  const double q = std::floor(E_e_eV / w_eV);
+  return q >= 1.8e19 ? 0 : (uint64_t)q;
+}
+
+int gcoreccd_generate_cloud(gcoreccd_t* h, uint64_t n, const double* c, double sigma, uint64_t gen_seed, uint64_t first_index) {
+  if (!h || !c) return GCORECCD_ERR_INVALID;
+  if (n == 0) return GCORECCD_OK;
+  if (!(sigma >= 0.0) || !std::isfinite(sigma) || !std::isfinite(c[0]) || !std::isfinite(c[1]) || !std::isfinite(c[2]) ||
+      c[2] > h->p.thickness_um)
+    return fail(h, GCORECCD_ERR_INVALID, "generate_cloud: sigma must be >= 0 and the centre finite and inside the slab");
+  if (n > h->p.max_carriers) return fail(h, GCORECCD_ERR_CAPACITY, "generate_cloud: capacity");
+  if (events_busy(h)) return fail(h, GCORECCD_ERR_STATE, "generate_cloud: a batch of events is still drifting");
+  DeviceGuard guard(h->device);
+  k_gen_cloud<<<tiles_for(n), kTPB, 0, h->stream>>>(h->Ep, (uint32_t)n, first_index, c[0], c[1], c[2], sigma, h->dp.thickness,
+                                                   (uint32_t)(gen_seed & 0xffffffffu), (uint32_t)(gen_seed >> 32));
+  h->launches += 1;
+  GC_CUDA(h, cudaGetLastError());
+  return gcoreccd_load_carriers(h, h->Ep, n, 1);          // the partial-sum buffer is scratch between steps
+}
+
+int gcoreccd_generate_xray_events(gcoreccd_t* h, uint64_t n_events, const double* E, const double* centre, const double* sigma,
+                                  double w_eV, uint64_t gen_seed, uint64_t first_index, uint64_t* counts_out) {
+  if (!h || !E || !centre || !sigma || n_events == 0 || n_events > 0x7fffffffull || !(w_eV > 0.0)) return GCORECCD_ERR_INVALID;
+  std::vector<uint64_t> off(n_events + 1);
+  std::vector<uint32_t> off32(n_events + 1);
+  off[0] = 0; off32[0] = 0;
+  for (uint64_t e = 0; e < n_events; ++e) {
+    if (!(sigma[e] >= 0.0) || !std::isfinite(sigma[e]) || !std::isfinite(centre[3 * e]) || !std::isfinite(centre[3 * e + 1]) ||
+        !std::isfinite(centre[3 * e + 2]) || centre[3 * e + 2] > h->p.thickness_um || !std::isfinite(E[e]))
+      return fail(h, GCORECCD_ERR_INVALID, "generate_xray_events: non-finite input, negative sigma or centre above the back surface");
+    const uint64_t cnt = gcoreccd_xray_hole_count(E[e], w_eV);
+    if (cnt > GCORECCD_EVENT_MAX_CARRIERS) return fail(h, GCORECCD_ERR_CAPACITY, "generate_xray_events: an event exceeds GCORECCD_EVENT_MAX_CARRIERS");
+    off[e + 1] = off[e] + cnt;
+    if (off[e + 1] > h->p.max_carriers) return fail(h, GCORECCD_ERR_CAPACITY, "generate_xray_events: capacity");
+    off32[e + 1] = (uint32_t)off[e + 1];
+    if (counts_out) counts_out[e] = cnt;
+  }
+  if (events_busy(h)) return fail(h, GCORECCD_ERR_STATE, "generate_xray_events: the previous batch is still drifting");
+  const uint64_t n = off[n_events];
+  DeviceGuard guard(h->device);
+  if (n) {
+    char* buf = nullptr;
+    const size_t b_off = align_up((n_events + 1) * 4, 256), b_c = align_up(n_events * 24, 256), b_s = align_up(n_events * 8, 256);
+    cudaError_t e = cudaMalloc((void**)&buf, b_off + b_c + b_s);
+    if (e != cudaSuccess) return fail(h, e == cudaErrorMemoryAllocation ? GCORECCD_ERR_NOMEM : GCORECCD_ERR_CUDA, "generate_xray_events: cudaMalloc", e);
+    uint32_t* d_off = (uint32_t*)buf;
+    double* d_c = (double*)(buf + b_off);
+    double* d_s = (double*)(buf + b_off + b_c);
+    e = cudaMemcpyAsync(d_off, off32.data(), (n_events + 1) * 4, cudaMemcpyHostToDevice, h->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_c, centre, n_events * 24, cudaMemcpyHostToDevice, h->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_s, sigma, n_events * 8, cudaMemcpyHostToDevice, h->stream);
+    if (e == cudaSuccess) {
+      k_gen_events<<<tiles_for(n), kTPB, 0, h->stream>>>(h->Ep, (uint32_t)n, d_off, (uint32_t)n_events, d_c, d_s, first_index,
+                                                        h->dp.thickness, (uint32_t)(gen_seed & 0xffffffffu), (uint32_t)(gen_seed >> 32));
+      h->launches += 1;
+      e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+    cudaFree(buf);
+    if (e != cudaSuccess) return fail(h, GCORECCD_ERR_CUDA, "generate_xray_events", e);
+  }
+  return gcoreccd_load_events(h, h->Ep, off.data(), n_events, 1);
+}
+
+int gcoreccd_load_carriers_file(gcoreccd_t* h, const char* path, uint64_t* n_read) {
+  if (!h || !path) return GCORECCD_ERR_INVALID;
+  FILE* f = fopen(path, "r");
+  if (!f) return fail(h, GCORECCD_ERR_INVALID, "load_carriers_file: cannot open the file");
+  std::vector<float> xyz;
+  char line[512];
+  bool bad = false;
+  while (fgets(line, sizeof(line), f)) {
+    char* s = line;
+    while (*s == ' ' || *s == '\t') ++s;
+    if (*s == '#' || *s == '\n' || *s == '\r' || *s == 0) continue;
+    float v[3];
+    int got = 0;
+    while (got < 3) {
+      char* end = nullptr;
+      v[got] = strtof(s, &end);
+      if (end == s) break;
+      ++got;
+      s = end;
+      while (*s == ' ' || *s == '\t' || *s == ',' || *s == ';') ++s;
+    }
+    if (got != 3 || !(*s == 0 || *s == '\n' || *s == '\r' || *s == '#')) { bad = true; break; }
+    xyz.push_back(v[0]); xyz.push_back(v[1]); xyz.push_back(v[2]);
+  }
+  fclose(f);
+  if (bad) return fail(h, GCORECCD_ERR_INVALID, "load_carriers_file: malformed line (expected x y z)");
+  if (n_read) *n_read = xyz.size() / 3;
+  if (xyz.empty()) return GCORECCD_OK;
+  return gcoreccd_load_carriers(h, xyz.data(), xyz.size() / 3, 0);
+}
+
+int gcoreccd_save_collected_file(gcoreccd_t* h, const char* path, uint64_t* n_written) {
+  if (!h || !path) return GCORECCD_ERR_INVALID;
+  uint64_t m = 0;
+  int rc = gcoreccd_read_collected(h, nullptr, nullptr, 0, &m);
+  if (rc) return rc;
+  std::vector<float> xyz(3 * m + 3);
+  std::vector<uint32_t> st(m + 1);
+  if (m) { rc = gcoreccd_read_collected(h, xyz.data(), st.data(), m, &m); if (rc) return rc; }
+  FILE* f = fopen(path, "w");
+  if (!f) return fail(h, GCORECCD_ERR_INVALID, "save_collected_file: cannot open the file");
+  fprintf(f, "# id x_um y_um z_um step   (holes collected at z <= z_well; PAPER.md:122 output positions)\n");
+  uint64_t w = 0;
+  for (uint64_t k = 0; k < m; ++k) {
+    if (st[k] == 0xffffffffu) continue;                    // still drifting
+    fprintf(f, "%llu %.9g %.9g %.9g %u\n", (unsigned long long)k, xyz[3 * k], xyz[3 * k + 1], xyz[3 * k + 2], st[k]);
+    ++w;
+  }
+  const bool ok = fclose(f) == 0;
+  if (n_written) *n_written = w;
+  return ok ? GCORECCD_OK : fail(h, GCORECCD_ERR_INVALID, "save_collected_file: write failed");
 }
 
 const char* gcoreccd_strerror(int code) {

@@ -1,0 +1,156 @@
+"""GPU parity tests (-m gpu) of the workload front end: the X-ray
+cloud generator against the oracle's generator hole by hole, generated batches against the oracle's clouds,
+and the hole-list / final-position files."""
+import os
+
+import numpy as np
+import pytest
+
+from oracle import goracle as g
+from paper_2203_11043_b200 import binding, workloads
+from util import gpu_sim
+
+pytestmark = pytest.mark.gpu
+
+
+def _ulp_close(a, b):
+    """FP64 expression rounded to FP32 on both sides: device and host libm may differ in the last FP64 bit, which
+    moves the FP32 result by at most one ulp, and only when the FP64 value sits on a rounding boundary."""
+    a = np.asarray(a, dtype=np.float32); b = np.asarray(b, dtype=np.float32)
+    ulp = np.spacing(np.maximum(np.abs(a), np.abs(b)))
+    assert np.all(np.abs(a.astype(np.float64) - b) <= ulp), float(np.abs(a.astype(np.float64) - b).max())
+    assert (a == b).mean() > 0.999
+
+
+def test_hole_count_matches_oracle():
+    for E, w in ((100.0, 3.77), (7500.0, 3.64), (3.77, 3.77), (3.76, 3.77), (5900.0, 3.77), (0.0, 3.77), (10.0, 0.0), (-5.0, 3.77)):
+        assert binding.xray_hole_count(E, w) == g.xray_hole_count(E, w)
+
+
+@pytest.mark.parametrize("n,centre,sigma,first", [(1, (0.0, 0.0, 200.0), 1.0, 0), (1000, (30.0, -45.0, 647.0), 0.5, 0),
+                                                  (4099, (-100.0, 7.0, 674.5), 2.0, (1 << 32) - 7), (257, (0.0, 0.0, 10.0), 0.0, 5)])
+def test_generate_cloud_matches_oracle(n, centre, sigma, first):
+    w = workloads.make(0, n=8)
+    with gpu_sim(w, max_carriers=8192) as sim:
+        sim.generate_cloud(n, centre, sigma, gen_seed=0xC0FFEE1234, first_index=first)
+        xyz, ids = sim.read_carriers()
+        ref = g.xray_cloud(0xC0FFEE1234, n, centre, sigma, thickness_um=w["params"]["thickness_um"], first_index=first)
+        keep = ref[:, 2].astype(np.float64) > w["params"]["z_well_um"]
+        # holes generated at z <= z_well are collected at load (R18); near that plane a 1-ulp difference may flip one
+        assert abs(len(xyz) - int(keep.sum())) <= 1
+        if len(xyz) == keep.sum():
+            assert np.array_equal(ids, np.nonzero(keep)[0].astype(np.uint32))
+            _ulp_close(xyz, ref[keep])
+        st = sim.state()
+        assert st["n_loaded"] == n and st["n_active"] + st["n_collected"] == n
+
+
+def test_generate_cloud_appends_and_chunks():
+    w = workloads.make(0, n=8)
+    c = (5.0, 5.0, 300.0)
+    with gpu_sim(w, max_carriers=4096) as a, gpu_sim(w, max_carriers=4096) as b:
+        a.generate_cloud(3000, c, 1.0, gen_seed=11)
+        b.generate_cloud(1234, c, 1.0, gen_seed=11)
+        b.generate_cloud(1766, c, 1.0, gen_seed=11, first_index=1234)
+        xa, ia = a.read_carriers(); xb, ib = b.read_carriers()
+        assert np.array_equal(xa, xb) and np.array_equal(ia, ib) and np.array_equal(ia, np.arange(3000, dtype=np.uint32))
+
+
+def test_generate_cloud_errors():
+    w = workloads.make(0, n=8)
+    with gpu_sim(w, max_carriers=100) as sim:
+        for bad in (lambda: sim.generate_cloud(10, (0, 0, 700.0), 1.0, 1), lambda: sim.generate_cloud(10, (0, 0, 100.0), -1.0, 1),
+                    lambda: sim.generate_cloud(10, (float("nan"), 0, 100.0), 1.0, 1)):
+            with pytest.raises(binding.GcoreccdError) as e:
+                bad()
+            assert e.value.code == binding.ERR_INVALID
+        with pytest.raises(binding.GcoreccdError) as e:
+            sim.generate_cloud(101, (0, 0, 100.0), 1.0, 1)
+        assert e.value.code == binding.ERR_CAPACITY
+        assert sim.state()["n_loaded"] == 0
+
+
+def test_generate_xray_events_matches_oracle_and_runs():
+    w = workloads.make_events([1])
+    P = w["params"]
+    rng = np.random.default_rng(5)
+    E = np.array([100.0, 5900.0, 3.0, 1000.0, 7500.0, 277.0, 100.0])
+    centres = np.stack([rng.uniform(-300, 300, len(E)), rng.uniform(-300, 300, len(E)), rng.uniform(20, 660, len(E))], axis=1)
+    sigmas = np.array([0.05, 0.6, 0.1, 0.2, 0.7, 0.1, 0.0])
+    with gpu_sim(w, max_carriers=8192) as sim:
+        counts = sim.generate_xray_events(E, centres, sigmas, gen_seed=77, first_index=3)
+        assert list(counts) == [g.xray_hole_count(e) for e in E]
+        assert counts[2] == 0
+        off = np.concatenate([[0], np.cumsum(counts)]).astype(int)
+        for e in range(len(E)):
+            xyz, ids = sim.read_event_carriers(e)
+            ref = g.xray_cloud(77, counts[e], centres[e], sigmas[e], thickness_um=P["thickness_um"], first_index=3 + off[e])
+            assert len(xyz) == counts[e]
+            if counts[e]:
+                _ulp_close(xyz, ref)
+                assert np.array_equal(ids, np.arange(off[e], off[e + 1], dtype=np.uint32))
+        ev_left, ca_left, rc = sim.run_events()
+        img, over = sim.read_image()
+        assert ca_left == 0 and int(img.sum()) + over == int(counts.sum())
+        # a 100 eV photon deep in the bulk spreads over several 15 um pixels (Fig. 5): all of event 0
+        # lands within a few pixels of its interaction point
+        fx, st = sim.read_collected()
+        d = fx[:counts[0], :2] - centres[0, :2]
+        assert np.all(np.abs(d) < 120.0)
+
+
+def test_generate_xray_events_errors():
+    w = workloads.make_events([1])
+    with gpu_sim(w, max_carriers=5000) as sim:
+        with pytest.raises(binding.GcoreccdError) as e:
+            sim.generate_xray_events([3.77 * 4097.5], [(0, 0, 100.0)], [0.1], 1)
+        assert e.value.code == binding.ERR_CAPACITY               # one event above GCORECCD_EVENT_MAX_CARRIERS
+        with pytest.raises(binding.GcoreccdError) as e:
+            sim.generate_xray_events([3.77 * 3000.5] * 2, [(0, 0, 100.0)] * 2, [0.1] * 2, 1)
+        assert e.value.code == binding.ERR_CAPACITY               # total above max_carriers
+        with pytest.raises(binding.GcoreccdError) as e:
+            sim.generate_xray_events([100.0], [(0, 0, 700.0)], [0.1], 1)
+        assert e.value.code == binding.ERR_INVALID
+
+
+def test_hole_list_file_roundtrip(tmp_path):
+    w = workloads.make(0, n=777)
+    path = os.path.join(tmp_path, "holes.txt")
+    with open(path, "w") as f:
+        f.write("# x y z (um)\n\n")
+        for k, (x, y, z) in enumerate(w["xyz"]):
+            sep = (" ", ", ", "\t", ";")[k % 4]
+            f.write("%s%.9g%s%.9g%s%.9g%s\n" % ("  " if k % 5 == 0 else "", x, sep, y, sep, z, "  # hole" if k % 7 == 0 else ""))
+    with gpu_sim(w) as a, gpu_sim(w) as b:
+        assert a.load_carriers_file(path) == 777
+        b.load_carriers(w["xyz"])
+        xa, ia = a.read_carriers(); xb, ib = b.read_carriers()
+        assert np.array_equal(xa, xb) and np.array_equal(ia, ib)        # %.9g round-trips FP32 exactly
+        a.run_to_collection(); b.run_to_collection()
+        out = os.path.join(tmp_path, "final.txt")
+        assert a.save_collected_file(out) == 777
+        rows = np.loadtxt(out)
+        fx, st = b.read_collected()
+        assert np.array_equal(rows[:, 0].astype(np.int64), np.arange(777))
+        assert np.array_equal(rows[:, 1:4].astype(np.float32), fx) and np.array_equal(rows[:, 4].astype(np.uint32), st)
+        assert open(out).readline().startswith("#")
+
+
+def test_hole_list_file_errors(tmp_path):
+    w = workloads.make(0, n=8)
+    with gpu_sim(w) as sim:
+        with pytest.raises(binding.GcoreccdError) as e:
+            sim.load_carriers_file(os.path.join(tmp_path, "missing.txt"))
+        assert e.value.code == binding.ERR_INVALID
+        bad = os.path.join(tmp_path, "bad.txt")
+        open(bad, "w").write("1 2 3\n4 5\n")
+        with pytest.raises(binding.GcoreccdError) as e:
+            sim.load_carriers_file(bad)
+        assert e.value.code == binding.ERR_INVALID and sim.state()["n_loaded"] == 0
+        bad2 = os.path.join(tmp_path, "bad2.txt")
+        open(bad2, "w").write("1 2 3 4\n")
+        with pytest.raises(binding.GcoreccdError):
+            sim.load_carriers_file(bad2)
+        empty = os.path.join(tmp_path, "empty.txt")
+        open(empty, "w").write("# nothing\n")
+        assert sim.load_carriers_file(empty) == 0
