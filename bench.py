@@ -355,6 +355,80 @@ def run_sweep(args):
     return 0
 
 
+def run_sharded(args):
+    """--sharded CFG: ONE event's targets sharded over the ranks (not the headline, whose
+    north_star fixes replicas).  Under torchrun: ShardedEvent over NCCL, strong scaling, device time max over ranks.
+    On one GPU: --virtual-ranks G handles stepped sequentially; reports every rank's measured device time per step
+    (shard_local + shard_commit, CUDA events) — the exchange over NVLink is NOT in that number."""
+    import torch
+    import torch.distributed as dist
+    from paper_2203_11043_b200 import binding, replicas, sharded, workloads
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    w = workloads.make(int(args.sharded))
+    xyz, n = w["xyz"], len(w["xyz"])
+    stream = torch.cuda.Stream()
+    torch.cuda.set_stream(stream)
+    alloc = lambda nb: torch.empty(nb, dtype=torch.uint8, device="cuda")
+    peaks, _ = measured_peaks()
+    peak_pairs = SM_COUNT * LANES * 2.0 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / FLOP_PER_PAIR
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        ev = sharded.ShardedEvent(binding.from_workload(w, stream=stream), rank, world,
+                                  lambda mb: sharded.DistExchange(torch, "cuda", mb, world), alloc)
+        ev.load_carriers(xyz)
+        ev.step(args.warmup)
+        st0 = ev.refresh()
+        dist.barrier(); torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); ev.step(args.steps); e1.record()
+        dist.barrier(); torch.cuda.synchronize()
+        tot = ev.totals(sharded.dist_reduce_sum(torch, "cuda"))
+        ms, _ = replicas.aggregate(e0.elapsed_time(e1), 0.0, device="cuda")
+        line = None
+        if rank == 0:
+            line = {"mode": "sharded", "n_gpus": world, "workload": w["name"], "n_holes": n, "steps": args.steps,
+                    "ms_per_step": ms / args.steps, "n_active": tot["n_active"], "scaling": "strong",
+                    "exchange": "NCCL all_gather_into_tensor of %d-byte messages" % ev.nbytes}
+            print(json.dumps(line), flush=True)
+        dist.destroy_process_group()
+        return 0
+    G = args.virtual_ranks
+    es = [binding.from_workload(w, stream=stream) for _ in range(G)]
+    vr = sharded.VirtualRanks(es, alloc)
+    vr.load_carriers(xyz)
+    vr.step(args.warmup)
+    st = vr.refresh()
+    na = st["n_active"]
+    K = args.steps
+    evs = [[(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+            for _ in range(G)] for _ in range(K)]
+    for k in range(K):                                    # VirtualRanks.step unrolled so each rank's kernels are bracketed
+        msgs = vr.msgs[vr.k & 1]; vr.k += 1
+        for g_, (e, m) in enumerate(zip(es, msgs)):
+            evs[k][g_][0].record(); e.shard_local(m.data_ptr(), vr.nbytes); evs[k][g_][1].record()
+        ptrs = [m.data_ptr() for m in msgs]
+        for g_, e in enumerate(es):
+            e.shard_commit(ptrs, vr.nbytes); evs[k][g_][2].record()
+    torch.cuda.synchronize()
+    local_ms = np.array([[evs[k][g_][0].elapsed_time(evs[k][g_][1]) for g_ in range(G)] for k in range(K)])
+    commit_ms = np.array([[(evs[k][g_ - 1][2] if g_ else evs[k][G - 1][1]).elapsed_time(evs[k][g_][2]) for g_ in range(G)]
+                          for k in range(K)])
+    per_rank = (local_ms + commit_ms).mean(axis=0)
+    st1 = vr.refresh()
+    line = {"mode": "sharded-virtual", "virtual_ranks": G, "workload": w["name"], "n_holes": n, "n_active_start": na,
+            "n_active_end": st1["n_active"], "steps": K, "per_rank_ms_per_step": [float(v) for v in per_rank],
+            "max_rank_ms_per_step": float(per_rank.max()), "sum_ranks_ms_per_step": float(per_rank.sum()),
+            "commit_ms": float(commit_ms.mean()), "message_bytes": vr.nbytes,
+            "frac_of_fp32_peak_per_rank": float(na * float(na) / G / (per_rank.max() * 1e-3) / peak_pairs),
+            "note": "each rank's kernels measured alone on one B200; the per-step all-gather of G messages over NVLink "
+                    "is not included (one GPU available)"}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -364,7 +438,11 @@ def main():
     ap.add_argument("--no-event", action="store_true", help="skip the seconds-per-event run")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", default="", help="comma-separated hole counts: per-step time vs N (not the headline)")
+    ap.add_argument("--sharded", default="", help="config number: one event sharded over the ranks (not the headline)")
+    ap.add_argument("--virtual-ranks", type=int, default=8, help="with --sharded on ONE GPU: ranks emulated sequentially")
     args = ap.parse_args()
+    if args.sharded:
+        return run_sharded(args)
     if args.sweep:
         return run_sweep(args)
     if args.impl == "reference":

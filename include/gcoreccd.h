@@ -194,6 +194,38 @@ int gcoreccd_generate_xray_events(gcoreccd_t* h, uint64_t n_events, const double
 int gcoreccd_load_carriers_file(gcoreccd_t* h, const char* path, uint64_t* n_read);
 int gcoreccd_save_collected_file(gcoreccd_t* h, const char* path, uint64_t* n_written);
 
+/* ---- Target sharding over several GPUs ---------------------------------------------
+ * The fields of different targets j of eq. 6 are independent given all source positions, so the rows of
+ * the interaction matrix shard over G GPUs: every rank holds the WHOLE active state (16 B per hole), rank g runs a1..a7
+ * for the targets of its share against all sources, compacts its survivors (a8) into a MESSAGE, and the G messages
+ * concatenated in rank order are the next step's state — in the same stable order one GPU would produce.  The share
+ * of rank g is the contiguous 256-hole tiles [floor(g T/G), floor((g+1) T/G)) of the T = ceil(n_active/256) tiles: a
+ * pure function of n_active, so shares re-balance every step without communication.  The only exchange per step is
+ * the all-gather of the messages, which is the CALLER's plumbing (NCCL through torch.distributed, or peer-mapped
+ * buffers); the library never waits on another rank inside a kernel.  Images, counters and collection records stay
+ * rank-local: the global image is the integer sum over ranks, and sum_g pair_interactions_g = sum_steps n_active^2.
+ *
+ * set_shard: rank < world <= 64; only on an empty handle (before the first load / after reset); world = 1 restores
+ *   the unsharded mode.  INVALID with GCORECCD_COULOMB_OFF (independent carriers: run replicas).  Every rank then
+ *   loads the SAME carriers in the same order (load_carriers / generate_cloud / load_snapshot); holes collected at
+ *   load are binned by rank 0 only.  While world > 1, step / run_to_collection / eval_field / profile_step return STATE.
+ * shard_message_bytes: bytes a message buffer should have for the handle's current upper bound on n_active (refreshed
+ *   by get_state): 256-byte header + 16 bytes x entries, entries = 256 x ceil(tiles/world) with tiles rounded up to a
+ *   power of two.  Identical on all ranks that called get_state at the same step.
+ * shard_local: a1..a7 for this rank's share + compaction of its survivors into msg_dev (DEVICE pointer, 16-byte
+ *   aligned, msg_bytes as above or larger; layout header | x[] | y[] | z[] | id[]).  Asynchronous on the stream.
+ *   Does not change the state.  CAPACITY if the buffer cannot hold the largest share.
+ * shard_commit: msgs_host is a HOST array of `world` DEVICE pointers, message g produced by rank g for the SAME step
+ *   with the SAME msg_bytes (slices of an all-gather receive buffer, or the ranks' own buffers mapped through CUDA
+ *   IPC / symmetric memory: the loads then cross NVLink inside this kernel).  Replaces the active state by the
+ *   concatenation, step += 1, pair_interactions += share x n_active, plans the next share.  Asynchronous.  A message
+ *   whose (n_active, step, rank) header disagrees with this rank sets a sticky flag that get_state reports as STATE.
+ *   The caller must not overwrite a message before every rank has committed it (alternate two buffers). */
+int gcoreccd_set_shard(gcoreccd_t* h, uint32_t rank, uint32_t world);
+uint64_t gcoreccd_shard_message_bytes(gcoreccd_t* h);
+int gcoreccd_shard_local(gcoreccd_t* h, void* msg_dev, uint64_t msg_bytes);
+int gcoreccd_shard_commit(gcoreccd_t* h, const void* const* msgs_host, uint32_t n_msgs, uint64_t msg_bytes);
+
 /* Run ONE step with CUDA events between its kernels (on the handle's stream) and return the device time of
  * each in milliseconds: ms[0] field, ms[1] integrate+collect, ms[2] compact, ms[3] whole step.  Synchronous. */
 int gcoreccd_profile_step(gcoreccd_t* h, float ms_host[4]);

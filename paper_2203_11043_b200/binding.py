@@ -22,6 +22,7 @@ EXPORTS = ["gcoreccd_workspace_size", "gcoreccd_create", "gcoreccd_destroy", "gc
            "gcoreccd_load_events", "gcoreccd_run_events", "gcoreccd_get_events", "gcoreccd_read_event_carriers",
            "gcoreccd_xray_hole_count", "gcoreccd_generate_cloud", "gcoreccd_generate_xray_events",
            "gcoreccd_load_carriers_file", "gcoreccd_save_collected_file",
+           "gcoreccd_set_shard", "gcoreccd_shard_message_bytes", "gcoreccd_shard_local", "gcoreccd_shard_commit",
            "gcoreccd_profile_step", "gcoreccd_kernel_launches", "gcoreccd_debug_normals", "gcoreccd_strerror",
            "gcoreccd_last_error", "gcoreccd_version"]
 
@@ -105,6 +106,14 @@ def lib():
     L.gcoreccd_load_carriers_file.argtypes = [vp, C.c_char_p, u64p]
     L.gcoreccd_save_collected_file.restype = C.c_int
     L.gcoreccd_save_collected_file.argtypes = [vp, C.c_char_p, u64p]
+    L.gcoreccd_set_shard.restype = C.c_int
+    L.gcoreccd_set_shard.argtypes = [vp, C.c_uint32, C.c_uint32]
+    L.gcoreccd_shard_message_bytes.restype = C.c_uint64
+    L.gcoreccd_shard_message_bytes.argtypes = [vp]
+    L.gcoreccd_shard_local.restype = C.c_int
+    L.gcoreccd_shard_local.argtypes = [vp, vp, C.c_uint64]
+    L.gcoreccd_shard_commit.restype = C.c_int
+    L.gcoreccd_shard_commit.argtypes = [vp, C.POINTER(vp), C.c_uint32, C.c_uint64]
     L.gcoreccd_profile_step.restype = C.c_int
     L.gcoreccd_profile_step.argtypes = [vp, fp]
     L.gcoreccd_kernel_launches.restype = C.c_uint64
@@ -373,6 +382,20 @@ class Gcoreccd:
         if k:
             self._check(lib().gcoreccd_eval_field(self._h, C.c_void_p(E.ctypes.data), k, 0), "gcoreccd_eval_field")
         return E
+
+    # ---- target sharding (include/gcoreccd.h "Target sharding"; the orchestration is sharded.py) ----
+    def set_shard(self, rank, world):
+        self._check(lib().gcoreccd_set_shard(self._h, int(rank), int(world)), "set_shard")
+
+    def shard_message_bytes(self):
+        return int(lib().gcoreccd_shard_message_bytes(self._h))
+
+    def shard_local(self, msg_ptr, msg_bytes):
+        self._check(lib().gcoreccd_shard_local(self._h, C.c_void_p(int(msg_ptr)), int(msg_bytes)), "shard_local")
+
+    def shard_commit(self, msg_ptrs, msg_bytes):
+        arr = (C.c_void_p * len(msg_ptrs))(*[int(p) for p in msg_ptrs])
+        self._check(lib().gcoreccd_shard_commit(self._h, arr, len(msg_ptrs), int(msg_bytes)), "shard_commit")
 
     def profile_step(self):
         ms = (C.c_float * 4)()

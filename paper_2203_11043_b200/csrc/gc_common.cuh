@@ -27,6 +27,8 @@ struct FieldPlan {
   uint32_t JC;       // sources per chunk (multiple of 8)
   uint32_t stride;   // row stride of the partial buffers (n rounded up to 256)
   uint32_t IB;       // targets per row block the plan was made for
+  uint32_t t0;       // first target of this rank's share (multiple of 256; 0 when not sharded)
+  uint32_t nt;       // targets in the share (= n when not sharded); row blocks and partial rows cover [t0, t0+nt)
 };
 
 struct Ctrl {                 // lives in device memory; only kernels write it (plus reset/load on the stream)
@@ -41,8 +43,9 @@ struct Ctrl {                 // lives in device memory; only kernels write it (
   uint32_t invalid;           // load validation flag
   uint32_t blocks_done;       // "last block finishes" counter of the compactor
   uint32_t multi_steps;       // scratch of the Coulomb-off multi-step kernel: steps the longest-lived carrier took
-  FieldPlan plan;             // valid for (n_active, current field variant)
-  uint32_t pad2_[2];
+  FieldPlan plan;             // valid for (n_active, current field variant, shard)
+  uint32_t diverged;          // sticky: a shard message disagreed with this rank's (n_active, step) (gc_shard.cuh)
+  uint32_t pad2_;
 };
 
 struct SoA {                  // one state set
@@ -70,7 +73,18 @@ struct Sink {                 // where a collected hole goes (a7)
   uint32_t fin_cap;           // ids >= fin_cap are binned but not recorded
 };
 
-struct PlanArgs { uint32_t IB; uint32_t grid; uint32_t part_cap_entries; };
+struct PlanArgs { uint32_t IB; uint32_t grid; uint32_t part_cap_entries; uint32_t rank; uint32_t world; };
+
+// Target sharding: the state is replicated on every rank, the rows of the
+// interaction matrix are not.  The n active carriers form ceil(n/256) tiles; rank g of G owns the contiguous tiles
+// [floor(g T / G), floor((g+1) T / G)), i.e. targets [t0, t0 + nt).  A pure function of (n, g, G): every rank
+// derives every share without communication, and the shares re-balance by themselves as carriers retire.
+__host__ __device__ inline void shard_range(uint32_t n, uint32_t rank, uint32_t world, uint32_t& t0, uint32_t& nt) {
+  const uint64_t T = ((uint64_t)n + 255u) >> 8;
+  const uint64_t a = (T * rank / world) << 8, b = (T * (rank + 1u) / world) << 8;
+  const uint64_t lo = a < n ? a : n, hi = b < n ? b : n;
+  t0 = (uint32_t)lo; nt = (uint32_t)(hi - lo);
+}
 
 #ifdef __CUDACC__
 // Executed by ONE full warp.  Static round-robin makespan model: a CTA runs ceil(items/grid) items, each costing
@@ -83,10 +97,11 @@ __device__ inline FieldPlan plan_search(uint32_t n, PlanArgs a) {
   const uint32_t lane = threadIdx.x & 31u;
   FieldPlan p;
   p.n = n; p.IB = a.IB;
-  p.nIB = (n + a.IB - 1) / a.IB;
-  p.stride = (n + 255u) & ~255u;
+  shard_range(n, a.rank, a.world, p.t0, p.nt);
+  p.nIB = (p.nt + a.IB - 1) / a.IB;
+  p.stride = (p.nt + 255u) & ~255u;
   p.S = 0; p.JC = 0;
-  if (n == 0) return p;
+  if (n == 0 || p.nt == 0) return p;
   uint32_t s_max = (n + kMinChunk - 1) / kMinChunk;
   const uint32_t s_cap = a.part_cap_entries / p.stride;
   const uint32_t s_bal = max(64u, (4u * a.grid + p.nIB - 1) / p.nIB);      // beyond ~4 rounds nothing improves

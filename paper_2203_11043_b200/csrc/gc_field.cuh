@@ -61,7 +61,7 @@ struct FieldCfg {
 };
 
 // Partial sums: Ep is three planes (x,y,z) of part_cap floats each; plane c, chunk s, target i at
-// Ep[c*part_cap + s*stride + i].  The value stored is sum (r_s - r_t) w = -S_t (sign folded by the consumer).
+// Ep[c*part_cap + s*stride + (i - t0)], [t0, t0+nt) being the targets this rank owns (all of them if unsharded).  The value stored is sum (r_s - r_t) w = -S_t (sign folded by the consumer).
 template <int NPACK, int TPB, int MINB, int UNROLL = 4>
 __global__ void __launch_bounds__(TPB, MINB)
 k_field(const float* __restrict__ px, const float* __restrict__ py, const float* __restrict__ pz,
@@ -80,7 +80,8 @@ k_field(const float* __restrict__ px, const float* __restrict__ py, const float*
 
   for (uint32_t item = blockIdx.x; item < items; item += gridDim.x) {
     const uint32_t ib = item / plan.S, sc = item - ib * plan.S;
-    const uint32_t i_base = ib * IB;
+    const uint32_t i_base = plan.t0 + ib * IB;             // this rank's share of the targets (whole set if unsharded)
+    const uint32_t i_end = plan.t0 + plan.nt;
     const uint32_t j0 = sc * plan.JC;
     const uint32_t j1 = min(j0 + plan.JC, n);
 
@@ -91,11 +92,11 @@ k_field(const float* __restrict__ px, const float* __restrict__ py, const float*
     for (int p = 0; p < NPACK; ++p) {
       const uint32_t i0 = i_base + (p * TPB + tid) * 2u;
       float2 vx = make_float2(0.f, 0.f), vy = vx, vz = vx;
-      if (i0 + 1 < n) {                               // arrays are padded, but keep padding out of the math
+      if (i0 + 1 < i_end) {                           // arrays are padded, but keep padding out of the math
         vx = *reinterpret_cast<const float2*>(px + i0);
         vy = *reinterpret_cast<const float2*>(py + i0);
         vz = *reinterpret_cast<const float2*>(pz + i0);
-      } else if (i0 < n) {
+      } else if (i0 < i_end) {
         vx.x = px[i0]; vy.x = py[i0]; vz.x = pz[i0];
       }
       ntx[p] = make_float2(-vx.x, -vx.y); nty[p] = make_float2(-vy.x, -vy.y); ntz[p] = make_float2(-vz.x, -vz.y);
@@ -152,8 +153,8 @@ k_field(const float* __restrict__ px, const float* __restrict__ py, const float*
     float* ez = ey + part_cap;
 #pragma unroll
     for (int p = 0; p < NPACK; ++p) {
-      const uint32_t i0 = i_base + (p * TPB + tid) * 2u;
-      if (i0 < plan.stride) {                          // stride >= n, even: the float2 store stays inside the row
+      const uint32_t i0 = i_base - plan.t0 + (p * TPB + tid) * 2u;   // partial rows are indexed from the share's start
+      if (i0 < plan.stride) {                          // stride >= nt, even: the float2 store stays inside the row
         *reinterpret_cast<float2*>(ex + i0) = tx[p];
         *reinterpret_cast<float2*>(ey + i0) = ty[p];
         *reinterpret_cast<float2*>(ez + i0) = tz[p];

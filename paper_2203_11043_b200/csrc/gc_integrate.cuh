@@ -132,17 +132,18 @@ __device__ __forceinline__ void tally(uint32_t coll, uint32_t over, uint32_t kee
 __global__ void __launch_bounds__(kTPB, 4)      // 64 registers: 4 CTAs/SM, 151,552 carriers in one wave on 148 SMs
 k_integrate(SoA A, SoA B, Ctrl* __restrict__ ctrl, const float* __restrict__ Ep, uint32_t part_cap,
             Sink sink, uint32_t* __restrict__ tile_count, DevParams P) {
-  const uint32_t n = ctrl->n_active;
-  const uint32_t i = blockIdx.x * kTPB + threadIdx.x;
-  if (blockIdx.x * kTPB >= n) return;
+  const uint32_t t0 = ctrl->plan.t0, nt = ctrl->plan.nt;     // this rank's share: [0, n_active) unless sharded
+  const uint32_t k = blockIdx.x * kTPB + threadIdx.x;        // index inside the share (= partial-sum row)
+  if (blockIdx.x * kTPB >= nt) return;
+  const uint32_t i = t0 + k;
   const uint64_t step = ctrl->step;
   uint32_t coll = 0, over = 0, keep = 0;
-  if (i < n) {
+  if (k < nt) {
     const float x = A.x[i], y = A.y[i], z = A.z[i];
     const uint32_t id = A.id[i];
     double Ex = 0.0, Ey = 0.0, Ez = 0.0;
     if (!(P.flags & 1u)) {                                   // GCORECCD_COULOMB_OFF
-      reduce_partials(Ep + i, part_cap, ctrl->plan.S, ctrl->plan.stride, Ex, Ey, Ez);
+      reduce_partials(Ep + k, part_cap, ctrl->plan.S, ctrl->plan.stride, Ex, Ey, Ez);
       Ex *= -P.Kp; Ey *= -P.Kp; Ez *= -P.Kp;                 // partials hold sum (r_s - r_t) w
     }
     float xf, yf, zf;
@@ -190,14 +191,15 @@ k_drift_multi(SoA A, SoA B, Ctrl* __restrict__ ctrl, Sink sink, uint32_t* __rest
 // Load path: unpack interleaved xyz into state B at [0,n), assign ids n_loaded + k, collect z <= z_well.
 __global__ void __launch_bounds__(kTPB)
 k_unpack(const float* __restrict__ xyz, uint32_t n, SoA B, Ctrl* __restrict__ ctrl, uint32_t id_base,
-         Sink sink, uint32_t* __restrict__ tile_count, DevParams P) {
+         Sink sink, uint32_t* __restrict__ tile_count, DevParams P, uint32_t record) {
   const uint32_t i = blockIdx.x * kTPB + threadIdx.x;
   uint32_t coll = 0, over = 0, keep = 0;
   const uint64_t step = ctrl->step;
   if (i < n) {
     const float x = xyz[3 * (size_t)i], y = xyz[3 * (size_t)i + 1], z = xyz[3 * (size_t)i + 2];
     B.x[i] = x; B.y[i] = y; B.z[i] = z; B.id[i] = id_base + i;
-    if ((double)z <= P.z_well) { coll = 1; uint32_t o = 0; collect(x, y, z, id_base + i, step, P, sink, o); over = o; }
+    // sharded runs load the same holes on every rank: only rank 0 (record = 1) bins the ones collected at load
+    if ((double)z <= P.z_well) { if (record) { coll = 1; uint32_t o = 0; collect(x, y, z, id_base + i, step, P, sink, o); over = o; } }
     else keep = 1;
   }
   tally(coll, over, keep, ctrl, tile_count);

@@ -17,6 +17,7 @@
 #include "gc_field.cuh"
 #include "gc_frontend.cuh"
 #include "gc_integrate.cuh"
+#include "gc_shard.cuh"
 
 using namespace gc;
 
@@ -78,6 +79,7 @@ struct gcoreccd {
   int graph_variant;
   uint32_t graph_tiles;
   cudaEvent_t ev[4];
+  uint32_t shard_rank, shard_world;   // target sharding (gc_shard.cuh); world 1 = not sharded
   char err[256];
   // batched independent events (gc_events.cuh)
   struct {
@@ -134,6 +136,8 @@ inline PlanArgs plan_args(const gcoreccd_t* h, int v) {
   a.IB = variant_ib(v);
   a.grid = (uint32_t)h->grid_field[v];
   a.part_cap_entries = (uint32_t)h->L.part_cap;
+  a.rank = h->shard_rank;
+  a.world = h->shard_world;
   return a;
 }
 
@@ -289,6 +293,7 @@ int gcoreccd_create(const gcoreccd_params* p, gcoreccd_t** out) {
   h->device = dev;
   h->num_sms = prop.multiProcessorCount;
   h->variant = -1;
+  h->shard_world = 1;
   DeviceGuard guard(dev);
 
   h->L = make_layout(p->max_carriers, p->img_nx, p->img_ny);
@@ -422,7 +427,7 @@ int gcoreccd_load_carriers(gcoreccd_t* h, const float* xyz, uint64_t n, int on_d
   const int v = pick_variant(n_act + n);
   h->variant = v;
   k_unpack<<<tiles, kTPB, 0, h->stream>>>(src, (uint32_t)n, h->B, h->ctrl, (uint32_t)h->n_loaded, h->sink,
-                                          h->tile_count, h->dp);
+                                          h->tile_count, h->dp, h->shard_rank == 0 ? 1u : 0u);
   k_compact<<<tiles, kTPB, 0, h->stream>>>(h->B, h->A, h->ctrl, h->tile_count, (uint32_t)n, (uint32_t)n_act, 1,
                                            h->dp.z_well, 0u, plan_args(h, v));
   h->launches += 2;
@@ -462,12 +467,14 @@ int gcoreccd_load_snapshot(gcoreccd_t* h, const float* xyz, const uint32_t* id, 
 
 int gcoreccd_step(gcoreccd_t* h, uint32_t n_steps) {
   if (!h) return GCORECCD_ERR_INVALID;
+  if (h->shard_world > 1) return fail(h, GCORECCD_ERR_STATE, "step: the handle is sharded (use shard_local / shard_commit)");
   DeviceGuard guard(h->device);
   return enqueue_steps(h, n_steps);
 }
 
 int gcoreccd_run_to_collection(gcoreccd_t* h, uint64_t max_steps, uint64_t* steps_done, uint64_t* n_active_left) {
   if (!h) return GCORECCD_ERR_INVALID;
+  if (h->shard_world > 1) return fail(h, GCORECCD_ERR_STATE, "run_to_collection: the handle is sharded");
   DeviceGuard guard(h->device);
   int rc = sync_ctrl(h);
   if (rc) return rc;
@@ -515,6 +522,7 @@ int gcoreccd_get_state(gcoreccd_t* h, uint64_t* step, uint64_t* n_active, uint64
   if (n_out_of_window) *n_out_of_window = h->h_ctrl->n_overflow;
   if (pair_interactions) *pair_interactions = h->h_ctrl->pairs;
   if (h->h_ctrl->nonfinite) return fail(h, GCORECCD_ERR_NONFINITE, "a carrier position became non-finite");
+  if (h->h_ctrl->diverged) return fail(h, GCORECCD_ERR_STATE, "shard messages disagree with this rank's state (ranks diverged)");
   return GCORECCD_OK;
 }
 
@@ -567,6 +575,7 @@ int gcoreccd_eval_field(gcoreccd_t* h, float* E, uint64_t cap, int on_device) {
   if (rc) return rc;
   const uint64_t na = h->h_ctrl->n_active;
   if (cap < na) return fail(h, GCORECCD_ERR_CAPACITY, "eval_field: buffer too small");
+  if (h->shard_world > 1) return fail(h, GCORECCD_ERR_STATE, "eval_field: the handle is sharded");
   if (na == 0) return GCORECCD_OK;
   rc = ensure_variant(h);
   if (rc) return rc;
@@ -584,6 +593,7 @@ int gcoreccd_profile_step(gcoreccd_t* h, float ms[4]) {
   if (!h || !ms) return GCORECCD_ERR_INVALID;
   DeviceGuard guard(h->device);
   ms[0] = ms[1] = ms[2] = ms[3] = 0.f;
+  if (h->shard_world > 1) return fail(h, GCORECCD_ERR_STATE, "profile_step: the handle is sharded");
   if (h->n_bound == 0) return GCORECCD_OK;
   int rc = ensure_variant(h);
   if (rc) return rc;
@@ -606,6 +616,83 @@ int gcoreccd_profile_step(gcoreccd_t* h, float ms[4]) {
   GC_CUDA(h, cudaEventElapsedTime(&ms[1], h->ev[1], h->ev[2]));
   GC_CUDA(h, cudaEventElapsedTime(&ms[2], h->ev[2], h->ev[3]));
   GC_CUDA(h, cudaEventElapsedTime(&ms[3], h->ev[0], h->ev[3]));
+  return GCORECCD_OK;
+}
+
+// ---- target sharding (gc_shard.cuh) ----------------------------------------------------------------------------
+namespace {
+// entries per coordinate array of a shard message for the host's current bound on n_active: the largest share of
+// ceil(tiles / world) tiles, tiles taken from the same power-of-two bucket on every rank
+inline uint64_t shard_bs(const gcoreccd_t* h) {
+  const uint64_t tiles = bucket_tiles(tiles_for(h->n_bound ? h->n_bound : 1));
+  return (uint64_t)kTPB * ((tiles + h->shard_world - 1) / h->shard_world);
+}
+// entries per coordinate array a caller's message of msg_bytes holds (0 if it cannot hold the largest share)
+inline uint64_t shard_bs_of(const gcoreccd_t* h, uint64_t msg_bytes) {
+  if (msg_bytes < kShardHeaderBytes + 16ull * kTPB) return 0;
+  const uint64_t bs = (msg_bytes - kShardHeaderBytes) / 16 / kTPB * kTPB;
+  const uint64_t need = (uint64_t)kTPB * ((tiles_for(h->n_bound ? h->n_bound : 1) + h->shard_world - 1) / h->shard_world);
+  return bs >= need && bs <= 0xffffff00ull ? bs : 0;
+}
+}  // namespace
+
+int gcoreccd_set_shard(gcoreccd_t* h, uint32_t rank, uint32_t world) {
+  if (!h || world == 0 || world > kShardMaxWorld || rank >= world) return GCORECCD_ERR_INVALID;
+  if (world > 1 && (h->dp.flags & GCORECCD_COULOMB_OFF))
+    return fail(h, GCORECCD_ERR_INVALID, "set_shard: without eq. 6 carriers are independent; run replicas instead");
+  if (h->n_loaded != 0 || h->evb.loaded) return fail(h, GCORECCD_ERR_STATE, "set_shard: only on an empty handle (reset first)");
+  h->shard_rank = rank;
+  h->shard_world = world;
+  h->variant = -1;
+  return GCORECCD_OK;
+}
+
+uint64_t gcoreccd_shard_message_bytes(gcoreccd_t* h) {
+  if (!h) return 0;
+  return kShardHeaderBytes + 16ull * shard_bs(h);
+}
+
+int gcoreccd_shard_local(gcoreccd_t* h, void* msg_dev, uint64_t msg_bytes) {
+  if (!h || !msg_dev) return GCORECCD_ERR_INVALID;
+  if (events_busy(h)) return fail(h, GCORECCD_ERR_STATE, "shard_local: a batch of events is loaded");
+  const uint64_t bs = shard_bs_of(h, msg_bytes);
+  if (bs == 0) return fail(h, GCORECCD_ERR_CAPACITY, "shard_local: message buffer too small");
+  if ((uintptr_t)msg_dev & 15u) return fail(h, GCORECCD_ERR_INVALID, "shard_local: message buffer must be 16-byte aligned");
+  DeviceGuard guard(h->device);
+  // the share shrinks with n_active: pick the field variant from the share, not from the whole population
+  const int v = pick_variant((h->n_bound + h->shard_world - 1) / h->shard_world);
+  if (v != h->variant) {
+    h->variant = v;
+    k_replan<<<1, 32, 0, h->stream>>>(h->ctrl, plan_args(h, v), 0, 0u, 0, 0ull);
+    h->launches += 1;
+  }
+  const uint32_t tiles = (uint32_t)(bs / kTPB);
+  launch_field(h, h->variant);
+  k_integrate<<<tiles, kTPB, 0, h->stream>>>(h->A, h->B, h->ctrl, h->Ep, (uint32_t)h->L.part_cap, h->sink,
+                                             h->tile_count, h->dp);
+  k_shard_compact<<<tiles, kTPB, 0, h->stream>>>(h->B, h->ctrl, h->tile_count, (char*)msg_dev, (uint32_t)bs,
+                                                 h->dp.z_well, h->shard_rank);
+  h->launches += 2;
+  GC_CUDA(h, cudaGetLastError());
+  return GCORECCD_OK;
+}
+
+int gcoreccd_shard_commit(gcoreccd_t* h, const void* const* msgs_host, uint32_t n_msgs, uint64_t msg_bytes) {
+  if (!h || !msgs_host) return GCORECCD_ERR_INVALID;
+  if (n_msgs != h->shard_world) return fail(h, GCORECCD_ERR_INVALID, "shard_commit: one message per rank is required");
+  const uint64_t bs = shard_bs_of(h, msg_bytes);
+  if (bs == 0) return fail(h, GCORECCD_ERR_CAPACITY, "shard_commit: message buffers too small");
+  ShardPtrs ptrs;
+  memset(&ptrs, 0, sizeof(ptrs));
+  for (uint32_t g = 0; g < n_msgs; ++g) {
+    if (!msgs_host[g] || ((uintptr_t)msgs_host[g] & 15u)) return fail(h, GCORECCD_ERR_INVALID, "shard_commit: bad message pointer");
+    ptrs.p[g] = (const char*)msgs_host[g];
+  }
+  DeviceGuard guard(h->device);
+  const uint32_t tiles = (uint32_t)(bs / kTPB);
+  k_shard_commit<<<tiles * n_msgs, kTPB, 0, h->stream>>>(ptrs, n_msgs, (uint32_t)bs, h->A, h->ctrl, plan_args(h, h->variant));
+  h->launches += 1;
+  GC_CUDA(h, cudaGetLastError());
   return GCORECCD_OK;
 }
 

@@ -8,7 +8,7 @@ import pytest
 
 from oracle import goracle as g
 from paper_2203_11043_b200 import workloads
-from util import field_rel_err, gpu_sim, image_moments, oracle_sim
+from util import field_rel_err, gpu_sim, image_moments, oracle_sim, traj_assert
 
 pytestmark = pytest.mark.gpu
 
@@ -91,23 +91,7 @@ def _trajectory_check(w, flags_gpu, flags_or, steps=10, tol=TRAJ_TOL, **over):
     assert st["step"] == ost["step"]
     assert st["n_active"] + st["n_collected"] == st["n_loaded"]
     sim.close()
-    common = np.intersect1d(ids, oids)
-    xyz_c, oxyz_c = xyz[np.isin(ids, common)], oxyz[np.isin(oids, common)]
-    d = np.abs(xyz_c.astype(np.float64) - oxyz_c).max(axis=1)
-    suspects = set(common[d > tol].tolist()) | set(np.setxor1d(ids, oids).tolist())   # incl. retire-flag mismatches
-    if suspects:
-        assert len(suspects) <= 0.02 * len(w["xyz"]) + 2, len(suspects)
-        closest = {i: np.inf for i in suspects}
-        for hx, hid in history:
-            for i in suspects:
-                k = np.searchsorted(hid, i)
-                if k < len(hid) and hid[k] == i:
-                    r = np.linalg.norm(hx - hx[k], axis=1)
-                    r[k] = np.inf
-                    closest[i] = min(closest[i], r.min())
-        # retire-flag mismatches must sit at the collection plane, or come from a close encounter like the rest
-        for i, r in closest.items():
-            assert r < 0.1, (i, r, "exceeds %g um without a close encounter" % tol)
+    d = traj_assert(xyz, ids, oxyz, oids, history, len(w["xyz"]), tol)
     return d
 
 
