@@ -226,6 +226,25 @@ uint64_t gcoreccd_shard_message_bytes(gcoreccd_t* h);
 int gcoreccd_shard_local(gcoreccd_t* h, void* msg_dev, uint64_t msg_bytes);
 int gcoreccd_shard_commit(gcoreccd_t* h, const void* const* msgs_host, uint32_t n_msgs, uint64_t msg_bytes);
 
+/* ---- Far-field approximation of eq. 6 — a VARIANT, off by default --------------------------
+ * The exact path sums all N_a^2 ordered pairs.  With set_farfield(theta >= 0) step a1 is replaced by
+ * a treecode: the active holes are kept in Hilbert-curve order (re-sorted every resort_every field evaluations; 0 => 8), an
+ * implicit 8-ary tree of runs of 32*8^l consecutive holes carries, per node, its hole count m, centre of charge c and
+ * bounding radius a; every group of 256 consecutive targets (ball (c_T, r_T)) replaces a node by ONE pseudo-hole of
+ * charge m at c when  a <= theta * (|c - c_T| - r_T)  and sums all other holes exactly.  a2..a8 are unchanged.
+ * Stated bound (monopole about the centre of charge; the dipole vanishes): for every target j
+ *     |E_approx,j - E_exact,j|  <=  B(theta) * sum_{accepted nodes} m K' / d_j^2 ,   B = theta^2 (3 - 2 theta)/(1 - theta)^2,
+ * d_j the distance from j to the node's centre; the near field is exact; theta = 0 accepts no node (exact sum in
+ * another order).  Measured errors are one to two orders below the bound (tests/test_gpu_farfield.py).
+ * Consequences: the active set is no longer in load order (read_carriers / eval_field return the current curve order;
+ * match by id); pair_interactions still counts N_a^2 per step (the pairs REPRESENTED) — the interactions actually
+ * evaluated are in farfield_stats and no throughput claim of the exact metric may use this variant.
+ * set_farfield: theta in [0, 1) switches the variant on, theta < 0 off; STATE on a sharded handle.  Synchronises.
+ * farfield_stats: interactions evaluated since set_farfield — pseudo-hole (far) and exact (near), each counted per
+ *   target — and B(theta).  Host pointers, any may be NULL.  STATE if the variant is off. */
+int gcoreccd_set_farfield(gcoreccd_t* h, double theta, uint32_t resort_every);
+int gcoreccd_farfield_stats(gcoreccd_t* h, uint64_t* far_evals, uint64_t* near_evals, double* bound_B);
+
 /* Run ONE step with CUDA events between its kernels (on the handle's stream) and return the device time of
  * each in milliseconds: ms[0] field, ms[1] integrate+collect, ms[2] compact, ms[3] whole step.  Synchronous. */
 int gcoreccd_profile_step(gcoreccd_t* h, float ms_host[4]);

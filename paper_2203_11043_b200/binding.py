@@ -22,6 +22,7 @@ EXPORTS = ["gcoreccd_workspace_size", "gcoreccd_create", "gcoreccd_destroy", "gc
            "gcoreccd_load_events", "gcoreccd_run_events", "gcoreccd_get_events", "gcoreccd_read_event_carriers",
            "gcoreccd_xray_hole_count", "gcoreccd_generate_cloud", "gcoreccd_generate_xray_events",
            "gcoreccd_load_carriers_file", "gcoreccd_save_collected_file",
+           "gcoreccd_set_farfield", "gcoreccd_farfield_stats",
            "gcoreccd_set_shard", "gcoreccd_shard_message_bytes", "gcoreccd_shard_local", "gcoreccd_shard_commit",
            "gcoreccd_profile_step", "gcoreccd_kernel_launches", "gcoreccd_debug_normals", "gcoreccd_strerror",
            "gcoreccd_last_error", "gcoreccd_version"]
@@ -114,6 +115,10 @@ def lib():
     L.gcoreccd_shard_local.argtypes = [vp, vp, C.c_uint64]
     L.gcoreccd_shard_commit.restype = C.c_int
     L.gcoreccd_shard_commit.argtypes = [vp, C.POINTER(vp), C.c_uint32, C.c_uint64]
+    L.gcoreccd_set_farfield.restype = C.c_int
+    L.gcoreccd_set_farfield.argtypes = [vp, C.c_double, C.c_uint32]
+    L.gcoreccd_farfield_stats.restype = C.c_int
+    L.gcoreccd_farfield_stats.argtypes = [vp, u64p, u64p, C.POINTER(C.c_double)]
     L.gcoreccd_profile_step.restype = C.c_int
     L.gcoreccd_profile_step.argtypes = [vp, fp]
     L.gcoreccd_kernel_launches.restype = C.c_uint64
@@ -382,6 +387,15 @@ class Gcoreccd:
         if k:
             self._check(lib().gcoreccd_eval_field(self._h, C.c_void_p(E.ctypes.data), k, 0), "gcoreccd_eval_field")
         return E
+
+    # ---- far-field variant (include/gcoreccd.h "Far-field approximation")
+    def set_farfield(self, theta, resort_every=0):
+        self._check(lib().gcoreccd_set_farfield(self._h, float(theta), int(resort_every)), "set_farfield")
+
+    def farfield_stats(self):
+        a, b, B = C.c_uint64(), C.c_uint64(), C.c_double()
+        self._check(lib().gcoreccd_farfield_stats(self._h, C.byref(a), C.byref(b), C.byref(B)), "farfield_stats")
+        return {"far_evals": int(a.value), "near_evals": int(b.value), "bound_B": float(B.value)}
 
     # ---- target sharding (include/gcoreccd.h "Target sharding"; the orchestration is sharded.py) ----
     def set_shard(self, rank, world):

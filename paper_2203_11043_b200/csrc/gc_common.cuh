@@ -73,7 +73,8 @@ struct Sink {                 // where a collected hole goes (a7)
   uint32_t fin_cap;           // ids >= fin_cap are binned but not recorded
 };
 
-struct PlanArgs { uint32_t IB; uint32_t grid; uint32_t part_cap_entries; uint32_t rank; uint32_t world; };
+struct PlanArgs { uint32_t IB; uint32_t grid; uint32_t part_cap_entries; uint32_t rank; uint32_t world;
+                  uint32_t force_S; };   // force_S > 0: no search, S chunks (the treecode's parts per group, gc_tree.cuh)
 
 // Target sharding: the state is replicated on every rank, the rows of the
 // interaction matrix are not.  The n active carriers form ceil(n/256) tiles; rank g of G owns the contiguous tiles
@@ -102,6 +103,7 @@ __device__ inline FieldPlan plan_search(uint32_t n, PlanArgs a) {
   p.stride = (p.nt + 255u) & ~255u;
   p.S = 0; p.JC = 0;
   if (n == 0 || p.nt == 0) return p;
+  if (a.force_S) { p.S = a.force_S; p.JC = (((n + p.S - 1) / p.S) + 7u) & ~7u; return p; }
   uint32_t s_max = (n + kMinChunk - 1) / kMinChunk;
   const uint32_t s_cap = a.part_cap_entries / p.stride;
   const uint32_t s_bal = max(64u, (4u * a.grid + p.nIB - 1) / p.nIB);      // beyond ~4 rounds nothing improves

@@ -1,0 +1,630 @@
+// gc_tree.cuh — far-field approximation of eq. 6 (second half; "O(N^2)", 92).
+// A VARIANT, off by default and reported separately from the exact all-pairs metric: gcoreccd_set_farfield(theta).
+//
+// Method (a GPU treecode over an implicit tree; nothing of it is in the paper, whose kernel is all-pairs):
+//   1. every `resort` steps the active carriers are reordered along a 48-bit Hilbert curve of their bounding box
+//      (LSD radix sort written here: block histograms, one scan, stable warp-match scatter; no Thrust/CUB);
+//   2. every step an implicit 8-ary tree is laid over that order: the level-l node k is the run of 32*8^l consecutive
+//      carriers starting at k*32*8^l; a node stores its hole count m, its centre of charge c (the dipole about c
+//      vanishes) and the radius a of the smallest ball about c holding its members (computed from the CURRENT
+//      positions, so the nodes stay valid between re-sorts, only less compact);
+//   3. every 256 consecutive targets (= one level-1 node; Q_T = the union of the axis-aligned boxes of its 8 leaves) walk
+//      the tree level by level: a node is
+//      ACCEPTED when  a <= theta * D,  D = dist(c, Q_T) > 0  (every target then sees it under a/d <= theta) and
+//      enters the group's far list as one pseudo-hole of charge m at c; otherwise it is opened (its 8 children join
+//      the next level's frontier) or, at the leaf level, its 32 holes enter the near list and are summed exactly;
+//   4. the lists are consumed by the same packed FP32x2 inner loop as k_field (weighted by m for pseudo-holes).
+//
+// Error bound (stated, and checked against the FP64 oracle in tests/test_gpu_farfield.py): for one accepted node,
+// expanding grad(1/|x - s|) about c, the monopole term is kept, the dipole terms cancel in the sum over the node,
+// and the rest is bounded by  (m K'/d^2) * sum_{k>=2} (k+1) (a/d)^k  =  (m K'/d^2) * t^2 (3 - 2t)/(1 - t)^2, t = a/d
+// <= theta.  Hence  |E_approx - E_exact|_j  <=  B(theta) * sum_{accepted nodes} m K'/d_j^2  <=  B(theta) * sum_i
+// K'/|r_ij|^2-like field-magnitude sum (the sum of the MAGNITUDES of the far pair fields, not of the net field),
+// B(theta) = theta^2 (3 - 2 theta)/(1 - theta)^2.  Softening (eps = 1e-3 um) enters at relative order eps^2/d^2.
+// The near field is exact.  theta = 0 accepts nothing: the result is the exact sum in a different order.
+#pragma once
+#include "gc_common.cuh"
+#include "gc_field.cuh"
+
+namespace gc {
+
+constexpr uint32_t kLeaf = 32;             // carriers per level-0 node
+constexpr uint32_t kFan = 8;               // children per node
+constexpr uint32_t kTreeMaxLevels = 9;     // 32 * 8^8 > 2^26
+constexpr uint32_t kGroup = 256;           // targets per traversal group = one level-1 node
+constexpr int kTreeTPB = 128;              // threads of k_tree_field: one packed pair of targets each
+constexpr uint32_t kFarCap = 2048, kNearCap = 512, kFrontCap = 2048;
+constexpr uint32_t kTopNodes = 64;         // the walk starts at the lowest level with at most this many nodes
+constexpr uint32_t kSortBlock = 2048;      // keys per block of the radix passes (256 threads x 8)
+
+struct TreeCtrl {                          // device resident, next to the tree arrays
+  uint32_t lo[3], hi[3];                   // bounding box, order-preserving integer images of the floats
+  uint32_t next_group;                     // dynamic work counter of k_tree_field
+  uint32_t pad_;
+  unsigned long long far_evals, near_evals;  // interactions actually evaluated (pseudo-hole and exact)
+};
+
+struct Tree {                              // device pointers carved from the workspace
+  TreeCtrl* tc;
+  float4* node_c;                          // (cx, cy, cz, m), all levels concatenated, level 0 first
+  float* node_r;
+  unsigned long long* key[2];              // radix sort double buffers: 48-bit curve keys ...
+  uint32_t* val[2];                        // ... and the carrier index they came from
+  uint32_t* counts;                        // [256][blocks] digit histograms
+};
+
+__host__ __device__ inline uint32_t level_size(uint32_t l) { return kLeaf << (3u * l); }
+__host__ __device__ inline uint32_t nodes_at(uint32_t n, uint32_t l) {
+  const uint64_t s = (uint64_t)kLeaf << (3u * l);
+  return (uint32_t)(((uint64_t)n + s - 1) / s);
+}
+__host__ __device__ inline uint32_t level_offset(uint32_t n, uint32_t l) {
+  uint32_t o = 0;
+  for (uint32_t k = 0; k < l; ++k) o += nodes_at(n, k);
+  return o;
+}
+
+__device__ __forceinline__ uint32_t f2ord(float f) {
+  const uint32_t b = __float_as_uint(f);
+  return b ^ ((b >> 31) ? 0xffffffffu : 0x80000000u);
+}
+__device__ __forceinline__ float ord2f(uint32_t o) {
+  return __uint_as_float(o ^ ((o >> 31) ? 0x80000000u : 0xffffffffu));
+}
+
+__global__ void k_tree_reset(TreeCtrl* __restrict__ tc, int reset_box) {
+  if (threadIdx.x == 0) {
+    tc->next_group = 0;
+    if (reset_box) {
+      for (int c = 0; c < 3; ++c) { tc->lo[c] = 0xffffffffu; tc->hi[c] = 0u; }
+    }
+  }
+}
+
+__global__ void __launch_bounds__(kTPB)
+k_tree_bbox(const float* __restrict__ px, const float* __restrict__ py, const float* __restrict__ pz,
+            const Ctrl* __restrict__ ctrl, TreeCtrl* __restrict__ tc) {
+  const uint32_t n = ctrl->n_active;
+  uint32_t lo[3] = {0xffffffffu, 0xffffffffu, 0xffffffffu}, hi[3] = {0u, 0u, 0u};
+  for (uint32_t i = blockIdx.x * kTPB + threadIdx.x; i < n; i += gridDim.x * kTPB) {
+    const uint32_t v[3] = {f2ord(px[i]), f2ord(py[i]), f2ord(pz[i])};
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { lo[c] = min(lo[c], v[c]); hi[c] = max(hi[c], v[c]); }
+  }
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    lo[c] = __reduce_min_sync(0xffffffffu, lo[c]);
+    hi[c] = __reduce_max_sync(0xffffffffu, hi[c]);
+  }
+  if ((threadIdx.x & 31u) == 0) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { atomicMin(&tc->lo[c], lo[c]); atomicMax(&tc->hi[c], hi[c]); }
+  }
+}
+
+constexpr uint32_t kKeyBits = 16;          // bits per axis: 65,536^3 cells (a 1,350 um track resolves to 0.02 um)
+constexpr uint32_t kKeyPasses = 6;         // 48-bit keys, 8 bits per radix pass
+
+__device__ __forceinline__ unsigned long long spread3(uint32_t v) {     // 16 bits -> every third bit of 48
+  unsigned long long x = v & 0xffffull;
+  x = (x | (x << 32)) & 0x001f00000000ffffull;
+  x = (x | (x << 16)) & 0x001f0000ff0000ffull;
+  x = (x | (x << 8)) & 0x100f00f00f00f00full;
+  x = (x | (x << 4)) & 0x10c30c30c30c30c3ull;
+  x = (x | (x << 2)) & 0x1249249249249249ull;
+  return x;
+}
+
+// 48-bit space-filling-curve key on a cubic grid of 65,536^3 cells spanning the largest extent of the bounding box.
+__global__ void __launch_bounds__(kTPB)
+k_tree_keys(const float* __restrict__ px, const float* __restrict__ py, const float* __restrict__ pz,
+            const Ctrl* __restrict__ ctrl, const TreeCtrl* __restrict__ tc, unsigned long long* __restrict__ key,
+            uint32_t* __restrict__ val) {
+  const uint32_t n = ctrl->n_active;
+  const uint32_t i = blockIdx.x * kTPB + threadIdx.x;
+  if (i >= n) return;
+  const float x0 = ord2f(tc->lo[0]), y0 = ord2f(tc->lo[1]), z0 = ord2f(tc->lo[2]);
+  const float ext = fmaxf(fmaxf(ord2f(tc->hi[0]) - x0, ord2f(tc->hi[1]) - y0), fmaxf(ord2f(tc->hi[2]) - z0, 1e-30f));
+  constexpr float kCells = (float)((1u << kKeyBits) - 1u);
+  const float sc = kCells / ext;
+  const uint32_t qx = (uint32_t)fminf(fmaxf((px[i] - x0) * sc, 0.f), kCells);
+  const uint32_t qy = (uint32_t)fminf(fmaxf((py[i] - y0) * sc, 0.f), kCells);
+  const uint32_t qz = (uint32_t)fminf(fmaxf((pz[i] - z0) * sc, 0.f), kCells);
+  // Hilbert index of the cell (Skilling's axes-to-transpose transform, AIP Conf. Proc. 707, 2004): consecutive
+  // indices are always face-adjacent cells, so a run of consecutive carriers is spatially compact — a Morton run
+  // is not (it jumps at octant boundaries), and loose runs inflate the exact near field of step 3.
+  uint32_t X0 = qx, X1 = qy, X2 = qz;
+  for (uint32_t Q = 1u << (kKeyBits - 1); Q > 1u; Q >>= 1) {
+    const uint32_t Pm = Q - 1u;
+    if (X0 & Q) X0 ^= Pm;
+    if (X1 & Q) X0 ^= Pm; else { const uint32_t t = (X0 ^ X1) & Pm; X0 ^= t; X1 ^= t; }
+    if (X2 & Q) X0 ^= Pm; else { const uint32_t t = (X0 ^ X2) & Pm; X0 ^= t; X2 ^= t; }
+  }
+  X1 ^= X0; X2 ^= X1;
+  uint32_t t = 0;
+  for (uint32_t Q = 1u << (kKeyBits - 1); Q > 1u; Q >>= 1) if (X2 & Q) t ^= Q - 1u;
+  X0 ^= t; X1 ^= t; X2 ^= t;
+  key[i] = (spread3(X0) << 2) | (spread3(X1) << 1) | spread3(X2);
+  val[i] = i;
+}
+
+// ---- LSD radix sort, 8 bits per pass, keys + values; stable ------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_radix_hist(const unsigned long long* __restrict__ key, const Ctrl* __restrict__ ctrl, uint32_t shift, uint32_t* __restrict__ counts) {
+  __shared__ uint32_t s_h[256];
+  const uint32_t n = ctrl->n_active;
+  const uint32_t nb = (n + kSortBlock - 1) / kSortBlock;
+  if (blockIdx.x >= nb) return;
+  s_h[threadIdx.x] = 0;
+  __syncthreads();
+  const uint32_t base = blockIdx.x * kSortBlock;
+  for (uint32_t k = threadIdx.x; k < kSortBlock; k += 256) {
+    const uint32_t i = base + k;
+    if (i < n) atomicAdd(&s_h[(uint32_t)(key[i] >> shift) & 255u], 1u);
+  }
+  __syncthreads();
+  counts[threadIdx.x * nb + blockIdx.x] = s_h[threadIdx.x];
+}
+
+// exclusive scan of counts[256][nb] (digit-major), one block of 32 warps: warp w owns digit rows w, w+32, ...;
+// row sums (coalesced), a scan of the 256 row totals, then the in-row scans
+__global__ void __launch_bounds__(1024)
+k_radix_scan(const Ctrl* __restrict__ ctrl, uint32_t* __restrict__ counts) {
+  __shared__ uint32_t s_tot[256];
+  const uint32_t n = ctrl->n_active;
+  const uint32_t nb = (n + kSortBlock - 1) / kSortBlock;
+  const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+  for (uint32_t d = warp; d < 256; d += 32) {
+    uint32_t sum = 0;
+    for (uint32_t b = lane; b < nb; b += 32) sum += counts[d * nb + b];
+    sum = __reduce_add_sync(0xffffffffu, sum);
+    if (lane == 0) s_tot[d] = sum;
+  }
+  __syncthreads();
+  if (warp == 0) {
+    uint32_t run = 0;
+    for (uint32_t d0 = 0; d0 < 256; d0 += 32) {
+      const uint32_t v = s_tot[d0 + lane];
+      uint32_t inc = v;
+      for (int o = 1; o < 32; o <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= (uint32_t)o) inc += t; }
+      s_tot[d0 + lane] = run + inc - v;
+      run += __shfl_sync(0xffffffffu, inc, 31);
+    }
+  }
+  __syncthreads();
+  for (uint32_t d = warp; d < 256; d += 32) {
+    uint32_t run = s_tot[d];
+    for (uint32_t b0 = 0; b0 < nb; b0 += 32) {
+      const uint32_t b = b0 + lane;
+      const uint32_t v = b < nb ? counts[d * nb + b] : 0u;
+      uint32_t inc = v;
+      for (int o = 1; o < 32; o <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= (uint32_t)o) inc += t; }
+      if (b < nb) counts[d * nb + b] = run + inc - v;
+      run += __shfl_sync(0xffffffffu, inc, 31);
+    }
+  }
+}
+
+__global__ void __launch_bounds__(256)
+k_radix_scatter(const unsigned long long* __restrict__ key_in, const uint32_t* __restrict__ val_in, unsigned long long* __restrict__ key_out,
+                uint32_t* __restrict__ val_out, const Ctrl* __restrict__ ctrl, uint32_t shift,
+                const uint32_t* __restrict__ offsets) {
+  __shared__ uint32_t s_wh[8][256];       // per-warp digit counts of the current round
+  __shared__ uint32_t s_run[256];         // digits already placed by this block
+  const uint32_t n = ctrl->n_active;
+  const uint32_t nb = (n + kSortBlock - 1) / kSortBlock;
+  if (blockIdx.x >= nb) return;
+  const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+  s_run[tid] = offsets[tid * nb + blockIdx.x];
+  const uint32_t base = blockIdx.x * kSortBlock;
+  for (uint32_t r = 0; r < kSortBlock / 256; ++r) {
+    for (int w = 0; w < 8; ++w) s_wh[w][tid] = 0;
+    __syncthreads();
+    const uint32_t i = base + r * 256 + tid;
+    const bool ok = i < n;
+    const unsigned long long k = ok ? key_in[i] : 0ull;
+    const uint32_t v = ok ? val_in[i] : 0u;
+    const uint32_t d = ok ? ((uint32_t)(k >> shift) & 255u) : 256u + lane;          // invalid lanes match nobody
+    const uint32_t m = __match_any_sync(0xffffffffu, d);
+    const uint32_t rank = __popc(m & ((1u << lane) - 1u));
+    if (ok && rank == 0) s_wh[warp][d] = __popc(m);
+    __syncthreads();
+    // exclusive prefix over the 8 warps for digit `tid`, plus the running base
+    uint32_t acc = s_run[tid];
+    for (int w = 0; w < 8; ++w) { const uint32_t c = s_wh[w][tid]; s_wh[w][tid] = acc; acc += c; }
+    __syncthreads();
+    if (ok) {
+      const uint32_t pos = s_wh[warp][d] + rank;
+      key_out[pos] = k; val_out[pos] = v;
+    }
+    __syncthreads();
+    s_run[tid] = acc;
+  }
+}
+
+// reorder the state along the sorted permutation: dst[i] = src[val[i]]
+__global__ void __launch_bounds__(kTPB)
+k_tree_permute(SoA src, SoA dst, const uint32_t* __restrict__ val, const Ctrl* __restrict__ ctrl) {
+  const uint32_t n = ctrl->n_active;
+  const uint32_t i = blockIdx.x * kTPB + threadIdx.x;
+  if (i >= n) return;
+  const uint32_t s = val[i];
+  dst.x[i] = src.x[s]; dst.y[i] = src.y[s]; dst.z[i] = src.z[s]; dst.id[i] = src.id[s];
+}
+__global__ void __launch_bounds__(kTPB)
+k_tree_copy(SoA src, SoA dst, const Ctrl* __restrict__ ctrl) {
+  const uint32_t n = ctrl->n_active;
+  const uint32_t i = blockIdx.x * kTPB + threadIdx.x;
+  if (i >= n) return;
+  dst.x[i] = src.x[i]; dst.y[i] = src.y[i]; dst.z[i] = src.z[i]; dst.id[i] = src.id[i];
+}
+
+// ---- nodes -------------------------------------------------------------------------------------------------------
+// Level 0: one warp per leaf (32 consecutive carriers): m, centre of charge, radius of the members about it.
+__global__ void __launch_bounds__(kTPB)
+k_tree_leaves(const float* __restrict__ px, const float* __restrict__ py, const float* __restrict__ pz,
+              const Ctrl* __restrict__ ctrl, float4* __restrict__ node_c, float* __restrict__ node_r) {
+  const uint32_t n = ctrl->n_active;
+  const uint32_t leaf = (blockIdx.x * kTPB + threadIdx.x) >> 5, lane = threadIdx.x & 31u;
+  if (leaf >= nodes_at(n, 0)) return;
+  const uint32_t i = leaf * kLeaf + lane;
+  const bool ok = i < n;
+  const uint32_t i0 = leaf * kLeaf;
+  const float x0 = px[i0], y0 = py[i0], z0 = pz[i0];                 // sums relative to the first member: no cancellation
+  const float dx = ok ? px[i] - x0 : 0.f, dy = ok ? py[i] - y0 : 0.f, dz = ok ? pz[i] - z0 : 0.f;
+  float sx = dx, sy = dy, sz = dz;
+  for (int o = 16; o > 0; o >>= 1) {
+    sx += __shfl_xor_sync(0xffffffffu, sx, o); sy += __shfl_xor_sync(0xffffffffu, sy, o); sz += __shfl_xor_sync(0xffffffffu, sz, o);
+  }
+  const uint32_t m = min(kLeaf, n - i0);
+  const float inv = 1.0f / (float)m;
+  const float cx = sx * inv, cy = sy * inv, cz = sz * inv;           // relative to (x0,y0,z0)
+  float r2 = ok ? (dx - cx) * (dx - cx) + (dy - cy) * (dy - cy) + (dz - cz) * (dz - cz) : 0.f;
+  for (int o = 16; o > 0; o >>= 1) r2 = fmaxf(r2, __shfl_xor_sync(0xffffffffu, r2, o));
+  if (lane == 0) {
+    node_c[leaf] = make_float4(x0 + cx, y0 + cy, z0 + cz, (float)m);
+    // the stored centre is rounded to FP32 (<= 1 ulp per coordinate): widen the radius accordingly
+    node_r[leaf] = sqrtf(r2) * 1.000001f + 2e-7f * (fabsf(x0) + fabsf(y0) + fabsf(z0));
+  }
+}
+
+// Levels >= 1, straight from the leaves: one CTA per node; centre = count-weighted mean of its leaves' centres (FP64),
+// radius = max over leaves of |c_leaf - c| + r_leaf (a valid, slightly generous ball).
+__global__ void __launch_bounds__(kTPB)
+k_tree_upper(const Ctrl* __restrict__ ctrl, float4* __restrict__ node_c, float* __restrict__ node_r) {
+  __shared__ double s_s[4][kTPB / 32];
+  __shared__ float s_r[kTPB / 32];
+  __shared__ float s_c[3];
+  const uint32_t n = ctrl->n_active;
+  // which (level, k) is this CTA?
+  uint32_t b = blockIdx.x, l = 1;
+  for (;; ++l) {
+    if (l >= kTreeMaxLevels) return;
+    const uint32_t c = nodes_at(n, l);
+    if (b < c) break;
+    b -= c;
+    if (c <= 1) return;                                      // past the root
+  }
+  const uint32_t per = 1u << (3u * l);                       // leaves per node at this level
+  const uint32_t n_leaves = nodes_at(n, 0);
+  const uint32_t f0 = b * per, f1 = min(f0 + per, n_leaves);
+  const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+  const float4 ref = node_c[f0];
+  double sx = 0, sy = 0, sz = 0, sm = 0;
+  for (uint32_t f = f0 + tid; f < f1; f += kTPB) {
+    const float4 c = node_c[f];
+    sx += (double)c.w * (double)(c.x - ref.x); sy += (double)c.w * (double)(c.y - ref.y); sz += (double)c.w * (double)(c.z - ref.z);
+    sm += (double)c.w;
+  }
+  for (int o = 16; o > 0; o >>= 1) {
+    sx += __shfl_xor_sync(0xffffffffu, sx, o); sy += __shfl_xor_sync(0xffffffffu, sy, o);
+    sz += __shfl_xor_sync(0xffffffffu, sz, o); sm += __shfl_xor_sync(0xffffffffu, sm, o);
+  }
+  if (lane == 0) { s_s[0][warp] = sx; s_s[1][warp] = sy; s_s[2][warp] = sz; s_s[3][warp] = sm; }
+  __syncthreads();
+  if (tid == 0) {
+    double a = 0, bb = 0, c = 0, m = 0;
+    for (int w = 0; w < kTPB / 32; ++w) { a += s_s[0][w]; bb += s_s[1][w]; c += s_s[2][w]; m += s_s[3][w]; }
+    s_c[0] = (float)((double)ref.x + a / m); s_c[1] = (float)((double)ref.y + bb / m); s_c[2] = (float)((double)ref.z + c / m);
+    s_s[3][0] = m;
+  }
+  __syncthreads();
+  const float cx = s_c[0], cy = s_c[1], cz = s_c[2];
+  float r = 0.f;
+  for (uint32_t f = f0 + tid; f < f1; f += kTPB) {
+    const float4 c = node_c[f];
+    const float dx = c.x - cx, dy = c.y - cy, dz = c.z - cz;
+    r = fmaxf(r, sqrtf(dx * dx + dy * dy + dz * dz) * 1.000001f + node_r[f]);
+  }
+  for (int o = 16; o > 0; o >>= 1) r = fmaxf(r, __shfl_xor_sync(0xffffffffu, r, o));
+  if (lane == 0) s_r[warp] = r;
+  __syncthreads();
+  if (tid == 0) {
+    for (int w = 1; w < kTPB / 32; ++w) r = fmaxf(r, s_r[w]);
+    const uint32_t idx = level_offset(n, l) + b;
+    node_c[idx] = make_float4(cx, cy, cz, (float)s_s[3][0]);
+    node_r[idx] = r + 2e-7f * (fabsf(cx) + fabsf(cy) + fabsf(cz));
+  }
+}
+
+// ---- traversal + evaluation ----------------------------------------------------------------------------------------
+// One source (hole, or pseudo-hole of charge m) against this thread's packed pair of targets: the inner loop of
+// gc_field.cuh with one more FMUL2 for the charge.
+template <bool WEIGHTED>
+__device__ __forceinline__ void interact_w(const float4 sxy, const float2 sz, const float2 sm, const float2 ntx, const float2 nty,
+                                           const float2 ntz, const float2 eps2v, float2& ax, float2& ay, float2& az) {
+  const float2 dx = __fadd2_rn(make_float2(sxy.x, sxy.y), ntx);
+  const float2 dy = __fadd2_rn(make_float2(sxy.z, sxy.w), nty);
+  const float2 dz = __fadd2_rn(sz, ntz);
+  float2 r2 = __ffma2_rn(dx, dx, eps2v);
+  r2 = __ffma2_rn(dy, dy, r2);
+  r2 = __ffma2_rn(dz, dz, r2);
+  const float2 inv = make_float2(rsqrt_ftz(r2.x), rsqrt_ftz(r2.y));
+  float2 w = __fmul2_rn(inv, inv);
+  w = __fmul2_rn(w, inv);
+  if (WEIGHTED) w = __fmul2_rn(w, sm);
+  ax = __ffma2_rn(dx, w, ax);
+  ay = __ffma2_rn(dy, w, ay);
+  az = __ffma2_rn(dz, w, az);
+}
+
+struct TreeShared {
+  float4 xy[256];
+  float2 z[256];
+  float2 m[256];
+  uint32_t far[kFarCap];
+  uint2 near[kNearCap];
+  uint32_t pref[kNearCap + 1];
+  uint32_t front[2][kFrontCap];
+  uint32_t wcnt[kTreeTPB / 32][3];
+  float4 tgt[kGroup];          // the group's targets (sentinel where the group is ragged)
+  float box8[8][6];            // boxes of 32 targets (lo xyz, hi xyz)
+  float box32[32][6];          // boxes of 8 targets
+  uint32_t n_far, n_near, n_front[2], group;
+};
+
+__device__ __forceinline__ float box_d2(const float (&b)[6], const float4 c) {
+  const float dx = fmaxf(fmaxf(b[0] - c.x, c.x - b[3]), 0.f), dy = fmaxf(fmaxf(b[1] - c.y, c.y - b[4]), 0.f),
+              dz = fmaxf(fmaxf(b[2] - c.z, c.z - b[5]), 0.f);
+  return dx * dx + dy * dy + dz * dz;
+}
+
+// True iff every target of the group is at least R = a / theta from the node's centre c (R < 0: never).
+__device__ __forceinline__ bool tree_accept(const TreeShared& S, const float4 c, const float R) {
+  if (!(R >= 0.f)) return false;
+  const float R2 = R * R * 1.000004f;                        // rounding of the distances below
+  for (int b = 0; b < 8; ++b) {
+    if (box_d2(S.box8[b], c) >= R2) continue;
+    for (int q = 4 * b; q < 4 * b + 4; ++q) {
+      if (box_d2(S.box32[q], c) >= R2) continue;
+      for (int t = 8 * q; t < 8 * q + 8; ++t) {
+        const float4 x = S.tgt[t];
+        const float dx = x.x - c.x, dy = x.y - c.y, dz = x.z - c.z;
+        if (dx * dx + dy * dy + dz * dz < R2) return false;
+      }
+    }
+  }
+  return true;
+}
+
+template <bool WEIGHTED>
+__device__ __forceinline__ void tree_eval_tile(const TreeShared& S, int len, const float2 ntx, const float2 nty, const float2 ntz,
+                                               const float2 eps2v, float2& tx, float2& ty, float2& tz) {
+  float2 ax = make_float2(0.f, 0.f), ay = ax, az = ax;
+#pragma unroll 4
+  for (int jj = 0; jj < len; ++jj) interact_w<WEIGHTED>(S.xy[jj], S.z[jj], S.m[jj], ntx, nty, ntz, eps2v, ax, ay, az);
+  tx = __fadd2_rn(tx, ax); ty = __fadd2_rn(ty, ay); tz = __fadd2_rn(tz, az);       // two-level accumulation
+}
+
+// Evaluation is split P ways: the P CTAs ("parts") working on one group build identical lists and each evaluates the
+// source tiles whose running number is congruent to its part; their partial sums go to P chunks that the integrator
+// adds in fixed order.  This keeps 148 SMs busy when there are few groups and breaks up the occasional heavy group.
+struct TileSplit { uint32_t no, P, part; };
+
+__device__ __forceinline__ void tree_flush_far(TreeShared& S, const Tree& T, TileSplit& ts, const float2 ntx, const float2 nty,
+                                               const float2 ntz, const float2 eps2v, float2& tx, float2& ty, float2& tz) {
+  const uint32_t tid = threadIdx.x;
+  const uint32_t nf = S.n_far;
+  for (uint32_t base = 0; base < nf; base += 256) {
+    if (ts.no++ % ts.P != ts.part) continue;
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const uint32_t slot = tid + h * kTreeTPB, q = base + slot;
+      float4 c = make_float4(kSentinel, kSentinel, kSentinel, 0.f);
+      if (q < nf) c = T.node_c[S.far[q]];
+      S.xy[slot] = make_float4(c.x, c.x, c.y, c.y); S.z[slot] = make_float2(c.z, c.z); S.m[slot] = make_float2(c.w, c.w);
+    }
+    __syncthreads();
+    const int len = (int)min(256u, (nf - base + 3u) & ~3u);
+    tree_eval_tile<true>(S, len, ntx, nty, ntz, eps2v, tx, ty, tz);
+    __syncthreads();
+  }
+  if (tid == 0) {
+    if (nf && ts.part == 0) atomicAdd(&T.tc->far_evals, (unsigned long long)nf * kGroup);
+    S.n_far = 0;
+  }
+  __syncthreads();
+}
+
+__device__ __forceinline__ void tree_flush_near(TreeShared& S, const Tree& T, TileSplit& ts, const float* __restrict__ px,
+                                                const float* __restrict__ py, const float* __restrict__ pz, const float2 ntx,
+                                                const float2 nty, const float2 ntz, const float2 eps2v, float2& tx, float2& ty,
+                                                float2& tz) {
+  const uint32_t tid = threadIdx.x, lane = tid & 31u;
+  const uint32_t nn = S.n_near;
+  if (tid < 32) {                                          // exclusive prefix of the range lengths, one warp
+    uint32_t run = 0;
+    for (uint32_t b = 0; b < nn; b += 32) {
+      const uint32_t v = b + lane < nn ? S.near[b + lane].y : 0u;
+      uint32_t inc = v;
+      for (int o = 1; o < 32; o <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= (uint32_t)o) inc += t; }
+      if (b + lane < nn) S.pref[b + lane] = run + inc - v;
+      run += __shfl_sync(0xffffffffu, inc, 31);
+    }
+    if (lane == 0) S.pref[nn] = run;
+  }
+  __syncthreads();
+  const uint32_t total = S.pref[nn];
+  for (uint32_t base = 0; base < total; base += 256) {
+    if (ts.no++ % ts.P != ts.part) continue;
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const uint32_t slot = tid + h * kTreeTPB, q = base + slot;
+      float x = kSentinel, y = kSentinel, z = kSentinel;
+      if (q < total) {
+        uint32_t lo = 0, hi = nn;                          // largest r with pref[r] <= q
+        while (hi - lo > 1) { const uint32_t mid = (lo + hi) >> 1; if (S.pref[mid] <= q) lo = mid; else hi = mid; }
+        const uint32_t i = S.near[lo].x + (q - S.pref[lo]);
+        x = px[i]; y = py[i]; z = pz[i];
+      }
+      S.xy[slot] = make_float4(x, x, y, y); S.z[slot] = make_float2(z, z);
+    }
+    __syncthreads();
+    const int len = (int)min(256u, (total - base + 3u) & ~3u);
+    tree_eval_tile<false>(S, len, ntx, nty, ntz, eps2v, tx, ty, tz);
+    __syncthreads();
+  }
+  if (tid == 0) {
+    if (total && ts.part == 0) atomicAdd(&T.tc->near_evals, (unsigned long long)total * kGroup);
+    S.n_near = 0;
+  }
+  __syncthreads();
+}
+
+// Field of every active carrier by the treecode; result in the first plan.S chunks of the partial planes, in the
+// same convention as k_field: sum over sources of (r_s - r_t) w.  Persistent grid, groups handed out dynamically (the
+// result of a group does not depend on which CTA computes it: list order and summation order are fixed).
+__global__ void __launch_bounds__(kTreeTPB, 6)
+k_tree_field(const float* __restrict__ px, const float* __restrict__ py, const float* __restrict__ pz,
+             const Ctrl* __restrict__ ctrl, Tree T, float* __restrict__ Ep, uint32_t part_cap, float eps2, float theta) {
+  __shared__ TreeShared S;
+  const uint32_t n = ctrl->n_active;
+  if (n == 0) return;
+  const uint32_t stride = ctrl->plan.stride;
+  const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+  const uint32_t n_groups = (n + kGroup - 1) / kGroup;
+  const uint32_t P = max(ctrl->plan.S, 1u);                  // parts per group = partial chunks (set by the planner)
+  uint32_t cnt[kTreeMaxLevels], off[kTreeMaxLevels];
+  uint32_t ltop = 0;
+  {
+    uint32_t o = 0;
+    bool found = false;
+#pragma unroll
+    for (uint32_t l = 0; l < kTreeMaxLevels; ++l) {
+      cnt[l] = nodes_at(n, l); off[l] = o; o += cnt[l];
+      if (!found && cnt[l] <= kTopNodes) { ltop = l; found = true; }
+    }
+  }
+  const float2 eps2v = make_float2(eps2, eps2);
+  constexpr uint32_t kInvalid = 0xffffffffu;
+
+  for (;;) {
+    if (tid == 0) S.group = atomicAdd(&T.tc->next_group, 1u);
+    __syncthreads();
+    const uint32_t item = S.group;
+    if (item >= n_groups * P) break;
+    const uint32_t g = item / P;
+    TileSplit ts = {0u, P, item - g * P};
+    // this thread's packed pair of targets, negated
+    const uint32_t i0 = g * kGroup + 2u * tid;
+    float2 vx = make_float2(0.f, 0.f), vy = vx, vz = vx;
+    if (i0 + 1 < n) {
+      vx = *reinterpret_cast<const float2*>(px + i0); vy = *reinterpret_cast<const float2*>(py + i0);
+      vz = *reinterpret_cast<const float2*>(pz + i0);
+    } else if (i0 < n) { vx.x = px[i0]; vy.x = py[i0]; vz.x = pz[i0]; }
+    const float2 ntx = make_float2(-vx.x, -vx.y), nty = make_float2(-vy.x, -vy.y), ntz = make_float2(-vz.x, -vz.y);
+    float2 tx = make_float2(0.f, 0.f), ty = tx, tz = tx;
+    // Acceptance needs  a <= theta |x_t - c|  for EVERY target t of the group.  It is decided exactly, through a
+    // small hierarchy over the group's own targets: 8 boxes of 32 targets, 32 boxes of 8, then the targets themselves
+    // (tree_accept).  A single box (or ball) about the group would not do: where the occupancy is sparse the curve
+    // leaves the cloud and re-enters it elsewhere, a run of 256 holes is then two distant pieces, and everything in
+    // between would be swallowed into its exact near field.
+    {
+      const bool v0 = i0 < n, v1 = i0 + 1 < n;
+      S.tgt[2 * tid] = v0 ? make_float4(vx.x, vy.x, vz.x, 0.f) : make_float4(kSentinel, kSentinel, kSentinel, 0.f);
+      S.tgt[2 * tid + 1] = v1 ? make_float4(vx.y, vy.y, vz.y, 0.f) : make_float4(kSentinel, kSentinel, kSentinel, 0.f);
+      float lo[3] = {v0 ? vx.x : 3e18f, v0 ? vy.x : 3e18f, v0 ? vz.x : 3e18f};
+      float hi[3] = {v0 ? vx.x : -3e18f, v0 ? vy.x : -3e18f, v0 ? vz.x : -3e18f};
+      if (v1) {
+        lo[0] = fminf(lo[0], vx.y); lo[1] = fminf(lo[1], vy.y); lo[2] = fminf(lo[2], vz.y);
+        hi[0] = fmaxf(hi[0], vx.y); hi[1] = fmaxf(hi[1], vy.y); hi[2] = fmaxf(hi[2], vz.y);
+      }
+#pragma unroll
+      for (int o = 1; o <= 8; o <<= 1) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+          lo[c] = fminf(lo[c], __shfl_xor_sync(0xffffffffu, lo[c], o)); hi[c] = fmaxf(hi[c], __shfl_xor_sync(0xffffffffu, hi[c], o));
+        }
+        if (o == 2 && (lane & 3u) == 0) {                    // 4 lanes = 8 targets
+#pragma unroll
+          for (int c = 0; c < 3; ++c) { S.box32[tid >> 2][c] = lo[c]; S.box32[tid >> 2][3 + c] = hi[c]; }
+        }
+      }
+      if ((lane & 15u) == 0) {                               // 16 lanes = 32 targets
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { S.box8[tid >> 4][c] = lo[c]; S.box8[tid >> 4][3 + c] = hi[c]; }
+      }
+    }
+    if (tid == 0) { S.n_far = 0; S.n_near = 0; S.n_front[0] = 0; S.n_front[1] = 0; }
+    __syncthreads();
+    // Level-by-level walk.  A frontier holds the OPENED nodes of the level above (one entry each); their children
+    // k = 8 p + c are the candidates of this level.  At the top level the candidates are all its nodes.
+    int cur = 0;
+    for (uint32_t l = ltop;; --l) {
+      const uint32_t n_cand = l == ltop ? cnt[ltop] : S.n_front[cur] * kFan;
+      const uint32_t lsize = level_size(l);
+      for (uint32_t base = 0; base < n_cand; base += kTreeTPB) {
+        if (S.n_far + kTreeTPB > kFarCap) tree_flush_far(S, T, ts, ntx, nty, ntz, eps2v, tx, ty, tz);
+        if (S.n_near + kTreeTPB > kNearCap) tree_flush_near(S, T, ts, px, py, pz, ntx, nty, ntz, eps2v, tx, ty, tz);
+        const bool room = l > 0 && S.n_front[cur ^ 1] + kTreeTPB <= kFrontCap;
+        const uint32_t q = base + tid;
+        uint32_t k = kInvalid;
+        if (q < n_cand) {
+          k = l == ltop ? q : S.front[cur][q >> 3] * kFan + (q & 7u);
+          if (k >= cnt[l]) k = kInvalid;
+        }
+        int cat = 0;                                        // 1 far, 2 near (exact), 3 open
+        if (k != kInvalid) {
+          const float4 c = T.node_c[off[l] + k];
+          const float r = T.node_r[off[l] + k];
+          if (tree_accept(S, c, theta > 0.f ? r / theta : -1.f)) cat = 1;
+          else cat = room ? 3 : 2;                          // no room to open: sum the whole node exactly (always valid)
+        }
+        const uint32_t b1 = __ballot_sync(0xffffffffu, cat == 1), b2 = __ballot_sync(0xffffffffu, cat == 2),
+                       b3 = __ballot_sync(0xffffffffu, cat == 3);
+        if (lane == 0) { S.wcnt[warp][0] = __popc(b1); S.wcnt[warp][1] = __popc(b2); S.wcnt[warp][2] = __popc(b3); }
+        __syncthreads();
+        uint32_t o1 = S.n_far, o2 = S.n_near, o3 = S.n_front[cur ^ 1];
+        for (uint32_t w = 0; w < warp; ++w) { o1 += S.wcnt[w][0]; o2 += S.wcnt[w][1]; o3 += S.wcnt[w][2]; }
+        const uint32_t lt = (1u << lane) - 1u;
+        if (cat == 1) S.far[o1 + __popc(b1 & lt)] = off[l] + k;
+        else if (cat == 2) {
+          const uint32_t start = k * lsize;
+          S.near[o2 + __popc(b2 & lt)] = make_uint2(start, min(lsize, n - start));
+        } else if (cat == 3) S.front[cur ^ 1][o3 + __popc(b3 & lt)] = k;
+        __syncthreads();
+        if (tid == 0) {
+          uint32_t a = 0, b = 0, c = 0;
+          for (int w = 0; w < kTreeTPB / 32; ++w) { a += S.wcnt[w][0]; b += S.wcnt[w][1]; c += S.wcnt[w][2]; }
+          S.n_far += a; S.n_near += b; S.n_front[cur ^ 1] += c;
+        }
+        __syncthreads();
+      }
+      if (l == 0) break;
+      if (tid == 0) S.n_front[cur] = 0;
+      cur ^= 1;
+      __syncthreads();
+    }
+    tree_flush_far(S, T, ts, ntx, nty, ntz, eps2v, tx, ty, tz);
+    tree_flush_near(S, T, ts, px, py, pz, ntx, nty, ntz, eps2v, tx, ty, tz);
+
+    if (i0 < stride) {
+      float* e = Ep + (size_t)ts.part * stride + i0;
+      *reinterpret_cast<float2*>(e) = tx;
+      *reinterpret_cast<float2*>(e + part_cap) = ty;
+      *reinterpret_cast<float2*>(e + 2 * (size_t)part_cap) = tz;
+    }
+  }
+}
+
+}  // namespace gc

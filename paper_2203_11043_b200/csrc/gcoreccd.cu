@@ -18,6 +18,7 @@
 #include "gc_frontend.cuh"
 #include "gc_integrate.cuh"
 #include "gc_shard.cuh"
+#include "gc_tree.cuh"
 
 using namespace gc;
 
@@ -80,6 +81,12 @@ struct gcoreccd {
   uint32_t graph_tiles;
   cudaEvent_t ev[4];
   uint32_t shard_rank, shard_world;   // target sharding (gc_shard.cuh); world 1 = not sharded
+  bool ff_on;                         // far-field approximation (gc_tree.cuh)
+  float ff_theta;
+  uint32_t ff_parts;                  // CTAs (= partial chunks) per group of 256 targets
+  uint32_t ff_resort, ff_age;         // re-sort cadence; field evaluations since the last Hilbert sort
+  int grid_tree;
+  Tree tree;
   char err[256];
   // batched independent events (gc_events.cuh)
   struct {
@@ -138,6 +145,7 @@ inline PlanArgs plan_args(const gcoreccd_t* h, int v) {
   a.part_cap_entries = (uint32_t)h->L.part_cap;
   a.rank = h->shard_rank;
   a.world = h->shard_world;
+  a.force_S = h->ff_on ? h->ff_parts : 0u;
   return a;
 }
 
@@ -149,7 +157,43 @@ inline uint32_t bucket_tiles(uint32_t t) {                  // power-of-two buck
   return b;
 }
 
+// Far-field variant (gc_tree.cuh): [Hilbert re-sort of the state every ff_resort evaluations] + nodes + walk/evaluate.
+int launch_tree_field(gcoreccd_t* h) {
+  const uint64_t nb = h->n_bound ? h->n_bound : 1;
+  const uint32_t tiles = tiles_for(nb);
+  const Tree& T = h->tree;
+  const bool sort = h->ff_age % h->ff_resort == 0;
+  h->ff_age += 1;
+  k_tree_reset<<<1, 32, 0, h->stream>>>(T.tc, sort ? 1 : 0);
+  h->launches += 1;
+  if (sort) {
+    k_tree_bbox<<<std::min<uint32_t>(tiles, (uint32_t)h->num_sms * 4u), kTPB, 0, h->stream>>>(h->A.x, h->A.y, h->A.z, h->ctrl, T.tc);
+    k_tree_keys<<<tiles, kTPB, 0, h->stream>>>(h->A.x, h->A.y, h->A.z, h->ctrl, T.tc, T.key[0], T.val[0]);
+    const uint32_t sb = (uint32_t)((nb + kSortBlock - 1) / kSortBlock);
+    int cur = 0;
+    for (uint32_t shift = 0; shift < 8 * kKeyPasses; shift += 8) {
+      k_radix_hist<<<sb, 256, 0, h->stream>>>(T.key[cur], h->ctrl, shift, T.counts);
+      k_radix_scan<<<1, 1024, 0, h->stream>>>(h->ctrl, T.counts);
+      k_radix_scatter<<<sb, 256, 0, h->stream>>>(T.key[cur], T.val[cur], T.key[cur ^ 1], T.val[cur ^ 1], h->ctrl, shift, T.counts);
+      cur ^= 1;
+    }
+    k_tree_permute<<<tiles, kTPB, 0, h->stream>>>(h->A, h->B, T.val[cur], h->ctrl);     // state B is scratch between steps
+    k_tree_copy<<<tiles, kTPB, 0, h->stream>>>(h->B, h->A, h->ctrl);
+    h->launches += 4 + 3 * kKeyPasses;
+  }
+  const uint32_t leaves = nodes_at((uint32_t)nb, 0);
+  k_tree_leaves<<<(leaves + 7) / 8, kTPB, 0, h->stream>>>(h->A.x, h->A.y, h->A.z, h->ctrl, T.node_c, T.node_r);
+  uint32_t upper = 0;
+  for (uint32_t l = 1; l < kTreeMaxLevels; ++l) { const uint32_t c = nodes_at((uint32_t)nb, l); upper += c; if (c <= 1) break; }
+  k_tree_upper<<<upper, kTPB, 0, h->stream>>>(h->ctrl, T.node_c, T.node_r);
+  k_tree_field<<<h->grid_tree, kTreeTPB, 0, h->stream>>>(h->A.x, h->A.y, h->A.z, h->ctrl, T, h->Ep, (uint32_t)h->L.part_cap,
+                                                         h->dp.eps2, h->ff_theta);
+  h->launches += 3;
+  return 0;
+}
+
 int launch_field(gcoreccd_t* h, int v) {
+  if (h->ff_on) return launch_tree_field(h);
   const int g = h->grid_field[v];
   const uint32_t pc = (uint32_t)h->L.part_cap;
   switch (v) {
@@ -172,9 +216,19 @@ void enqueue_step(gcoreccd_t* h, uint32_t tiles) {
   h->launches += 2;
 }
 
+// parts per treecode group: enough work items for ~4 per resident CTA, power of two, at most 8 (workspace layout)
+inline uint32_t pick_parts(const gcoreccd_t* h) {
+  const uint64_t groups = (h->n_bound + kGroup - 1) / kGroup;
+  uint32_t P = 1;
+  while (P < 8 && groups * P < 4ull * (uint64_t)h->grid_tree) P <<= 1;
+  return P;
+}
+
 int ensure_variant(gcoreccd_t* h) {
   const int v = pick_variant(h->n_bound);
-  if (v != h->variant) {
+  const uint32_t parts = h->ff_on ? pick_parts(h) : 0u;
+  if (v != h->variant || parts != h->ff_parts) {
+    h->ff_parts = parts;
     h->variant = v;
     k_replan<<<1, 32, 0, h->stream>>>(h->ctrl, plan_args(h, v), 0, 0u, 0, 0ull);
     h->launches += 1;
@@ -232,7 +286,8 @@ int enqueue_steps(gcoreccd_t* h, uint64_t n_steps) {
   }
   const uint32_t per_step = (h->dp.flags & GCORECCD_COULOMB_OFF) ? 2u : 3u;
   // stream capture is not permitted on the legacy / per-thread default streams: plain launches there
-  const bool can_graph = h->stream != cudaStreamLegacy && h->stream != cudaStreamPerThread && h->stream != nullptr;
+  // (the treecode's re-sort cadence is host-scheduled: plain launches there too)
+  const bool can_graph = h->stream != cudaStreamLegacy && h->stream != cudaStreamPerThread && h->stream != nullptr && !h->ff_on;
   while (can_graph && n_steps >= (uint64_t)kGraphSteps) {
     rc = ensure_graph(h, tiles);
     if (rc) return rc;
@@ -366,6 +421,22 @@ int gcoreccd_create(const gcoreccd_params* p, gcoreccd_t** out) {
   if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[2], k_field<4, 256, 1>, kTPB, 0);
   if (e != cudaSuccess) { fail(h, GCORECCD_ERR_CUDA, "occupancy query", e); gcoreccd_destroy(h); return GCORECCD_ERR_CUDA; }
   for (int v = 0; v < kNumVariants; ++v) h->grid_field[v] = h->num_sms * (occ[v] > 0 ? occ[v] : 1);
+  int occ_tree = 0;
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_tree, k_tree_field, kTreeTPB, 0);
+  if (e != cudaSuccess) { fail(h, GCORECCD_ERR_CUDA, "occupancy query", e); gcoreccd_destroy(h); return GCORECCD_ERR_CUDA; }
+  h->grid_tree = h->num_sms * (occ_tree > 0 ? occ_tree : 1);
+  {
+    // treecode scratch: the last 8 cap_pad floats of partial plane 0 (free while S = 1; the load paths stage at its start)
+    float* r = h->Ep + (h->L.part_cap - 8 * cp);
+    Tree& T = h->tree;
+    T.tc = (TreeCtrl*)r;                         r += 64;
+    T.node_c = (float4*)r;                       r += cp / 4 + 64;          // <= cp/28 + 9 nodes of 4 floats
+    T.node_r = r;                                r += cp / 16 + 64;
+    T.key[0] = (unsigned long long*)r; r += 2 * cp;  T.key[1] = (unsigned long long*)r; r += 2 * cp;
+    T.val[0] = (uint32_t*)r; r += cp;  T.val[1] = (uint32_t*)r; r += cp;
+    T.counts = (uint32_t*)r;                                                // 256 * cp / 2048 = cp / 8 entries
+  }
+  h->ff_resort = 8;
 
   rc = gcoreccd_reset(h);
   if (rc != GCORECCD_OK) { gcoreccd_destroy(h); return rc; }
@@ -641,6 +712,7 @@ int gcoreccd_set_shard(gcoreccd_t* h, uint32_t rank, uint32_t world) {
   if (world > 1 && (h->dp.flags & GCORECCD_COULOMB_OFF))
     return fail(h, GCORECCD_ERR_INVALID, "set_shard: without eq. 6 carriers are independent; run replicas instead");
   if (h->n_loaded != 0 || h->evb.loaded) return fail(h, GCORECCD_ERR_STATE, "set_shard: only on an empty handle (reset first)");
+  if (world > 1 && h->ff_on) return fail(h, GCORECCD_ERR_STATE, "set_shard: the far-field variant is on");
   h->shard_rank = rank;
   h->shard_world = world;
   h->variant = -1;
@@ -693,6 +765,37 @@ int gcoreccd_shard_commit(gcoreccd_t* h, const void* const* msgs_host, uint32_t 
   k_shard_commit<<<tiles * n_msgs, kTPB, 0, h->stream>>>(ptrs, n_msgs, (uint32_t)bs, h->A, h->ctrl, plan_args(h, h->variant));
   h->launches += 1;
   GC_CUDA(h, cudaGetLastError());
+  return GCORECCD_OK;
+}
+
+// ---- far-field variant (gc_tree.cuh) ---------------------------------------------------------------------------
+int gcoreccd_set_farfield(gcoreccd_t* h, double theta, uint32_t resort_every) {
+  if (!h || !(theta < 1.0)) return GCORECCD_ERR_INVALID;
+  if (theta >= 0.0 && h->shard_world > 1) return fail(h, GCORECCD_ERR_STATE, "set_farfield: the handle is sharded");
+  if (theta >= 0.0 && h->L.cap_pad > (1ull << 26)) return fail(h, GCORECCD_ERR_CAPACITY, "set_farfield: capacity");
+  DeviceGuard guard(h->device);
+  GC_CUDA(h, cudaStreamSynchronize(h->stream));
+  drop_graph(h);
+  h->ff_on = theta >= 0.0;
+  h->ff_theta = (float)(theta >= 0.0 ? theta : 0.0);
+  h->ff_resort = resort_every ? resort_every : 8u;
+  h->ff_age = 0;
+  h->variant = -1;                                           // re-plan: the treecode writes one chunk (S = 1)
+  if (h->ff_on) GC_CUDA(h, cudaMemsetAsync(h->tree.tc, 0, sizeof(TreeCtrl), h->stream));
+  return GCORECCD_OK;
+}
+
+int gcoreccd_farfield_stats(gcoreccd_t* h, uint64_t* far_evals, uint64_t* near_evals, double* bound_B) {
+  if (!h) return GCORECCD_ERR_INVALID;
+  if (!h->ff_on) return fail(h, GCORECCD_ERR_STATE, "farfield_stats: the far-field variant is off");
+  DeviceGuard guard(h->device);
+  TreeCtrl tc;
+  GC_CUDA(h, cudaMemcpyAsync(&tc, h->tree.tc, sizeof(tc), cudaMemcpyDeviceToHost, h->stream));
+  GC_CUDA(h, cudaStreamSynchronize(h->stream));
+  if (far_evals) *far_evals = tc.far_evals;
+  if (near_evals) *near_evals = tc.near_evals;
+  const double t = h->ff_theta;
+  if (bound_B) *bound_B = t * t * (3.0 - 2.0 * t) / ((1.0 - t) * (1.0 - t));
   return GCORECCD_OK;
 }
 
