@@ -228,7 +228,7 @@ int gcoreccd_shard_commit(gcoreccd_t* h, const void* const* msgs_host, uint32_t 
 
 /* ---- Far-field approximation of eq. 6 — a VARIANT, off by default --------------------------
  * The exact path sums all N_a^2 ordered pairs.  With set_farfield(theta >= 0) step a1 is replaced by
- * a treecode: the active holes are kept in Hilbert-curve order (re-sorted every resort_every field evaluations; 0 => 8), an
+ * a treecode: the active holes are kept in Hilbert-curve order (re-sorted every resort_every field evaluations; 0 => 4), an
  * implicit 8-ary tree of runs of 32*8^l consecutive holes carries, per node, its hole count m, centre of charge c and
  * bounding radius a; every group of 256 consecutive targets (ball (c_T, r_T)) replaces a node by ONE pseudo-hole of
  * charge m at c when  a <= theta * (|c - c_T| - r_T)  and sums all other holes exactly.  a2..a8 are unchanged.
@@ -240,9 +240,11 @@ int gcoreccd_shard_commit(gcoreccd_t* h, const void* const* msgs_host, uint32_t 
  * match by id); pair_interactions still counts N_a^2 per step (the pairs REPRESENTED) — the interactions actually
  * evaluated are in farfield_stats and no throughput claim of the exact metric may use this variant.
  * set_farfield: theta in [0, 1) switches the variant on, theta < 0 off; STATE on a sharded handle.  Synchronises.
+ *   While fewer than min_active holes are drifting (0 => 24,576; 1 => never) the all-pairs kernel is used instead:
+ *   below a few 1e4 holes it is the faster of the two (measured), and it is exact.
  * farfield_stats: interactions evaluated since set_farfield — pseudo-hole (far) and exact (near), each counted per
  *   target — and B(theta).  Host pointers, any may be NULL.  STATE if the variant is off. */
-int gcoreccd_set_farfield(gcoreccd_t* h, double theta, uint32_t resort_every);
+int gcoreccd_set_farfield(gcoreccd_t* h, double theta, uint32_t resort_every, uint64_t min_active);
 int gcoreccd_farfield_stats(gcoreccd_t* h, uint64_t* far_evals, uint64_t* near_evals, double* bound_B);
 
 /* Run ONE step with CUDA events between its kernels (on the handle's stream) and return the device time of

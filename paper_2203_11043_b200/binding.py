@@ -116,7 +116,7 @@ def lib():
     L.gcoreccd_shard_commit.restype = C.c_int
     L.gcoreccd_shard_commit.argtypes = [vp, C.POINTER(vp), C.c_uint32, C.c_uint64]
     L.gcoreccd_set_farfield.restype = C.c_int
-    L.gcoreccd_set_farfield.argtypes = [vp, C.c_double, C.c_uint32]
+    L.gcoreccd_set_farfield.argtypes = [vp, C.c_double, C.c_uint32, C.c_uint64]
     L.gcoreccd_farfield_stats.restype = C.c_int
     L.gcoreccd_farfield_stats.argtypes = [vp, u64p, u64p, C.POINTER(C.c_double)]
     L.gcoreccd_profile_step.restype = C.c_int
@@ -389,8 +389,8 @@ class Gcoreccd:
         return E
 
     # ---- far-field variant (include/gcoreccd.h "Far-field approximation")
-    def set_farfield(self, theta, resort_every=0):
-        self._check(lib().gcoreccd_set_farfield(self._h, float(theta), int(resort_every)), "set_farfield")
+    def set_farfield(self, theta, resort_every=0, min_active=0):
+        self._check(lib().gcoreccd_set_farfield(self._h, float(theta), int(resort_every), int(min_active)), "set_farfield")
 
     def farfield_stats(self):
         a, b, B = C.c_uint64(), C.c_uint64(), C.c_double()

@@ -83,7 +83,8 @@ struct gcoreccd {
   uint32_t shard_rank, shard_world;   // target sharding (gc_shard.cuh); world 1 = not sharded
   bool ff_on;                         // far-field approximation (gc_tree.cuh)
   float ff_theta;
-  uint32_t ff_parts;                  // CTAs (= partial chunks) per group of 256 targets
+  uint32_t ff_parts;                  // CTAs (= partial chunks) per group of 256 targets; 0 = all-pairs kernel in use
+  uint64_t ff_min_active;             // below this many active holes the all-pairs kernel is faster and is used
   uint32_t ff_resort, ff_age;         // re-sort cadence; field evaluations since the last Hilbert sort
   int grid_tree;
   Tree tree;
@@ -145,7 +146,7 @@ inline PlanArgs plan_args(const gcoreccd_t* h, int v) {
   a.part_cap_entries = (uint32_t)h->L.part_cap;
   a.rank = h->shard_rank;
   a.world = h->shard_world;
-  a.force_S = h->ff_on ? h->ff_parts : 0u;
+  a.force_S = h->ff_parts;
   return a;
 }
 
@@ -193,7 +194,7 @@ int launch_tree_field(gcoreccd_t* h) {
 }
 
 int launch_field(gcoreccd_t* h, int v) {
-  if (h->ff_on) return launch_tree_field(h);
+  if (h->ff_parts) return launch_tree_field(h);
   const int g = h->grid_field[v];
   const uint32_t pc = (uint32_t)h->L.part_cap;
   switch (v) {
@@ -226,7 +227,7 @@ inline uint32_t pick_parts(const gcoreccd_t* h) {
 
 int ensure_variant(gcoreccd_t* h) {
   const int v = pick_variant(h->n_bound);
-  const uint32_t parts = h->ff_on ? pick_parts(h) : 0u;
+  const uint32_t parts = h->ff_on && h->n_bound >= h->ff_min_active ? pick_parts(h) : 0u;
   if (v != h->variant || parts != h->ff_parts) {
     h->ff_parts = parts;
     h->variant = v;
@@ -287,7 +288,7 @@ int enqueue_steps(gcoreccd_t* h, uint64_t n_steps) {
   const uint32_t per_step = (h->dp.flags & GCORECCD_COULOMB_OFF) ? 2u : 3u;
   // stream capture is not permitted on the legacy / per-thread default streams: plain launches there
   // (the treecode's re-sort cadence is host-scheduled: plain launches there too)
-  const bool can_graph = h->stream != cudaStreamLegacy && h->stream != cudaStreamPerThread && h->stream != nullptr && !h->ff_on;
+  const bool can_graph = h->stream != cudaStreamLegacy && h->stream != cudaStreamPerThread && h->stream != nullptr && !h->ff_parts;
   while (can_graph && n_steps >= (uint64_t)kGraphSteps) {
     rc = ensure_graph(h, tiles);
     if (rc) return rc;
@@ -436,7 +437,8 @@ int gcoreccd_create(const gcoreccd_params* p, gcoreccd_t** out) {
     T.val[0] = (uint32_t*)r; r += cp;  T.val[1] = (uint32_t*)r; r += cp;
     T.counts = (uint32_t*)r;                                                // 256 * cp / 2048 = cp / 8 entries
   }
-  h->ff_resort = 8;
+  h->ff_resort = 4;
+  h->ff_min_active = 24576;
 
   rc = gcoreccd_reset(h);
   if (rc != GCORECCD_OK) { gcoreccd_destroy(h); return rc; }
@@ -769,7 +771,7 @@ int gcoreccd_shard_commit(gcoreccd_t* h, const void* const* msgs_host, uint32_t 
 }
 
 // ---- far-field variant (gc_tree.cuh) ---------------------------------------------------------------------------
-int gcoreccd_set_farfield(gcoreccd_t* h, double theta, uint32_t resort_every) {
+int gcoreccd_set_farfield(gcoreccd_t* h, double theta, uint32_t resort_every, uint64_t min_active) {
   if (!h || !(theta < 1.0)) return GCORECCD_ERR_INVALID;
   if (theta >= 0.0 && h->shard_world > 1) return fail(h, GCORECCD_ERR_STATE, "set_farfield: the handle is sharded");
   if (theta >= 0.0 && h->L.cap_pad > (1ull << 26)) return fail(h, GCORECCD_ERR_CAPACITY, "set_farfield: capacity");
@@ -778,7 +780,9 @@ int gcoreccd_set_farfield(gcoreccd_t* h, double theta, uint32_t resort_every) {
   drop_graph(h);
   h->ff_on = theta >= 0.0;
   h->ff_theta = (float)(theta >= 0.0 ? theta : 0.0);
-  h->ff_resort = resort_every ? resort_every : 8u;
+  h->ff_resort = resort_every ? resort_every : 4u;
+  h->ff_min_active = min_active ? min_active : 24576u;
+  h->ff_parts = 0;
   h->ff_age = 0;
   h->variant = -1;                                           // re-plan: the treecode writes one chunk (S = 1)
   if (h->ff_on) GC_CUDA(h, cudaMemsetAsync(h->tree.tc, 0, sizeof(TreeCtrl), h->stream));

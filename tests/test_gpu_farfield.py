@@ -37,7 +37,7 @@ def test_theta_zero_is_the_exact_field(cfg, n):
     w = workloads.make(cfg, n=n)
     sim = gpu_sim(w)
     sim.load_carriers(w["xyz"])
-    sim.set_farfield(0.0)
+    sim.set_farfield(0.0, 0, 1)                        # min_active = 1: the treecode at every size
     E = sim.eval_field()
     xyz, ids = sim.read_carriers()                       # current (curve) order, the order E is in
     loaded = w["xyz"][w["xyz"][:, 2] > 0]
@@ -61,7 +61,7 @@ def test_error_stays_inside_the_stated_bound(cfg, n, theta):
     Kp = g.coulomb_constant(P["eps_si"])
     sim = gpu_sim(w)
     sim.load_carriers(w["xyz"])
-    sim.set_farfield(theta)
+    sim.set_farfield(theta, 0, 1)
     E = sim.eval_field()
     xyz, _ = sim.read_carriers()
     st = sim.farfield_stats()
@@ -89,7 +89,7 @@ def test_theta_zero_trajectories_match_the_oracle_and_runs_are_deterministic():
     for _ in range(2):
         sim = gpu_sim(w)
         sim.load_carriers(w["xyz"])
-        sim.set_farfield(0.0, 3)                          # re-sort every 3 steps
+        sim.set_farfield(0.0, 3, 1)                       # re-sort every 3 steps
         sim.step(10)
         xyz, ids = sim.read_carriers()
         out.append((xyz, ids, sim.state()))
@@ -114,7 +114,7 @@ def test_farfield_run_is_deterministic_and_conserves_on_a_decaying_track():
     for _ in range(2):
         sim = gpu_sim(w)
         sim.load_carriers(w["xyz"])
-        sim.set_farfield(0.4, 4)
+        sim.set_farfield(0.4, 4, 12000)                   # ... and the run ends on the all-pairs kernel
         for _ in range(5):
             sim.step(40)
             st = sim.state()
@@ -136,7 +136,7 @@ def test_farfield_full_run_reproduces_the_exact_paths_cloud_statistics():
         sim = gpu_sim(w)
         sim.load_carriers(w["xyz"])
         if theta >= 0:
-            sim.set_farfield(theta)
+            sim.set_farfield(theta, 0, 2000)
         done, left, _ = sim.run_to_collection()
         assert left == 0
         img, over = sim.read_image()
@@ -164,7 +164,7 @@ def test_farfield_api_errors_and_switching_back():
         sim.farfield_stats()                              # variant is off
     sim.load_carriers(w["xyz"])
     E0 = sim.eval_field()
-    sim.set_farfield(0.5)
+    sim.set_farfield(0.5, 0, 1)
     sim.eval_field()
     sim.set_farfield(-1.0)                                # back to all-pairs; the state stays in curve order
     E1 = sim.eval_field()
