@@ -117,6 +117,17 @@ def oracle_sample(xyz, P, seconds_target, rng):
     return m * n / dt / 1e9, m, dt, g.num_threads()
 
 
+def image_sigma(img, P):
+    """Standard deviations (um) of the collected image along x and y, from pixel centres."""
+    im = np.asarray(img, dtype=np.float64)
+    ny, nx = im.shape
+    xs = P["img_x0_um"] + (np.arange(nx) + 0.5) * P["pixel_pitch_um"]
+    ys = P["img_y0_um"] + (np.arange(ny) + 0.5) * P["pixel_pitch_um"]
+    tot = im.sum()
+    mx, my = (im.sum(axis=0) * xs).sum() / tot, (im.sum(axis=1) * ys).sum() / tot
+    return (np.sqrt((im.sum(axis=0) * (xs - mx) ** 2).sum() / tot), np.sqrt((im.sum(axis=1) * (ys - my) ** 2).sum() / tot))
+
+
 def run_reference(args):
     """--impl reference: the FP64 oracle as it stands, on the host cores, same metric/unit/config."""
     rank = int(os.environ.get("RANK", "0"))
@@ -261,6 +272,30 @@ def run_ours(args):
         event = {"seconds": ev_s, "steps": done, "pair_interactions": st2["pair_interactions"],
                  "avg_G_pairs_per_s": st2["pair_interactions"] / ev_s / 1e9, "holes": n, "collected_in_window": int(img.sum())}
 
+    # ---- far-field VARIANT (reported separately, never part of `value`): same event, treecode
+    farfield = None
+    if not args.no_event and rank == 0 and event is not None:
+        theta = 0.5
+        sim.reset()
+        sim.set_farfield(theta)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        sim.load_carriers_ptr(host_in.data_ptr(), n)
+        done_f, left_f, rc = sim.run_to_collection(10 ** 7)
+        img_f, over_f = sim.read_image()
+        torch.cuda.synchronize()
+        ff_s = time.perf_counter() - t0
+        stf, ffs = sim.state(), sim.farfield_stats()
+        assert left_f == 0 and int(img_f.sum()) + over_f == n, "hole count not conserved (far-field)"
+        mom = lambda im: [float(v) for v in image_sigma(im, P)]
+        farfield = {"theta": theta, "bound_B": ffs["bound_B"], "seconds": ff_s, "steps": done_f,
+                    "interactions_evaluated": ffs["far_evals"] + ffs["near_evals"],
+                    "fraction_of_all_pairs": (ffs["far_evals"] + ffs["near_evals"]) / float(stf["pair_interactions"]),
+                    "speedup_vs_exact_event": event["seconds"] / ff_s,
+                    "image_sigma_xy_um": mom(img_f), "exact_image_sigma_xy_um": mom(img),
+                    "note": "approximate variant (treecode, monopole about the centre of charge); not the exact O(N^2) metric"}
+        sim.set_farfield(-1.0)
+
     # ---- batched independent events (secondary numbers, not the headline): one CTA per event
     batched = None
     if not args.no_event and rank == 0:
@@ -315,7 +350,8 @@ def run_ours(args):
             "clocks": clocks, "gpu_launches": launches,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": n * 12, "d2h_bytes_per_step": n * 12,
                     "what": "reset + load_carriers(pinned host) + step(1) + read_carriers(host), wall clock"},
-            "roofline": roofline, "cpu_baseline": cpu, "seconds_per_event": event, "batched_events": batched}
+            "roofline": roofline, "cpu_baseline": cpu, "seconds_per_event": event, "farfield_variant": farfield,
+            "batched_events": batched}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

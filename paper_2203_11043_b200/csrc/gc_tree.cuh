@@ -4,15 +4,15 @@
 // Method (a GPU treecode over an implicit tree; nothing of it is in the paper, whose kernel is all-pairs):
 //   1. every `resort` steps the active carriers are reordered along a 48-bit Hilbert curve of their bounding box
 //      (LSD radix sort written here: block histograms, one scan, stable warp-match scatter; no Thrust/CUB);
-//   2. every step an implicit 8-ary tree is laid over that order: the level-l node k is the run of 32*8^l consecutive
-//      carriers starting at k*32*8^l; a node stores its hole count m, its centre of charge c (the dipole about c
+//   2. every step an implicit 8-ary tree is laid over that order: the level-l node k is the run of 8*8^l consecutive
+//      carriers starting at k*8*8^l; a node stores its hole count m, its centre of charge c (the dipole about c
 //      vanishes) and the radius a of the smallest ball about c holding its members (computed from the CURRENT
 //      positions, so the nodes stay valid between re-sorts, only less compact);
 //   3. every 256 consecutive targets (= one level-1 node; Q_T = the union of the axis-aligned boxes of its 8 leaves) walk
 //      the tree level by level: a node is
 //      ACCEPTED when  a <= theta * D,  D = dist(c, Q_T) > 0  (every target then sees it under a/d <= theta) and
 //      enters the group's far list as one pseudo-hole of charge m at c; otherwise it is opened (its 8 children join
-//      the next level's frontier) or, at the leaf level, its 32 holes enter the near list and are summed exactly;
+//      the next level's frontier) or, at the leaf level, its 8 holes enter the near list and are summed exactly;
 //   4. the lists are consumed by the same packed FP32x2 inner loop as k_field (weighted by m for pseudo-holes).
 //
 // Error bound (stated, and checked against the FP64 oracle in tests/test_gpu_farfield.py): for one accepted node,
@@ -28,12 +28,12 @@
 
 namespace gc {
 
-constexpr uint32_t kLeaf = 32;             // carriers per level-0 node
+constexpr uint32_t kLeaf = 8;              // carriers per level-0 node (32 and 16 measured slower: more exact near field)
 constexpr uint32_t kFan = 8;               // children per node
-constexpr uint32_t kTreeMaxLevels = 9;     // 32 * 8^8 > 2^26
+constexpr uint32_t kTreeMaxLevels = 9;     // 8 * 8^8 = 2^27 > 2^26
 constexpr uint32_t kGroup = 256;           // targets per traversal group = one level-1 node
 constexpr int kTreeTPB = 128;              // threads of k_tree_field: one packed pair of targets each
-constexpr uint32_t kFarCap = 2048, kNearCap = 512, kFrontCap = 2048;
+constexpr uint32_t kFarCap = 2048, kNearCap = 1024, kFrontCap = 1024;
 constexpr uint32_t kTopNodes = 64;         // the walk starts at the lowest level with at most this many nodes
 constexpr uint32_t kSortBlock = 2048;      // keys per block of the radix passes (256 threads x 8)
 
@@ -260,28 +260,31 @@ k_tree_copy(SoA src, SoA dst, const Ctrl* __restrict__ ctrl) {
 }
 
 // ---- nodes -------------------------------------------------------------------------------------------------------
-// Level 0: one warp per leaf (32 consecutive carriers): m, centre of charge, radius of the members about it.
+// Level 0: kLeaf lanes per leaf: m, centre of charge, radius of the members about it.
 __global__ void __launch_bounds__(kTPB)
 k_tree_leaves(const float* __restrict__ px, const float* __restrict__ py, const float* __restrict__ pz,
               const Ctrl* __restrict__ ctrl, float4* __restrict__ node_c, float* __restrict__ node_r) {
   const uint32_t n = ctrl->n_active;
-  const uint32_t leaf = (blockIdx.x * kTPB + threadIdx.x) >> 5, lane = threadIdx.x & 31u;
-  if (leaf >= nodes_at(n, 0)) return;
-  const uint32_t i = leaf * kLeaf + lane;
-  const bool ok = i < n;
-  const uint32_t i0 = leaf * kLeaf;
-  const float x0 = px[i0], y0 = py[i0], z0 = pz[i0];                 // sums relative to the first member: no cancellation
+  const uint32_t gt = blockIdx.x * kTPB + threadIdx.x;
+  const uint32_t leaf = gt / kLeaf, sub = gt % kLeaf;
+  const bool live = leaf < nodes_at(n, 0);                // whole warps stay for the shuffles
+  const uint32_t i0 = live ? leaf * kLeaf : 0u;
+  const uint32_t i = i0 + sub;
+  const bool ok = live && i < n;
+  const float x0 = live ? px[i0] : 0.f, y0 = live ? py[i0] : 0.f, z0 = live ? pz[i0] : 0.f;   // sums relative to the first member
   const float dx = ok ? px[i] - x0 : 0.f, dy = ok ? py[i] - y0 : 0.f, dz = ok ? pz[i] - z0 : 0.f;
   float sx = dx, sy = dy, sz = dz;
-  for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+  for (int o = kLeaf / 2; o > 0; o >>= 1) {
     sx += __shfl_xor_sync(0xffffffffu, sx, o); sy += __shfl_xor_sync(0xffffffffu, sy, o); sz += __shfl_xor_sync(0xffffffffu, sz, o);
   }
-  const uint32_t m = min(kLeaf, n - i0);
+  const uint32_t m = live ? min(kLeaf, n - i0) : 1u;
   const float inv = 1.0f / (float)m;
   const float cx = sx * inv, cy = sy * inv, cz = sz * inv;           // relative to (x0,y0,z0)
   float r2 = ok ? (dx - cx) * (dx - cx) + (dy - cy) * (dy - cy) + (dz - cz) * (dz - cz) : 0.f;
-  for (int o = 16; o > 0; o >>= 1) r2 = fmaxf(r2, __shfl_xor_sync(0xffffffffu, r2, o));
-  if (lane == 0) {
+#pragma unroll
+  for (int o = kLeaf / 2; o > 0; o >>= 1) r2 = fmaxf(r2, __shfl_xor_sync(0xffffffffu, r2, o));
+  if (live && sub == 0) {
     node_c[leaf] = make_float4(x0 + cx, y0 + cy, z0 + cz, (float)m);
     // the stored centre is rounded to FP32 (<= 1 ulp per coordinate): widen the radius accordingly
     node_r[leaf] = sqrtf(r2) * 1.000001f + 2e-7f * (fabsf(x0) + fabsf(y0) + fabsf(z0));
@@ -378,7 +381,8 @@ struct TreeShared {
   uint32_t front[2][kFrontCap];
   uint32_t wcnt[kTreeTPB / 32][3];
   float4 tgt[kGroup];          // the group's targets (sentinel where the group is ragged)
-  float box8[8][6];            // boxes of 32 targets (lo xyz, hi xyz)
+  float box1[6];               // box of the whole group (lo xyz, hi xyz)
+  float box8[8][6];            // boxes of 32 targets
   float box32[32][6];          // boxes of 8 targets
   uint32_t n_far, n_near, n_front[2], group;
 };
@@ -393,6 +397,7 @@ __device__ __forceinline__ float box_d2(const float (&b)[6], const float4 c) {
 __device__ __forceinline__ bool tree_accept(const TreeShared& S, const float4 c, const float R) {
   if (!(R >= 0.f)) return false;
   const float R2 = R * R * 1.000004f;                        // rounding of the distances below
+  if (box_d2(S.box1, c) >= R2) return true;                  // far from the whole group: the common case
   for (int b = 0; b < 8; ++b) {
     if (box_d2(S.box8[b], c) >= R2) continue;
     for (int q = 4 * b; q < 4 * b + 4; ++q) {
@@ -411,14 +416,15 @@ template <bool WEIGHTED>
 __device__ __forceinline__ void tree_eval_tile(const TreeShared& S, int len, const float2 ntx, const float2 nty, const float2 ntz,
                                                const float2 eps2v, float2& tx, float2& ty, float2& tz) {
   float2 ax = make_float2(0.f, 0.f), ay = ax, az = ax;
-#pragma unroll 4
+#pragma unroll 8
   for (int jj = 0; jj < len; ++jj) interact_w<WEIGHTED>(S.xy[jj], S.z[jj], S.m[jj], ntx, nty, ntz, eps2v, ax, ay, az);
   tx = __fadd2_rn(tx, ax); ty = __fadd2_rn(ty, ay); tz = __fadd2_rn(tz, az);       // two-level accumulation
 }
 
-// Evaluation is split P ways: the P CTAs ("parts") working on one group build identical lists and each evaluates the
-// source tiles whose running number is congruent to its part; their partial sums go to P chunks that the integrator
-// adds in fixed order.  This keeps 148 SMs busy when there are few groups and breaks up the occasional heavy group.
+// A group's work is split P ways: CTA ("part") p walks only the subtrees of the top-level nodes k = p (mod P) and
+// evaluates what it finds; the P partial sums go to P chunks that the integrator adds in fixed order.  This keeps 148
+// SMs busy when there are few groups and breaks up the occasional heavy group.  (Splitting the TILES of identical
+// lists instead balanced the parts better but repeated the whole walk P times: slower once leaves hold 8 holes.)
 struct TileSplit { uint32_t no, P, part; };
 
 __device__ __forceinline__ void tree_flush_far(TreeShared& S, const Tree& T, TileSplit& ts, const float2 ntx, const float2 nty,
@@ -426,7 +432,6 @@ __device__ __forceinline__ void tree_flush_far(TreeShared& S, const Tree& T, Til
   const uint32_t tid = threadIdx.x;
   const uint32_t nf = S.n_far;
   for (uint32_t base = 0; base < nf; base += 256) {
-    if (ts.no++ % ts.P != ts.part) continue;
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
       const uint32_t slot = tid + h * kTreeTPB, q = base + slot;
@@ -435,12 +440,12 @@ __device__ __forceinline__ void tree_flush_far(TreeShared& S, const Tree& T, Til
       S.xy[slot] = make_float4(c.x, c.x, c.y, c.y); S.z[slot] = make_float2(c.z, c.z); S.m[slot] = make_float2(c.w, c.w);
     }
     __syncthreads();
-    const int len = (int)min(256u, (nf - base + 3u) & ~3u);
+    const int len = (int)min(256u, (nf - base + 7u) & ~7u);
     tree_eval_tile<true>(S, len, ntx, nty, ntz, eps2v, tx, ty, tz);
     __syncthreads();
   }
   if (tid == 0) {
-    if (nf && ts.part == 0) atomicAdd(&T.tc->far_evals, (unsigned long long)nf * kGroup);
+    if (nf) atomicAdd(&T.tc->far_evals, (unsigned long long)nf * kGroup);
     S.n_far = 0;
   }
   __syncthreads();
@@ -466,7 +471,6 @@ __device__ __forceinline__ void tree_flush_near(TreeShared& S, const Tree& T, Ti
   __syncthreads();
   const uint32_t total = S.pref[nn];
   for (uint32_t base = 0; base < total; base += 256) {
-    if (ts.no++ % ts.P != ts.part) continue;
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
       const uint32_t slot = tid + h * kTreeTPB, q = base + slot;
@@ -480,12 +484,12 @@ __device__ __forceinline__ void tree_flush_near(TreeShared& S, const Tree& T, Ti
       S.xy[slot] = make_float4(x, x, y, y); S.z[slot] = make_float2(z, z);
     }
     __syncthreads();
-    const int len = (int)min(256u, (total - base + 3u) & ~3u);
+    const int len = (int)min(256u, (total - base + 7u) & ~7u);
     tree_eval_tile<false>(S, len, ntx, nty, ntz, eps2v, tx, ty, tz);
     __syncthreads();
   }
   if (tid == 0) {
-    if (total && ts.part == 0) atomicAdd(&T.tc->near_evals, (unsigned long long)total * kGroup);
+    if (total) atomicAdd(&T.tc->near_evals, (unsigned long long)total * kGroup);
     S.n_near = 0;
   }
   __syncthreads();
@@ -567,6 +571,12 @@ k_tree_field(const float* __restrict__ px, const float* __restrict__ py, const f
     }
     if (tid == 0) { S.n_far = 0; S.n_near = 0; S.n_front[0] = 0; S.n_front[1] = 0; }
     __syncthreads();
+    if (tid < 3) {
+      float lo = S.box8[0][tid], hi = S.box8[0][3 + tid];
+      for (int b = 1; b < 8; ++b) { lo = fminf(lo, S.box8[b][tid]); hi = fmaxf(hi, S.box8[b][3 + tid]); }
+      S.box1[tid] = lo; S.box1[3 + tid] = hi;
+    }
+    __syncthreads();
     // Level-by-level walk.  A frontier holds the OPENED nodes of the level above (one entry each); their children
     // k = 8 p + c are the candidates of this level.  At the top level the candidates are all its nodes.
     int cur = 0;
@@ -581,7 +591,7 @@ k_tree_field(const float* __restrict__ px, const float* __restrict__ py, const f
         uint32_t k = kInvalid;
         if (q < n_cand) {
           k = l == ltop ? q : S.front[cur][q >> 3] * kFan + (q & 7u);
-          if (k >= cnt[l]) k = kInvalid;
+          if (k >= cnt[l] || (l == ltop && k % ts.P != ts.part)) k = kInvalid;     // this part's share of the top level
         }
         int cat = 0;                                        // 1 far, 2 near (exact), 3 open
         if (k != kInvalid) {

@@ -183,7 +183,7 @@ int launch_tree_field(gcoreccd_t* h) {
     h->launches += 4 + 3 * kKeyPasses;
   }
   const uint32_t leaves = nodes_at((uint32_t)nb, 0);
-  k_tree_leaves<<<(leaves + 7) / 8, kTPB, 0, h->stream>>>(h->A.x, h->A.y, h->A.z, h->ctrl, T.node_c, T.node_r);
+  k_tree_leaves<<<(leaves * kLeaf + kTPB - 1) / kTPB, kTPB, 0, h->stream>>>(h->A.x, h->A.y, h->A.z, h->ctrl, T.node_c, T.node_r);
   uint32_t upper = 0;
   for (uint32_t l = 1; l < kTreeMaxLevels; ++l) { const uint32_t c = nodes_at((uint32_t)nb, l); upper += c; if (c <= 1) break; }
   k_tree_upper<<<upper, kTPB, 0, h->stream>>>(h->ctrl, T.node_c, T.node_r);
@@ -217,11 +217,11 @@ void enqueue_step(gcoreccd_t* h, uint32_t tiles) {
   h->launches += 2;
 }
 
-// parts per treecode group: enough work items for ~4 per resident CTA, power of two, at most 8 (workspace layout)
+// parts per treecode group: enough work items for ~1.5 per resident CTA, power of two, at most 8 (workspace layout)
 inline uint32_t pick_parts(const gcoreccd_t* h) {
   const uint64_t groups = (h->n_bound + kGroup - 1) / kGroup;
   uint32_t P = 1;
-  while (P < 8 && groups * P < 4ull * (uint64_t)h->grid_tree) P <<= 1;
+  while (P < 8 && groups * P * 2 < 3ull * (uint64_t)h->grid_tree) P <<= 1;      // 1.5 measured best of 0.25 .. 4
   return P;
 }
 
@@ -431,8 +431,8 @@ int gcoreccd_create(const gcoreccd_params* p, gcoreccd_t** out) {
     float* r = h->Ep + (h->L.part_cap - 8 * cp);
     Tree& T = h->tree;
     T.tc = (TreeCtrl*)r;                         r += 64;
-    T.node_c = (float4*)r;                       r += cp / 4 + 64;          // <= cp/28 + 9 nodes of 4 floats
-    T.node_r = r;                                r += cp / 16 + 64;
+    T.node_c = (float4*)r;                       r += cp * 5 / 8 + 64;      // <= cp/7 + 9 nodes of 4 floats
+    T.node_r = r;                                r += cp * 3 / 16 + 64;
     T.key[0] = (unsigned long long*)r; r += 2 * cp;  T.key[1] = (unsigned long long*)r; r += 2 * cp;
     T.val[0] = (uint32_t*)r; r += cp;  T.val[1] = (uint32_t*)r; r += cp;
     T.counts = (uint32_t*)r;                                                // 256 * cp / 2048 = cp / 8 entries
