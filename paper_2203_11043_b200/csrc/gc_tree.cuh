@@ -291,30 +291,44 @@ k_tree_leaves(const float* __restrict__ px, const float* __restrict__ py, const 
   }
 }
 
-// Levels >= 1, straight from the leaves: one CTA per node; centre = count-weighted mean of its leaves' centres (FP64),
-// radius = max over leaves of |c_leaf - c| + r_leaf (a valid, slightly generous ball).
+// Level of the walk's start: the lowest level with at most kTopNodes nodes.  Higher levels are never visited.
+__host__ __device__ inline uint32_t top_level(uint32_t n) {
+  uint32_t l = 0;
+  while (l + 1 < kTreeMaxLevels && nodes_at(n, l) > kTopNodes) ++l;
+  return l;
+}
+
+// Levels 1 .. top_level, straight from the leaves: centre = count-weighted mean of the leaves' centres (FP64),
+// radius = max over leaves of |c_leaf - c| + r_leaf (a valid, slightly generous ball; tighter than nesting level by
+// level).  TPN threads per node: a warp for levels [l_lo, l_hi] = [1, 2] (8 and 64 leaves), a CTA above.
+template <int TPN>
 __global__ void __launch_bounds__(kTPB)
-k_tree_upper(const Ctrl* __restrict__ ctrl, float4* __restrict__ node_c, float* __restrict__ node_r) {
+k_tree_upper(const Ctrl* __restrict__ ctrl, float4* __restrict__ node_c, float* __restrict__ node_r, uint32_t l_lo,
+             uint32_t l_hi) {
+  constexpr int kWarps = TPN / 32;
   __shared__ double s_s[4][kTPB / 32];
   __shared__ float s_r[kTPB / 32];
   __shared__ float s_c[3];
   const uint32_t n = ctrl->n_active;
-  // which (level, k) is this CTA?
-  uint32_t b = blockIdx.x, l = 1;
-  for (;; ++l) {
-    if (l >= kTreeMaxLevels) return;
+  const uint32_t ltop = top_level(n);
+  if (l_hi > ltop) l_hi = ltop;
+  // which (level, k) is this thread group?
+  uint32_t b = (blockIdx.x * kTPB + threadIdx.x) / TPN, l = l_lo;
+  bool live = false;
+  for (; l <= l_hi; ++l) {
     const uint32_t c = nodes_at(n, l);
-    if (b < c) break;
+    if (b < c) { live = true; break; }
     b -= c;
-    if (c <= 1) return;                                      // past the root
   }
+  if (TPN > 32 && !live) return;                             // whole CTA; warps of the TPN = 32 variant exit below
+  if (TPN == 32 && !live) return;                            // whole warp
   const uint32_t per = 1u << (3u * l);                       // leaves per node at this level
   const uint32_t n_leaves = nodes_at(n, 0);
   const uint32_t f0 = b * per, f1 = min(f0 + per, n_leaves);
-  const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+  const uint32_t tid = threadIdx.x % TPN, lane = threadIdx.x & 31u, warp = tid >> 5;
   const float4 ref = node_c[f0];
   double sx = 0, sy = 0, sz = 0, sm = 0;
-  for (uint32_t f = f0 + tid; f < f1; f += kTPB) {
+  for (uint32_t f = f0 + tid; f < f1; f += TPN) {
     const float4 c = node_c[f];
     sx += (double)c.w * (double)(c.x - ref.x); sy += (double)c.w * (double)(c.y - ref.y); sz += (double)c.w * (double)(c.z - ref.z);
     sm += (double)c.w;
@@ -323,29 +337,30 @@ k_tree_upper(const Ctrl* __restrict__ ctrl, float4* __restrict__ node_c, float* 
     sx += __shfl_xor_sync(0xffffffffu, sx, o); sy += __shfl_xor_sync(0xffffffffu, sy, o);
     sz += __shfl_xor_sync(0xffffffffu, sz, o); sm += __shfl_xor_sync(0xffffffffu, sm, o);
   }
-  if (lane == 0) { s_s[0][warp] = sx; s_s[1][warp] = sy; s_s[2][warp] = sz; s_s[3][warp] = sm; }
-  __syncthreads();
-  if (tid == 0) {
-    double a = 0, bb = 0, c = 0, m = 0;
-    for (int w = 0; w < kTPB / 32; ++w) { a += s_s[0][w]; bb += s_s[1][w]; c += s_s[2][w]; m += s_s[3][w]; }
-    s_c[0] = (float)((double)ref.x + a / m); s_c[1] = (float)((double)ref.y + bb / m); s_c[2] = (float)((double)ref.z + c / m);
-    s_s[3][0] = m;
+  if (kWarps > 1) {
+    if (lane == 0) { s_s[0][warp] = sx; s_s[1][warp] = sy; s_s[2][warp] = sz; s_s[3][warp] = sm; }
+    __syncthreads();
+    sx = sy = sz = sm = 0;
+    for (int w = 0; w < kWarps; ++w) { sx += s_s[0][w]; sy += s_s[1][w]; sz += s_s[2][w]; sm += s_s[3][w]; }
   }
-  __syncthreads();
-  const float cx = s_c[0], cy = s_c[1], cz = s_c[2];
+  const float cx = (float)((double)ref.x + sx / sm), cy = (float)((double)ref.y + sy / sm), cz = (float)((double)ref.z + sz / sm);
   float r = 0.f;
-  for (uint32_t f = f0 + tid; f < f1; f += kTPB) {
+  for (uint32_t f = f0 + tid; f < f1; f += TPN) {
     const float4 c = node_c[f];
     const float dx = c.x - cx, dy = c.y - cy, dz = c.z - cz;
     r = fmaxf(r, sqrtf(dx * dx + dy * dy + dz * dz) * 1.000001f + node_r[f]);
   }
   for (int o = 16; o > 0; o >>= 1) r = fmaxf(r, __shfl_xor_sync(0xffffffffu, r, o));
-  if (lane == 0) s_r[warp] = r;
-  __syncthreads();
+  if (kWarps > 1) {
+    if (lane == 0) s_r[warp] = r;
+    __syncthreads();
+    r = s_r[0];
+    for (int w = 1; w < kWarps; ++w) r = fmaxf(r, s_r[w]);
+  }
+  (void)s_c;
   if (tid == 0) {
-    for (int w = 1; w < kTPB / 32; ++w) r = fmaxf(r, s_r[w]);
     const uint32_t idx = level_offset(n, l) + b;
-    node_c[idx] = make_float4(cx, cy, cz, (float)s_s[3][0]);
+    node_c[idx] = make_float4(cx, cy, cz, (float)sm);
     node_r[idx] = r + 2e-7f * (fabsf(cx) + fabsf(cy) + fabsf(cz));
   }
 }
@@ -516,7 +531,7 @@ k_tree_field(const float* __restrict__ px, const float* __restrict__ py, const f
 #pragma unroll
     for (uint32_t l = 0; l < kTreeMaxLevels; ++l) {
       cnt[l] = nodes_at(n, l); off[l] = o; o += cnt[l];
-      if (!found && cnt[l] <= kTopNodes) { ltop = l; found = true; }
+      if (!found && (cnt[l] <= kTopNodes || l + 1 == kTreeMaxLevels)) { ltop = l; found = true; }
     }
   }
   const float2 eps2v = make_float2(eps2, eps2);

@@ -184,9 +184,14 @@ int launch_tree_field(gcoreccd_t* h) {
   }
   const uint32_t leaves = nodes_at((uint32_t)nb, 0);
   k_tree_leaves<<<(leaves * kLeaf + kTPB - 1) / kTPB, kTPB, 0, h->stream>>>(h->A.x, h->A.y, h->A.z, h->ctrl, T.node_c, T.node_r);
-  uint32_t upper = 0;
-  for (uint32_t l = 1; l < kTreeMaxLevels; ++l) { const uint32_t c = nodes_at((uint32_t)nb, l); upper += c; if (c <= 1) break; }
-  k_tree_upper<<<upper, kTPB, 0, h->stream>>>(h->ctrl, T.node_c, T.node_r);
+  // levels 1-2 (8 and 64 leaves per node): a warp per node; levels 3 .. top: a CTA per node; nothing above the top
+  const uint32_t ltop = top_level((uint32_t)nb);
+  const uint32_t low = (ltop >= 1 ? nodes_at((uint32_t)nb, 1) : 0u) + (ltop >= 2 ? nodes_at((uint32_t)nb, 2) : 0u);
+  uint32_t high = 0;
+  for (uint32_t l = 3; l <= ltop; ++l) high += nodes_at((uint32_t)nb, l);
+  if (low) k_tree_upper<32><<<(low + 7) / 8, kTPB, 0, h->stream>>>(h->ctrl, T.node_c, T.node_r, 1u, 2u);
+  if (high) k_tree_upper<kTPB><<<high, kTPB, 0, h->stream>>>(h->ctrl, T.node_c, T.node_r, 3u, kTreeMaxLevels - 1);
+  h->launches += (low ? 1 : 0) + (high ? 1 : 0) - 1;
   k_tree_field<<<h->grid_tree, kTreeTPB, 0, h->stream>>>(h->A.x, h->A.y, h->A.z, h->ctrl, T, h->Ep, (uint32_t)h->L.part_cap,
                                                          h->dp.eps2, h->ff_theta);
   h->launches += 3;
