@@ -410,10 +410,16 @@ def run_sharded(args):
     alloc = lambda nb: torch.empty(nb, dtype=torch.uint8, device="cuda")
     peaks, _ = measured_peaks()
     peak_pairs = SM_COUNT * LANES * 2.0 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / FLOP_PER_PAIR
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-        ev = sharded.ShardedEvent(binding.from_workload(w, stream=stream), rank, world,
-                                  lambda mb: sharded.DistExchange(torch, "cuda", mb, world), alloc)
+    if world > 1 or args.exchange != "virtual":        # torchrun (any world size, also 1): the real multi-process path
+        if not dist.is_initialized():
+            if "RANK" not in os.environ:
+                os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=os.environ.get("MASTER_PORT", "29511"), RANK="0", WORLD_SIZE="1")
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        if args.exchange == "symm":
+            xf = lambda mb: sharded.SymmMemExchange(torch, "cuda", mb, world)
+        else:
+            xf = lambda mb: sharded.DistExchange(torch, "cuda", mb, world)
+        ev = sharded.ShardedEvent(binding.from_workload(w, stream=stream), rank, world, xf, alloc)
         ev.load_carriers(xyz)
         ev.step(args.warmup)
         st0 = ev.refresh()
@@ -427,7 +433,9 @@ def run_sharded(args):
         if rank == 0:
             line = {"mode": "sharded", "n_gpus": world, "workload": w["name"], "n_holes": n, "steps": args.steps,
                     "ms_per_step": ms / args.steps, "n_active": tot["n_active"], "scaling": "strong",
-                    "exchange": "NCCL all_gather_into_tensor of %d-byte messages" % ev.nbytes}
+                    "pair_interactions": tot["pair_interactions"],
+                    "exchange": ("symmetric memory (peer loads in shard_commit)" if args.exchange == "symm" else
+                                 "NCCL all_gather_into_tensor") + " of %d-byte messages" % ev.nbytes}
             print(json.dumps(line), flush=True)
         dist.destroy_process_group()
         return 0
@@ -476,6 +484,8 @@ def main():
     ap.add_argument("--sweep", default="", help="comma-separated hole counts: per-step time vs N (not the headline)")
     ap.add_argument("--sharded", default="", help="config number: one event sharded over the ranks (not the headline)")
     ap.add_argument("--virtual-ranks", type=int, default=8, help="with --sharded on ONE GPU: ranks emulated sequentially")
+    ap.add_argument("--exchange", default="virtual", choices=["virtual", "nccl", "symm"],
+                    help="with --sharded: how the shard messages travel (virtual = one process, no exchange)")
     args = ap.parse_args()
     if args.sharded:
         return run_sharded(args)

@@ -11,7 +11,7 @@ Exchanges (how the G messages reach a rank):
                    the CPU tests (tests/test_sharded_gloo.py drives it with an oracle-backed engine).
   SymmMemExchange  the messages live in torch symmetric memory; shard_commit reads the PEERS' buffers directly, so
                    the all-gather is fused into the commit kernel's loads over NVLink and the only collective left is
-                   a barrier.  Needs > 1 GPU: not exercised on this build's single-GPU boxes.
+                   a barrier.  Exercised at world size 1 only (tests, bench --exchange symm): this build's boxes have one GPU.
   VirtualRanks     G handles on ONE device stepped one after the other on one stream, messages passed by pointer:
                    the same kernels and the same pointer-table commit as the multi-GPU path, with no kernel ever
                    waiting on another (B200_PROFILING.md: emulate ranks sequentially, never concurrently).

@@ -179,9 +179,11 @@ def test_shard_api_errors():
     c.close()
 
 
-def test_sharded_event_through_nccl_all_gather_world_1():
-    """The torch.distributed plumbing of a real multi-GPU run (ShardedEvent + DistExchange on the NCCL backend), with
-    the only world size one GPU allows; G > 1 host logic is covered by tests/test_sharded_gloo.py."""
+@pytest.mark.parametrize("exchange", ["nccl", "symm"])
+def test_sharded_event_through_torch_distributed_world_1(exchange):
+    """The torch.distributed plumbing of a real multi-GPU run — ShardedEvent with DistExchange (NCCL all-gather) or
+    SymmMemExchange (messages in symmetric memory, shard_commit loads them through the rendezvous' peer pointers and a
+    device barrier) — at the only world size one GPU allows; G > 1 host logic is in tests/test_sharded_gloo.py."""
     import socket
     import torch
     import torch.distributed as dist
@@ -193,23 +195,30 @@ def test_sharded_event_through_nccl_all_gather_world_1():
     dist.init_process_group("nccl", init_method="tcp://127.0.0.1:%d" % port, rank=0, world_size=1,
                             device_id=torch.device("cuda", torch.cuda.current_device()))
     try:
-        w = workloads.make(1, n=4096)
+        w = workloads.make(3, n=6000)                      # a track: the message size shrinks during the run
         stream = torch.cuda.Stream()
         with torch.cuda.stream(stream):
             eng = binding.from_workload(w, stream=stream)
-            ev = sharded.ShardedEvent(eng, 0, 1, lambda mb: sharded.DistExchange(torch, "cuda", mb, 1),
-                                      lambda nb: torch.empty(nb, dtype=torch.uint8, device="cuda"))
+            if exchange == "symm":
+                xf = lambda mb: sharded.SymmMemExchange(torch, "cuda", mb, 1)
+            else:
+                xf = lambda mb: sharded.DistExchange(torch, "cuda", mb, 1)
+            ev = sharded.ShardedEvent(eng, 0, 1, xf, lambda nb: torch.empty(nb, dtype=torch.uint8, device="cuda"))
             ev.load_carriers(w["xyz"])
             ev.step(10)
             st = ev.refresh()
+            ev.step(30)
+            st = ev.refresh()
             red = sharded.dist_reduce_sum(torch, "cuda")
             tot = ev.totals(red)
+            img = ev.image(red)
         ref = binding.from_workload(w)
         ref.load_carriers(w["xyz"])
-        ref.step(10)
+        ref.step(40)
         a, b = eng.read_carriers(), ref.read_carriers()
-        assert st["step"] == 10 and np.array_equal(a[1], b[1]) and np.array_equal(a[0], b[0])
+        assert st["step"] == 40 and np.array_equal(a[1], b[1]) and np.array_equal(a[0], b[0])
         assert tot["pair_interactions"] == ref.state()["pair_interactions"]
+        assert np.array_equal(img, ref.read_image()[0].astype(np.uint32))
         ref.close()
         eng.close()
     finally:
