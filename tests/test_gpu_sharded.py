@@ -223,3 +223,37 @@ def test_sharded_event_through_torch_distributed_world_1(exchange):
         eng.close()
     finally:
         dist.destroy_process_group()
+
+
+def test_full_size_sharded_step_against_sampled_oracle():
+    """cfg3 at full size (262,144 holes) over 8 virtual ranks — the configuration `bench.py --sharded 3` times: the
+    oracle advances sampled carriers one step from the exported snapshot (needs only their fields: eq. 6 at the sampled
+    targets against all sources) and must land within 2e-4 um of the sharded GPU step (DESIGN.md §7 snapshot-restart)."""
+    from util import oracle_params
+    w = workloads.make(3)
+    P = w["params"]
+    vr, es = _virtual(w, 8)
+    vr.load_carriers(w["xyz"])
+    vr.step(3)                                             # shares have moved: the track's front end is retiring
+    st = vr.refresh()
+    xyz, ids = es[5].read_carriers()
+    rng = np.random.default_rng(3)
+    t = np.sort(rng.choice(len(xyz), size=768, replace=False)).astype(np.uint64)
+    Eref = g.coulomb_field(xyz.astype(np.float64), eps_um=P["softening_um"], Kp=g.coulomb_constant(P["eps_si"]), targets=t)
+    op = oracle_params(w, flags=g.FP32_STATE)
+    vr.step(1)
+    xyz1, ids1 = es[2].read_carriers()
+    pos_of = {int(i): k for k, i in enumerate(ids1)}
+    worst, mismatch = 0.0, 0
+    for k, j in enumerate(t.astype(np.int64)):
+        r_new, collected = g.advance(op, st["step"], int(ids[j]), xyz[j].astype(np.float64), Eref[k])
+        here = int(ids[j]) in pos_of
+        if here != (not collected):
+            mismatch += 1
+            assert abs(r_new[2]) < 1e-3
+        elif here:
+            worst = max(worst, float(np.abs(xyz1[pos_of[int(ids[j])]].astype(np.float64) - r_new).max()))
+    assert worst <= 2e-4 and mismatch <= 1, (worst, mismatch)
+    tot = vr.totals()
+    assert tot["n_active"] + tot["n_collected"] == tot["n_loaded"] == len(w["xyz"])
+    _close(es)
