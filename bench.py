@@ -421,6 +421,8 @@ def run_sharded(args):
             xf = lambda mb: sharded.DistExchange(torch, "cuda", mb, world)
         ev = sharded.ShardedEvent(binding.from_workload(w, stream=stream), rank, world, xf, alloc)
         ev.load_carriers(xyz)
+        if args.farfield >= 0:
+            ev.e.set_farfield(args.farfield)
         ev.step(args.warmup)
         st0 = ev.refresh()
         dist.barrier(); torch.cuda.synchronize()
@@ -443,6 +445,9 @@ def run_sharded(args):
     es = [binding.from_workload(w, stream=stream) for _ in range(G)]
     vr = sharded.VirtualRanks(es, alloc)
     vr.load_carriers(xyz)
+    if args.farfield >= 0:
+        for e in es:
+            e.set_farfield(args.farfield)
     vr.step(args.warmup)
     st = vr.refresh()
     na = st["n_active"]
@@ -462,11 +467,12 @@ def run_sharded(args):
                           for k in range(K)])
     per_rank = (local_ms + commit_ms).mean(axis=0)
     st1 = vr.refresh()
-    line = {"mode": "sharded-virtual", "virtual_ranks": G, "workload": w["name"], "n_holes": n, "n_active_start": na,
+    line = {"mode": "sharded-virtual", "farfield_theta": args.farfield if args.farfield >= 0 else None, "virtual_ranks": G, "workload": w["name"], "n_holes": n, "n_active_start": na,
             "n_active_end": st1["n_active"], "steps": K, "per_rank_ms_per_step": [float(v) for v in per_rank],
             "max_rank_ms_per_step": float(per_rank.max()), "sum_ranks_ms_per_step": float(per_rank.sum()),
             "commit_ms": float(commit_ms.mean()), "message_bytes": vr.nbytes,
-            "frac_of_fp32_peak_per_rank": float(na * float(na) / G / (per_rank.max() * 1e-3) / peak_pairs),
+            "frac_of_fp32_peak_per_rank": (float(na * float(na) / G / (per_rank.max() * 1e-3) / peak_pairs)
+                                           if args.farfield < 0 else None),      # pairs evaluated only in the exact path
             "note": "each rank's kernels measured alone on one B200; the per-step all-gather of G messages over NVLink "
                     "is not included (one GPU available)"}
     print(json.dumps(line), flush=True)
@@ -484,6 +490,7 @@ def main():
     ap.add_argument("--sweep", default="", help="comma-separated hole counts: per-step time vs N (not the headline)")
     ap.add_argument("--sharded", default="", help="config number: one event sharded over the ranks (not the headline)")
     ap.add_argument("--virtual-ranks", type=int, default=8, help="with --sharded on ONE GPU: ranks emulated sequentially")
+    ap.add_argument("--farfield", type=float, default=-1.0, help="with --sharded: theta of the far-field variant (< 0: exact)")
     ap.add_argument("--exchange", default="virtual", choices=["virtual", "nccl", "symm"],
                     help="with --sharded: how the shard messages travel (virtual = one process, no exchange)")
     args = ap.parse_args()

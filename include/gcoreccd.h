@@ -239,7 +239,9 @@ int gcoreccd_shard_commit(gcoreccd_t* h, const void* const* msgs_host, uint32_t 
  * Consequences: the active set is no longer in load order (read_carriers / eval_field return the current curve order;
  * match by id); pair_interactions still counts N_a^2 per step (the pairs REPRESENTED) — the interactions actually
  * evaluated are in farfield_stats and no throughput claim of the exact metric may use this variant.
- * set_farfield: theta in [0, 1) switches the variant on, theta < 0 off; STATE on a sharded handle.  Synchronises.
+ * set_farfield: theta in [0, 1) switches the variant on, theta < 0 off.  Synchronises.  On a sharded handle every rank
+ *   must make the same call at the same step: the re-sort and the tree are then computed identically on every rank
+ *   (replicated state) and only the walk is sharded, each rank walking the groups of its own share.
  *   While fewer than min_active holes are drifting (0 => 24,576; 1 => never) the all-pairs kernel is used instead:
  *   below a few 1e4 holes it is the faster of the two (measured), and it is exact.
  * farfield_stats: interactions evaluated since set_farfield — pseudo-hole (far) and exact (near), each counted per

@@ -521,7 +521,8 @@ k_tree_field(const float* __restrict__ px, const float* __restrict__ py, const f
   if (n == 0) return;
   const uint32_t stride = ctrl->plan.stride;
   const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
-  const uint32_t n_groups = (n + kGroup - 1) / kGroup;
+  const uint32_t t0 = ctrl->plan.t0, t_end = t0 + ctrl->plan.nt;   // this rank's share of the targets (all, if unsharded)
+  const uint32_t n_groups = (ctrl->plan.nt + kGroup - 1) / kGroup;
   const uint32_t P = max(ctrl->plan.S, 1u);                  // parts per group = partial chunks (set by the planner)
   uint32_t cnt[kTreeMaxLevels], off[kTreeMaxLevels];
   uint32_t ltop = 0;
@@ -545,12 +546,12 @@ k_tree_field(const float* __restrict__ px, const float* __restrict__ py, const f
     const uint32_t g = item / P;
     TileSplit ts = {0u, P, item - g * P};
     // this thread's packed pair of targets, negated
-    const uint32_t i0 = g * kGroup + 2u * tid;
+    const uint32_t i0 = t0 + g * kGroup + 2u * tid;
     float2 vx = make_float2(0.f, 0.f), vy = vx, vz = vx;
-    if (i0 + 1 < n) {
+    if (i0 + 1 < t_end) {
       vx = *reinterpret_cast<const float2*>(px + i0); vy = *reinterpret_cast<const float2*>(py + i0);
       vz = *reinterpret_cast<const float2*>(pz + i0);
-    } else if (i0 < n) { vx.x = px[i0]; vy.x = py[i0]; vz.x = pz[i0]; }
+    } else if (i0 < t_end) { vx.x = px[i0]; vy.x = py[i0]; vz.x = pz[i0]; }
     const float2 ntx = make_float2(-vx.x, -vx.y), nty = make_float2(-vy.x, -vy.y), ntz = make_float2(-vz.x, -vz.y);
     float2 tx = make_float2(0.f, 0.f), ty = tx, tz = tx;
     // Acceptance needs  a <= theta |x_t - c|  for EVERY target t of the group.  It is decided exactly, through a
@@ -559,7 +560,7 @@ k_tree_field(const float* __restrict__ px, const float* __restrict__ py, const f
     // leaves the cloud and re-enters it elsewhere, a run of 256 holes is then two distant pieces, and everything in
     // between would be swallowed into its exact near field.
     {
-      const bool v0 = i0 < n, v1 = i0 + 1 < n;
+      const bool v0 = i0 < t_end, v1 = i0 + 1 < t_end;
       S.tgt[2 * tid] = v0 ? make_float4(vx.x, vy.x, vz.x, 0.f) : make_float4(kSentinel, kSentinel, kSentinel, 0.f);
       S.tgt[2 * tid + 1] = v1 ? make_float4(vx.y, vy.y, vz.y, 0.f) : make_float4(kSentinel, kSentinel, kSentinel, 0.f);
       float lo[3] = {v0 ? vx.x : 3e18f, v0 ? vy.x : 3e18f, v0 ? vz.x : 3e18f};
@@ -643,8 +644,8 @@ k_tree_field(const float* __restrict__ px, const float* __restrict__ py, const f
     tree_flush_far(S, T, ts, ntx, nty, ntz, eps2v, tx, ty, tz);
     tree_flush_near(S, T, ts, px, py, pz, ntx, nty, ntz, eps2v, tx, ty, tz);
 
-    if (i0 < stride) {
-      float* e = Ep + (size_t)ts.part * stride + i0;
+    if (i0 - t0 < stride) {                                   // partial rows are indexed from the share's start
+      float* e = Ep + (size_t)ts.part * stride + (i0 - t0);
       *reinterpret_cast<float2*>(e) = tx;
       *reinterpret_cast<float2*>(e + part_cap) = ty;
       *reinterpret_cast<float2*>(e + 2 * (size_t)part_cap) = tz;

@@ -224,7 +224,7 @@ void enqueue_step(gcoreccd_t* h, uint32_t tiles) {
 
 // parts per treecode group: enough work items for ~1.5 per resident CTA, power of two, at most 8 (workspace layout)
 inline uint32_t pick_parts(const gcoreccd_t* h) {
-  const uint64_t groups = (h->n_bound + kGroup - 1) / kGroup;
+  const uint64_t groups = ((h->n_bound + h->shard_world - 1) / h->shard_world + kGroup - 1) / kGroup;   // of this rank's share
   uint32_t P = 1;
   while (P < 8 && groups * P * 2 < 3ull * (uint64_t)h->grid_tree) P <<= 1;      // 1.5 measured best of 0.25 .. 4
   return P;
@@ -719,7 +719,6 @@ int gcoreccd_set_shard(gcoreccd_t* h, uint32_t rank, uint32_t world) {
   if (world > 1 && (h->dp.flags & GCORECCD_COULOMB_OFF))
     return fail(h, GCORECCD_ERR_INVALID, "set_shard: without eq. 6 carriers are independent; run replicas instead");
   if (h->n_loaded != 0 || h->evb.loaded) return fail(h, GCORECCD_ERR_STATE, "set_shard: only on an empty handle (reset first)");
-  if (world > 1 && h->ff_on) return fail(h, GCORECCD_ERR_STATE, "set_shard: the far-field variant is on");
   h->shard_rank = rank;
   h->shard_world = world;
   h->variant = -1;
@@ -740,8 +739,10 @@ int gcoreccd_shard_local(gcoreccd_t* h, void* msg_dev, uint64_t msg_bytes) {
   DeviceGuard guard(h->device);
   // the share shrinks with n_active: pick the field variant from the share, not from the whole population
   const int v = pick_variant((h->n_bound + h->shard_world - 1) / h->shard_world);
-  if (v != h->variant) {
+  const uint32_t parts = h->ff_on && h->n_bound >= h->ff_min_active ? pick_parts(h) : 0u;   // treecode walk of the share
+  if (v != h->variant || parts != h->ff_parts) {
     h->variant = v;
+    h->ff_parts = parts;
     k_replan<<<1, 32, 0, h->stream>>>(h->ctrl, plan_args(h, v), 0, 0u, 0, 0ull);
     h->launches += 1;
   }
@@ -778,7 +779,6 @@ int gcoreccd_shard_commit(gcoreccd_t* h, const void* const* msgs_host, uint32_t 
 // ---- far-field variant (gc_tree.cuh) ---------------------------------------------------------------------------
 int gcoreccd_set_farfield(gcoreccd_t* h, double theta, uint32_t resort_every, uint64_t min_active) {
   if (!h || !(theta < 1.0)) return GCORECCD_ERR_INVALID;
-  if (theta >= 0.0 && h->shard_world > 1) return fail(h, GCORECCD_ERR_STATE, "set_farfield: the handle is sharded");
   if (theta >= 0.0 && h->L.cap_pad > (1ull << 26)) return fail(h, GCORECCD_ERR_CAPACITY, "set_farfield: capacity");
   DeviceGuard guard(h->device);
   GC_CUDA(h, cudaStreamSynchronize(h->stream));

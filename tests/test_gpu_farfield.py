@@ -173,9 +173,74 @@ def test_farfield_api_errors_and_switching_back():
     assert np.allclose(E1[np.argsort(ids)], E0, rtol=2e-5, atol=1e-6 * np.abs(E0).max())
     sim.step(3)
     assert sim.state()["step"] == 3
-    sh = gpu_sim(w)
-    sh.set_shard(0, 2)
-    with pytest.raises(binding.GcoreccdError):
-        sh.set_farfield(0.3)
-    sh.close()
     sim.close()
+
+
+def _virtual_ff(w, G, theta, resort, min_active):
+    import torch
+    from paper_2203_11043_b200 import binding, sharded
+    stream = torch.cuda.Stream()
+    es = [binding.from_workload(w, stream=stream) for _ in range(G)]
+    vr = sharded.VirtualRanks(es, lambda nb: torch.empty(nb, dtype=torch.uint8, device="cuda"))
+    vr.load_carriers(w["xyz"])
+    for e in es:
+        e.set_farfield(theta, resort, min_active)
+    return vr, es
+
+
+def test_sharded_treecode_theta_zero_matches_the_oracle():
+    """Far-field variant on a sharded event (3 virtual ranks): every rank re-sorts and builds the same tree, each walks
+    the groups of its own share.  theta = 0 => exact field => the 10-step tolerance of the exact path."""
+    w = workloads.make(1, n=8192)
+    vr, es = _virtual_ff(w, 3, 0.0, 3, 1)
+    vr.step(10)
+    o = oracle_sim(w, flags=g.FP32_STATE)
+    o.load(w["xyz"])
+    history = []
+    for _ in range(10):
+        history.append(o.carriers())
+        o.step(1)
+    oxyz, oids = o.carriers()
+    tot = vr.totals()
+    assert tot["step"] == 10 and tot["pair_interactions"] == o.state()["pair_interactions"]
+    first = None
+    for e in es:
+        xyz, ids = e.read_carriers()
+        if first is None:
+            first = (xyz, ids)
+            order = np.argsort(ids)
+            traj_assert(xyz[order], ids[order], oxyz, oids, history, len(w["xyz"]), 1e-3)
+        else:
+            assert np.array_equal(ids, first[1]) and np.array_equal(xyz, first[0])     # replicated state stays identical
+    for e in es:
+        e.close()
+
+
+def test_sharded_treecode_run_conserves_and_tracks_the_single_gpu_treecode():
+    w = workloads.make(3, n=40000)
+    vr, es = _virtual_ff(w, 4, 0.4, 4, 1)
+    single = gpu_sim(w)
+    single.load_carriers(w["xyz"])
+    single.set_farfield(0.4, 4, 1)
+    vr.step(6)
+    single.step(6)
+    a, ia = es[1].read_carriers()
+    b, ib = single.read_carriers()
+    oa, ob = np.argsort(ia), np.argsort(ib)
+    assert np.array_equal(ia[oa], ib[ob])
+    # same lists, same arithmetic; only the number of parts per group (hence the FP32 summation split) may differ
+    d = np.abs(a[oa].astype(np.float64) - b[ob]).max(axis=1)
+    assert np.median(d) <= 1e-4 and (d > 1e-3).mean() <= 0.02, (np.median(d), (d > 1e-3).mean())
+    for _ in range(4):
+        vr.step(40)
+        st = vr.refresh()
+        tot = vr.totals()
+        assert int(vr.image().sum()) + tot["n_out_of_window"] + st["n_active"] == 40000
+    ids = [e.read_carriers()[1] for e in es]
+    assert all(np.array_equal(ids[0], i) for i in ids[1:])
+    stats = [e.farfield_stats() for e in es]
+    assert all(s_["far_evals"] > 0 for s_ in stats)
+    assert max(s_["near_evals"] + s_["far_evals"] for s_ in stats) < 0.5 * sum(s_["near_evals"] + s_["far_evals"] for s_ in stats)
+    single.close()
+    for e in es:
+        e.close()
