@@ -34,6 +34,8 @@ constexpr uint32_t kTreeMaxLevels = 9;     // 8 * 8^8 = 2^27 > 2^26
 constexpr uint32_t kGroup = 256;           // targets per traversal group = one level-1 node
 constexpr int kTreeTPB = 128;              // threads of k_tree_field: one packed pair of targets each
 constexpr uint32_t kFarCap = 2048, kNearCap = 1024, kFrontCap = 1024;
+constexpr int kCPT = 2;                    // candidates per thread and batch of the walk
+constexpr uint32_t kBatch = kCPT * kTreeTPB;
 constexpr uint32_t kTopNodes = 64;         // the walk starts at the lowest level with at most this many nodes
 constexpr uint32_t kSortBlock = 2048;      // keys per block of the radix passes (256 threads x 8)
 
@@ -394,12 +396,12 @@ struct TreeShared {
   uint2 near[kNearCap];
   uint32_t pref[kNearCap + 1];
   uint32_t front[2][kFrontCap];
-  uint32_t wcnt[kTreeTPB / 32][3];
+  uint32_t wcnt[2][kCPT][kTreeTPB / 32][3];
   float4 tgt[kGroup];          // the group's targets (sentinel where the group is ragged)
   float box1[6];               // box of the whole group (lo xyz, hi xyz)
   float box8[8][6];            // boxes of 32 targets
   float box32[32][6];          // boxes of 8 targets
-  uint32_t n_far, n_near, n_front[2], group;
+  uint32_t group;
 };
 
 __device__ __forceinline__ float box_d2(const float (&b)[6], const float4 c) {
@@ -440,12 +442,12 @@ __device__ __forceinline__ void tree_eval_tile(const TreeShared& S, int len, con
 // evaluates what it finds; the P partial sums go to P chunks that the integrator adds in fixed order.  This keeps 148
 // SMs busy when there are few groups and breaks up the occasional heavy group.  (Splitting the TILES of identical
 // lists instead balanced the parts better but repeated the whole walk P times: slower once leaves hold 8 holes.)
-struct TileSplit { uint32_t no, P, part; };
-
-__device__ __forceinline__ void tree_flush_far(TreeShared& S, const Tree& T, TileSplit& ts, const float2 ntx, const float2 nty,
+// Callers guarantee a block barrier between the last list append and the flush; n_far / n_near are the (uniform)
+// register copies of the list lengths and are reset here.
+__device__ __forceinline__ void tree_flush_far(TreeShared& S, const Tree& T, uint32_t& n_far, const float2 ntx, const float2 nty,
                                                const float2 ntz, const float2 eps2v, float2& tx, float2& ty, float2& tz) {
   const uint32_t tid = threadIdx.x;
-  const uint32_t nf = S.n_far;
+  const uint32_t nf = n_far;
   for (uint32_t base = 0; base < nf; base += 256) {
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
@@ -459,19 +461,16 @@ __device__ __forceinline__ void tree_flush_far(TreeShared& S, const Tree& T, Til
     tree_eval_tile<true>(S, len, ntx, nty, ntz, eps2v, tx, ty, tz);
     __syncthreads();
   }
-  if (tid == 0) {
-    if (nf) atomicAdd(&T.tc->far_evals, (unsigned long long)nf * kGroup);
-    S.n_far = 0;
-  }
-  __syncthreads();
+  if (tid == 0 && nf) atomicAdd(&T.tc->far_evals, (unsigned long long)nf * kGroup);
+  n_far = 0;
 }
 
-__device__ __forceinline__ void tree_flush_near(TreeShared& S, const Tree& T, TileSplit& ts, const float* __restrict__ px,
+__device__ __forceinline__ void tree_flush_near(TreeShared& S, const Tree& T, uint32_t& n_near, const float* __restrict__ px,
                                                 const float* __restrict__ py, const float* __restrict__ pz, const float2 ntx,
                                                 const float2 nty, const float2 ntz, const float2 eps2v, float2& tx, float2& ty,
                                                 float2& tz) {
   const uint32_t tid = threadIdx.x, lane = tid & 31u;
-  const uint32_t nn = S.n_near;
+  const uint32_t nn = n_near;
   if (tid < 32) {                                          // exclusive prefix of the range lengths, one warp
     uint32_t run = 0;
     for (uint32_t b = 0; b < nn; b += 32) {
@@ -503,11 +502,8 @@ __device__ __forceinline__ void tree_flush_near(TreeShared& S, const Tree& T, Ti
     tree_eval_tile<false>(S, len, ntx, nty, ntz, eps2v, tx, ty, tz);
     __syncthreads();
   }
-  if (tid == 0) {
-    if (total) atomicAdd(&T.tc->near_evals, (unsigned long long)total * kGroup);
-    S.n_near = 0;
-  }
-  __syncthreads();
+  if (tid == 0 && total) atomicAdd(&T.tc->near_evals, (unsigned long long)total * kGroup);
+  n_near = 0;
 }
 
 // Field of every active carrier by the treecode; result in the first plan.S chunks of the partial planes, in the
@@ -536,15 +532,16 @@ k_tree_field(const float* __restrict__ px, const float* __restrict__ py, const f
     }
   }
   const float2 eps2v = make_float2(eps2, eps2);
+  const float inv_theta = theta > 0.f ? 1.0f / theta * 1.000001f : 0.f;      // rounded up: never accepts more than a <= theta d
   constexpr uint32_t kInvalid = 0xffffffffu;
 
   for (;;) {
-    if (tid == 0) S.group = atomicAdd(&T.tc->next_group, 1u);
-    __syncthreads();
+    if (tid == 0) S.group = atomicAdd(&T.tc->next_group, 1u);      // dynamic: with ~1.5 items per CTA, fetching ahead
+    __syncthreads();                                                // (tried) costs more in balance than it hides
     const uint32_t item = S.group;
     if (item >= n_groups * P) break;
     const uint32_t g = item / P;
-    TileSplit ts = {0u, P, item - g * P};
+    const uint32_t part = item - g * P;
     // this thread's packed pair of targets, negated
     const uint32_t i0 = t0 + g * kGroup + 2u * tid;
     float2 vx = make_float2(0.f, 0.f), vy = vx, vz = vx;
@@ -585,7 +582,6 @@ k_tree_field(const float* __restrict__ px, const float* __restrict__ py, const f
         for (int c = 0; c < 3; ++c) { S.box8[tid >> 4][c] = lo[c]; S.box8[tid >> 4][3 + c] = hi[c]; }
       }
     }
-    if (tid == 0) { S.n_far = 0; S.n_near = 0; S.n_front[0] = 0; S.n_front[1] = 0; }
     __syncthreads();
     if (tid < 3) {
       float lo = S.box8[0][tid], hi = S.box8[0][3 + tid];
@@ -594,58 +590,76 @@ k_tree_field(const float* __restrict__ px, const float* __restrict__ py, const f
     }
     __syncthreads();
     // Level-by-level walk.  A frontier holds the OPENED nodes of the level above (one entry each); their children
-    // k = 8 p + c are the candidates of this level.  At the top level the candidates are all its nodes.
+    // k = 8 p + c are the candidates of this level.  At the top level the candidates are this part's share of its
+    // nodes.  The list lengths live in registers, identical in every thread (each derives them from the per-warp
+    // counts), so a batch of 256 candidates costs ONE barrier (three with shared-memory counters: the barrier after
+    // the divergent acceptance test was the largest single stall of the kernel).
+    uint32_t n_far = 0, n_near = 0, n_front_cur = 0, n_front_next = 0, par = 0;
     int cur = 0;
     for (uint32_t l = ltop;; --l) {
-      const uint32_t n_cand = l == ltop ? cnt[ltop] : S.n_front[cur] * kFan;
+      const uint32_t n_cand = l == ltop ? cnt[ltop] : n_front_cur * kFan;
       const uint32_t lsize = level_size(l);
-      for (uint32_t base = 0; base < n_cand; base += kTreeTPB) {
-        if (S.n_far + kTreeTPB > kFarCap) tree_flush_far(S, T, ts, ntx, nty, ntz, eps2v, tx, ty, tz);
-        if (S.n_near + kTreeTPB > kNearCap) tree_flush_near(S, T, ts, px, py, pz, ntx, nty, ntz, eps2v, tx, ty, tz);
-        const bool room = l > 0 && S.n_front[cur ^ 1] + kTreeTPB <= kFrontCap;
-        const uint32_t q = base + tid;
-        uint32_t k = kInvalid;
-        if (q < n_cand) {
-          k = l == ltop ? q : S.front[cur][q >> 3] * kFan + (q & 7u);
-          if (k >= cnt[l] || (l == ltop && k % ts.P != ts.part)) k = kInvalid;     // this part's share of the top level
+      for (uint32_t base = 0; base < n_cand; base += kBatch) {
+        if (n_far + kBatch > kFarCap) { __syncthreads(); tree_flush_far(S, T, n_far, ntx, nty, ntz, eps2v, tx, ty, tz); }
+        if (n_near + kBatch > kNearCap) { __syncthreads(); tree_flush_near(S, T, n_near, px, py, pz, ntx, nty, ntz, eps2v, tx, ty, tz); }
+        const bool room = l > 0 && n_front_next + kBatch <= kFrontCap;
+        uint32_t k[kCPT], b1[kCPT], b2[kCPT], b3[kCPT];
+        float4 c[kCPT];
+        float r[kCPT];
+#pragma unroll
+        for (int u = 0; u < kCPT; ++u) {                    // both candidates' node loads are in flight together
+          const uint32_t q = base + u * kTreeTPB + tid;
+          k[u] = kInvalid;
+          if (q < n_cand) {
+            k[u] = l == ltop ? q : S.front[cur][q >> 3] * kFan + (q & 7u);
+            if (k[u] >= cnt[l] || (l == ltop && k[u] % P != part)) k[u] = kInvalid;   // this part's share of the top level
+          }
+          if (k[u] != kInvalid) { c[u] = T.node_c[off[l] + k[u]]; r[u] = T.node_r[off[l] + k[u]]; }
         }
-        int cat = 0;                                        // 1 far, 2 near (exact), 3 open
-        if (k != kInvalid) {
-          const float4 c = T.node_c[off[l] + k];
-          const float r = T.node_r[off[l] + k];
-          if (tree_accept(S, c, theta > 0.f ? r / theta : -1.f)) cat = 1;
-          else cat = room ? 3 : 2;                          // no room to open: sum the whole node exactly (always valid)
+        int cat[kCPT];                                      // 1 far, 2 near (exact), 3 open
+#pragma unroll
+        for (int u = 0; u < kCPT; ++u) {
+          cat[u] = 0;
+          if (k[u] != kInvalid) {
+            if (theta > 0.f && tree_accept(S, c[u], r[u] * inv_theta)) cat[u] = 1;
+            else cat[u] = room ? 3 : 2;                     // no room to open: sum the whole node exactly (always valid)
+          }
+          b1[u] = __ballot_sync(0xffffffffu, cat[u] == 1); b2[u] = __ballot_sync(0xffffffffu, cat[u] == 2);
+          b3[u] = __ballot_sync(0xffffffffu, cat[u] == 3);
+          if (lane == 0) {
+            S.wcnt[par][u][warp][0] = __popc(b1[u]); S.wcnt[par][u][warp][1] = __popc(b2[u]); S.wcnt[par][u][warp][2] = __popc(b3[u]);
+          }
         }
-        const uint32_t b1 = __ballot_sync(0xffffffffu, cat == 1), b2 = __ballot_sync(0xffffffffu, cat == 2),
-                       b3 = __ballot_sync(0xffffffffu, cat == 3);
-        if (lane == 0) { S.wcnt[warp][0] = __popc(b1); S.wcnt[warp][1] = __popc(b2); S.wcnt[warp][2] = __popc(b3); }
         __syncthreads();
-        uint32_t o1 = S.n_far, o2 = S.n_near, o3 = S.n_front[cur ^ 1];
-        for (uint32_t w = 0; w < warp; ++w) { o1 += S.wcnt[w][0]; o2 += S.wcnt[w][1]; o3 += S.wcnt[w][2]; }
         const uint32_t lt = (1u << lane) - 1u;
-        if (cat == 1) S.far[o1 + __popc(b1 & lt)] = off[l] + k;
-        else if (cat == 2) {
-          const uint32_t start = k * lsize;
-          S.near[o2 + __popc(b2 & lt)] = make_uint2(start, min(lsize, n - start));
-        } else if (cat == 3) S.front[cur ^ 1][o3 + __popc(b3 & lt)] = k;
-        __syncthreads();
-        if (tid == 0) {
-          uint32_t a = 0, b = 0, c = 0;
-          for (int w = 0; w < kTreeTPB / 32; ++w) { a += S.wcnt[w][0]; b += S.wcnt[w][1]; c += S.wcnt[w][2]; }
-          S.n_far += a; S.n_near += b; S.n_front[cur ^ 1] += c;
+#pragma unroll
+        for (int u = 0; u < kCPT; ++u) {                    // list order: (u, warp, lane) — fixed, hence reproducible sums
+          uint32_t o1 = n_far, o2 = n_near, o3 = n_front_next;
+#pragma unroll
+          for (uint32_t w = 0; w < kTreeTPB / 32; ++w) {
+            const uint32_t c1 = S.wcnt[par][u][w][0], c2 = S.wcnt[par][u][w][1], c3 = S.wcnt[par][u][w][2];
+            if (w < warp) { o1 += c1; o2 += c2; o3 += c3; }
+            n_far += c1; n_near += c2; n_front_next += c3;
+          }
+          if (cat[u] == 1) S.far[o1 + __popc(b1[u] & lt)] = off[l] + k[u];
+          else if (cat[u] == 2) {
+            const uint32_t start = k[u] * lsize;
+            S.near[o2 + __popc(b2[u] & lt)] = make_uint2(start, min(lsize, n - start));
+          } else if (cat[u] == 3) S.front[cur ^ 1][o3 + __popc(b3[u] & lt)] = k[u];
         }
-        __syncthreads();
+        par ^= 1u;                                          // double-buffered counts: the next batch may write at once
       }
       if (l == 0) break;
-      if (tid == 0) S.n_front[cur] = 0;
+      __syncthreads();                                      // the next level's frontier is complete
+      n_front_cur = n_front_next; n_front_next = 0;
       cur ^= 1;
-      __syncthreads();
     }
-    tree_flush_far(S, T, ts, ntx, nty, ntz, eps2v, tx, ty, tz);
-    tree_flush_near(S, T, ts, px, py, pz, ntx, nty, ntz, eps2v, tx, ty, tz);
+    __syncthreads();
+    tree_flush_far(S, T, n_far, ntx, nty, ntz, eps2v, tx, ty, tz);
+    tree_flush_near(S, T, n_near, px, py, pz, ntx, nty, ntz, eps2v, tx, ty, tz);
 
     if (i0 - t0 < stride) {                                   // partial rows are indexed from the share's start
-      float* e = Ep + (size_t)ts.part * stride + (i0 - t0);
+      float* e = Ep + (size_t)part * stride + (i0 - t0);
       *reinterpret_cast<float2*>(e) = tx;
       *reinterpret_cast<float2*>(e + part_cap) = ty;
       *reinterpret_cast<float2*>(e + 2 * (size_t)part_cap) = tz;
