@@ -30,7 +30,8 @@ struct EventTable {            // device arrays, one entry per event
   uint64_t* step;              // steps taken so far = index of the event's next step (Philox counter)
 };
 
-// Three variants, chosen per event by its size at load:
+// Four variants, chosen per event by its size at load (k_events_warp below for the first, k_events for the rest):
+constexpr uint32_t kEvCapMicro = 32;       // one WARP per event, state in registers, no block barrier at all
 constexpr uint32_t kEvCapTiny  = 128;      // NPACK 1,  64 threads: one pass covers 128 targets, ~12 CTAs (events) per SM
 constexpr uint32_t kEvCapSmall = 512;      // NPACK 1, 256 threads: one pass covers 512 targets, 3 CTAs per SM
 constexpr uint32_t kEvCapLarge = 4096;     // NPACK 4, 256 threads: 2,048 targets per pass, one CTA per SM
@@ -216,6 +217,105 @@ k_events(SoA A, EventTable ev, const uint32_t* __restrict__ order, uint32_t n_or
       ev.step[e] = step;
       if (s_coll) atomicAdd((unsigned long long*)&ctrl->n_collected, (unsigned long long)s_coll);
       if (s_over) atomicAdd((unsigned long long*)&ctrl->n_overflow, (unsigned long long)s_over);
+      if (pairs) atomicAdd((unsigned long long*)&ctrl->pairs, (unsigned long long)pairs);
+    }
+  }
+  if (nonfinite) atomicOr(&ctrl->nonfinite, 1u);
+}
+
+// Events of at most 32 holes (a 100 eV deposit is 26 holes): ONE WARP OWNS ONE EVENT, one hole per lane,
+// the state in registers for the event's whole life; a CTA is four such warps that never synchronise with each other.
+// With a CTA per event (k_events<1,64,12>) such an event keeps 26 of 64 threads busy and pays three block barriers per
+// step, and the per-hole FP64 update chain (Philox, Box-Muller, eq. 2) that dominates its step has one warp in two to
+// hide its latency behind.  Per step: positions to the warp's 384 bytes of shared memory as x[], y[], z[] (dead lanes
+// write the sentinel), so one LDS.64 per coordinate brings TWO consecutive sources as a packed pair; the field of lane
+// t is accumulated over source pairs with the packed FP32x2 instructions of gc_field.cuh (even sources in the low
+// half, odd in the high half, added at the end); advance_carrier as everywhere; collection by ballot, compaction by
+// __fns + shuffle (stable).  Same arithmetic per pair and per hole as k_events; only the order of the FP32 field sum
+// differs.
+__global__ void __launch_bounds__(128)
+k_events_warp(SoA A, EventTable ev, const uint32_t* __restrict__ order, uint32_t n_order, uint32_t* __restrict__ queue,
+              Ctrl* __restrict__ ctrl, Sink sink, DevParams P, uint64_t max_steps) {
+  __shared__ __align__(16) float s_pos[4][3][kEvCapMicro + 2];
+  const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+  float* sx = s_pos[warp][0];
+  float* sy = s_pos[warp][1];
+  float* sz = s_pos[warp][2];
+  const uint32_t lt = (1u << lane) - 1u;
+  const float2 eps2v = make_float2(P.eps2, P.eps2);
+  uint32_t nonfinite = 0;
+
+  for (;;) {
+    uint32_t slot = 0;
+    if (lane == 0) slot = atomicAdd(queue, 1u);
+    slot = __shfl_sync(0xffffffffu, slot, 0);
+    if (slot >= n_order) break;
+    const uint32_t e = order[slot];
+    const uint32_t off = ev.off[e];
+    uint32_t n = ev.cnt[e];
+    uint64_t step = ev.step[e];
+    if (n == 0) continue;
+    bool live = lane < n;
+    float x = 0.f, y = 0.f, z = 0.f;
+    uint32_t id = 0;
+    if (live) { x = A.x[off + lane]; y = A.y[off + lane]; z = A.z[off + lane]; id = A.id[off + lane]; }
+    uint64_t pairs = 0, done = 0;
+    uint32_t n_coll = 0, n_over = 0;
+    bool first = true;
+    for (;;) {
+      // ---- a7 + a8: bin the holes that crossed z_well, compact the survivors (stable)
+      const bool crossed = live && (double)z <= P.z_well;
+      uint32_t over = 0;
+      if (crossed) collect(x, y, z, id, step, P, sink, over);
+      n_coll += __popc(__ballot_sync(0xffffffffu, crossed));
+      n_over += __popc(__ballot_sync(0xffffffffu, over != 0u));
+      const uint32_t bal = __ballot_sync(0xffffffffu, live && !crossed);
+      const uint32_t total = __popc(bal);
+      const uint32_t src = lane < total ? __fns(bal, 0u, lane + 1u) : lane;     // lane of the (lane+1)-th survivor
+      x = __shfl_sync(0xffffffffu, x, src); y = __shfl_sync(0xffffffffu, y, src); z = __shfl_sync(0xffffffffu, z, src);
+      id = __shfl_sync(0xffffffffu, id, src);
+      live = lane < total;
+      if (!first) { step += 1; done += 1; if (!(P.flags & 1u)) pairs += (uint64_t)n * (uint64_t)n; }
+      first = false;
+      n = total;
+      if (n == 0 || done >= max_steps) break;
+
+      // ---- a1: field of lane's hole from all n sources, two sources per packed instruction
+      float2 ax = make_float2(0.f, 0.f), ay = ax, az = ax;
+      if (!(P.flags & 1u)) {                                 // GCORECCD_COULOMB_OFF
+        __syncwarp();                                        // last step's readers are done
+        sx[lane] = live ? x : kSentinel; sy[lane] = live ? y : kSentinel; sz[lane] = live ? z : kSentinel;
+        if (lane < 2) { sx[32 + lane] = kSentinel; sy[32 + lane] = kSentinel; sz[32 + lane] = kSentinel; }
+        __syncwarp();
+        const float2 ntx = make_float2(-x, -x), nty = make_float2(-y, -y), ntz = make_float2(-z, -z);
+        for (uint32_t j = 0; j < n; j += 2) {
+          const float2 px2 = *reinterpret_cast<const float2*>(sx + j), py2 = *reinterpret_cast<const float2*>(sy + j),
+                       pz2 = *reinterpret_cast<const float2*>(sz + j);
+          const float2 dx = __fadd2_rn(px2, ntx), dy = __fadd2_rn(py2, nty), dz = __fadd2_rn(pz2, ntz);
+          float2 r2 = __ffma2_rn(dx, dx, eps2v);
+          r2 = __ffma2_rn(dy, dy, r2);
+          r2 = __ffma2_rn(dz, dz, r2);
+          const float2 inv = make_float2(rsqrt_ftz(r2.x), rsqrt_ftz(r2.y));
+          float2 w = __fmul2_rn(inv, inv);
+          w = __fmul2_rn(w, inv);
+          ax = __ffma2_rn(dx, w, ax); ay = __ffma2_rn(dy, w, ay); az = __ffma2_rn(dz, w, az);
+        }
+      }
+      // ---- a2..a6
+      if (live) {
+        const double Ex = -P.Kp * (double)(ax.x + ax.y), Ey = -P.Kp * (double)(ay.x + ay.y), Ez = -P.Kp * (double)(az.x + az.y);
+        float xf, yf, zf;
+        if (!advance_carrier(x, y, z, id, step, Ex, Ey, Ez, P, xf, yf, zf)) nonfinite = 1u;
+        x = xf; y = yf; z = zf;
+      }
+    }
+    // ---- retire
+    if (live) { A.x[off + lane] = x; A.y[off + lane] = y; A.z[off + lane] = z; A.id[off + lane] = id; }
+    if (lane == 0) {
+      ev.cnt[e] = n;
+      ev.step[e] = step;
+      if (n_coll) atomicAdd((unsigned long long*)&ctrl->n_collected, (unsigned long long)n_coll);
+      if (n_over) atomicAdd((unsigned long long*)&ctrl->n_overflow, (unsigned long long)n_over);
       if (pairs) atomicAdd((unsigned long long*)&ctrl->pairs, (unsigned long long)pairs);
     }
   }

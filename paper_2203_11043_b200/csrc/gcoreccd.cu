@@ -94,15 +94,15 @@ struct gcoreccd {
     bool loaded;
     uint64_t n_events, n_carriers;        // as loaded
     uint64_t events_left, carriers_left;  // after the last run_events
-    uint32_t n_q[3];                      // events per queue: tiny, small, large (order = [tiny..., small..., large...])
+    uint32_t n_q[4];                      // events per queue: micro, tiny, small, large (order = [micro..., tiny..., ...])
     char* d_buf;                          // one allocation: off | cnt | order | queue | step
     uint32_t *d_off, *d_cnt, *d_order, *d_queue;
     uint64_t* d_step;
     uint32_t *h_off, *h_cnt;              // host mirrors
     uint64_t* h_step;
-    int grid_q[3];
-    cudaStream_t aux[2];                  // the small and tiny queues run beside the large one
-    cudaEvent_t fork, join[2];
+    int grid_q[4];
+    cudaStream_t aux[3];                  // the small, tiny and micro queues run beside the large one
+    cudaEvent_t fork, join[3];
   } evb;
 };
 
@@ -308,7 +308,7 @@ int enqueue_steps(gcoreccd_t* h, uint64_t n_steps) {
 
 void drop_events(gcoreccd_t* h) {
   if (h->evb.d_buf) cudaFree(h->evb.d_buf);
-  for (int k = 0; k < 2; ++k) {
+  for (int k = 0; k < 3; ++k) {
     if (h->evb.aux[k]) cudaStreamDestroy(h->evb.aux[k]);
     if (h->evb.join[k]) cudaEventDestroy(h->evb.join[k]);
   }
@@ -912,7 +912,7 @@ int gcoreccd_load_events(gcoreccd_t* h, const float* xyz, const uint64_t* offset
   if (e == cudaSuccess) e = cudaMemcpyAsync(zmean, B.d_order, ne * 4, cudaMemcpyDeviceToHost, h->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
   if (e != cudaSuccess) { free(order); free(zmean); drop_events(h); return fail(h, GCORECCD_ERR_CUDA, "load_events", e); }
-  // three queues (one per kernel variant), each in longest-processing-time-first order
+  // four queues (one per kernel variant), each in longest-processing-time-first order
   // estimated work of an event = n^2 x steps, steps ~ the low-field drift time from its mean depth,
   // ln(a2 / (a2 - a1 z)) (eq. 1 with constant mobility); plain z where that is undefined.  Order only: never physics.
   const uint32_t* cnt = B.h_cnt;
@@ -926,9 +926,9 @@ int gcoreccd_load_events(gcoreccd_t* h, const float* xyz, const uint64_t* offset
   }
   const float* cost = zmean;
   auto by_size = [cost](uint32_t a, uint32_t b) { return cost[a] != cost[b] ? cost[a] > cost[b] : a < b; };
-  const uint32_t lim[4] = {0u, kEvCapTiny, kEvCapSmall, kEvCapLarge};
+  const uint32_t lim[5] = {0u, kEvCapMicro, kEvCapTiny, kEvCapSmall, kEvCapLarge};
   uint32_t filled = 0;
-  for (int q = 0; q < 3; ++q) {
+  for (int q = 0; q < 4; ++q) {
     const uint32_t first = filled;
     for (size_t k = 0; k < ne; ++k)
       if ((q == 0 ? true : B.h_cnt[k] > lim[q]) && B.h_cnt[k] <= lim[q + 1]) order[filled++] = (uint32_t)k;
@@ -942,16 +942,17 @@ int gcoreccd_load_events(gcoreccd_t* h, const float* xyz, const uint64_t* offset
   if (e != cudaSuccess) { drop_events(h); return fail(h, GCORECCD_ERR_CUDA, "load_events", e); }
 
   // persistent grids: resident CTAs per SM x SM count
-  const size_t smem[3] = {event_smem_bytes(kEvCapTiny), event_smem_bytes(kEvCapSmall), event_smem_bytes(kEvCapLarge)};
-  int occ[3] = {0, 0, 0};
-  e = cudaFuncSetAttribute(k_events<4, 256, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem[2]);
-  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[0], k_events<1, 64, 12>, 64, smem[0]);
-  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[1], k_events<1, 256, 3>, 256, smem[1]);
-  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[2], k_events<4, 256, 1>, 256, smem[2]);
+  const size_t smem[4] = {0, event_smem_bytes(kEvCapTiny), event_smem_bytes(kEvCapSmall), event_smem_bytes(kEvCapLarge)};
+  int occ[4] = {0, 0, 0, 0};
+  e = cudaFuncSetAttribute(k_events<4, 256, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem[3]);
+  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[0], k_events_warp, 128, 0);
+  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[1], k_events<1, 64, 12>, 64, smem[1]);
+  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[2], k_events<1, 256, 3>, 256, smem[2]);
+  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[3], k_events<4, 256, 1>, 256, smem[3]);
   if (e != cudaSuccess) { drop_events(h); return fail(h, GCORECCD_ERR_CUDA, "load_events: kernel attributes", e); }
-  for (int q = 0; q < 3; ++q) B.grid_q[q] = h->num_sms * (occ[q] > 0 ? occ[q] : 1);
+  for (int q = 0; q < 4; ++q) B.grid_q[q] = h->num_sms * (occ[q] > 0 ? occ[q] : 1);
   e = cudaEventCreateWithFlags(&B.fork, cudaEventDisableTiming);
-  for (int k = 0; k < 2 && e == cudaSuccess; ++k) {
+  for (int k = 0; k < 3 && e == cudaSuccess; ++k) {
     e = cudaStreamCreateWithFlags(&B.aux[k], cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&B.join[k], cudaEventDisableTiming);
   }
@@ -971,33 +972,41 @@ int gcoreccd_run_events(gcoreccd_t* h, uint64_t max_steps, uint64_t* events_left
   int ret = GCORECCD_OK;
   if (B.carriers_left > 0) {
     const EventTable tab{B.d_off, B.d_cnt, B.d_step};
-    GC_CUDA(h, cudaMemsetAsync(B.d_queue, 0, 12, h->stream));
+    GC_CUDA(h, cudaMemsetAsync(B.d_queue, 0, 16, h->stream));
     // one kernel per queue, forked onto side streams so that the small events fill the SMs the large ones leave
-    const uint32_t first[3] = {0u, B.n_q[0], B.n_q[0] + B.n_q[1]};
+    const uint32_t first[4] = {0u, B.n_q[0], B.n_q[0] + B.n_q[1], B.n_q[0] + B.n_q[1] + B.n_q[2]};
     GC_CUDA(h, cudaEventRecord(B.fork, h->stream));
-    if (B.n_q[2]) {
-      const int g = (int)std::min<uint32_t>(B.n_q[2], (uint32_t)B.grid_q[2]);
-      k_events<4, 256, 1><<<g, 256, event_smem_bytes(kEvCapLarge), h->stream>>>(h->A, tab, B.d_order + first[2], B.n_q[2], B.d_queue + 2,
+    if (B.n_q[3]) {
+      const int g = (int)std::min<uint32_t>(B.n_q[3], (uint32_t)B.grid_q[3]);
+      k_events<4, 256, 1><<<g, 256, event_smem_bytes(kEvCapLarge), h->stream>>>(h->A, tab, B.d_order + first[3], B.n_q[3], B.d_queue + 3,
                                                                               h->ctrl, h->sink, h->dp, max_steps, kEvCapLarge);
       h->launches += 1;
     }
-    if (B.n_q[1]) {
+    if (B.n_q[2]) {
       GC_CUDA(h, cudaStreamWaitEvent(B.aux[0], B.fork, 0));
-      const int g = (int)std::min<uint32_t>(B.n_q[1], (uint32_t)B.grid_q[1]);
-      k_events<1, 256, 3><<<g, 256, event_smem_bytes(kEvCapSmall), B.aux[0]>>>(h->A, tab, B.d_order + first[1], B.n_q[1], B.d_queue + 1,
+      const int g = (int)std::min<uint32_t>(B.n_q[2], (uint32_t)B.grid_q[2]);
+      k_events<1, 256, 3><<<g, 256, event_smem_bytes(kEvCapSmall), B.aux[0]>>>(h->A, tab, B.d_order + first[2], B.n_q[2], B.d_queue + 2,
                                                                              h->ctrl, h->sink, h->dp, max_steps, kEvCapSmall);
       h->launches += 1;
       GC_CUDA(h, cudaEventRecord(B.join[0], B.aux[0]));
       GC_CUDA(h, cudaStreamWaitEvent(h->stream, B.join[0], 0));
     }
-    if (B.n_q[0]) {
+    if (B.n_q[1]) {
       GC_CUDA(h, cudaStreamWaitEvent(B.aux[1], B.fork, 0));
-      const int g = (int)std::min<uint32_t>(B.n_q[0], (uint32_t)B.grid_q[0]);
-      k_events<1, 64, 12><<<g, 64, event_smem_bytes(kEvCapTiny), B.aux[1]>>>(h->A, tab, B.d_order, B.n_q[0], B.d_queue, h->ctrl,
-                                                                           h->sink, h->dp, max_steps, kEvCapTiny);
+      const int g = (int)std::min<uint32_t>(B.n_q[1], (uint32_t)B.grid_q[1]);
+      k_events<1, 64, 12><<<g, 64, event_smem_bytes(kEvCapTiny), B.aux[1]>>>(h->A, tab, B.d_order + first[1], B.n_q[1], B.d_queue + 1,
+                                                                           h->ctrl, h->sink, h->dp, max_steps, kEvCapTiny);
       h->launches += 1;
       GC_CUDA(h, cudaEventRecord(B.join[1], B.aux[1]));
       GC_CUDA(h, cudaStreamWaitEvent(h->stream, B.join[1], 0));
+    }
+    if (B.n_q[0]) {                                          // one warp per event, four events per CTA
+      GC_CUDA(h, cudaStreamWaitEvent(B.aux[2], B.fork, 0));
+      const int g = (int)std::min<uint32_t>((B.n_q[0] + 3u) / 4u, (uint32_t)B.grid_q[0]);
+      k_events_warp<<<g, 128, 0, B.aux[2]>>>(h->A, tab, B.d_order, B.n_q[0], B.d_queue, h->ctrl, h->sink, h->dp, max_steps);
+      h->launches += 1;
+      GC_CUDA(h, cudaEventRecord(B.join[2], B.aux[2]));
+      GC_CUDA(h, cudaStreamWaitEvent(h->stream, B.join[2], 0));
     }
     GC_CUDA(h, cudaGetLastError());
     GC_CUDA(h, cudaMemcpyAsync(B.h_cnt, B.d_cnt, B.n_events * 4, cudaMemcpyDeviceToHost, h->stream));

@@ -250,3 +250,35 @@ def test_batch_records_final_positions_per_id():
             assert np.linalg.norm(c.mean(axis=0) - oc.mean(axis=0)) <= 4.0 * ro / np.sqrt(hi - lo) + 1e-3
             assert abs(r - ro) <= max(0.05 * ro, 4.0 * ro / np.sqrt(2.0 * (hi - lo)))
     sim.close()
+
+
+def test_warp_per_event_kernel_follows_the_oracle_to_collection_boundaries():
+    """Events of <= 32 holes run on k_events_warp (one warp per event, state in registers).  Sizes around the warp
+    width, shallow clouds so that holes are collected inside the window (ballot + __fns compaction), a partial run
+    (max_steps) followed by a second one, and a 33-hole event that must take the CTA-per-event kernel instead."""
+    sizes = [1, 2, 3, 26, 26, 31, 32, 33, 17, 0, 8]
+    w = workloads.make_events(sizes, seed=21, depth_range=(3.0, 12.0))
+    n = len(w["xyz"])
+    sim = gpu_sim(w, max_carriers=n)
+    sim.load_events(w["xyz"], w["offsets"])
+    sim.run_events(4)
+    sim.run_events(6)                                       # 10 steps in two legs: state leaves and re-enters the registers
+    act, stp = sim.events()
+    st = sim.state()
+    assert st["n_active"] + st["n_collected"] == n and st["n_active"] == int(act.sum())
+    collected_some = 0
+    for e, size in enumerate(sizes):
+        if size == 0:
+            continue
+        o, hist = _oracle_event(w, e, 10)
+        ost = o.state()
+        assert int(stp[e]) == ost["step"], (e, size)
+        collected_some += ost["n_collected"]
+        xyz, ids = sim.read_event_carriers(e)
+        assert len(ids) == int(act[e]) and np.all(np.diff(ids.astype(np.int64)) > 0)
+        _check_event(xyz, ids, o, hist, size, TRAJ_TOL)
+    assert collected_some > 0                               # the window did contain collections
+    done = sim.run_events()
+    img, over = sim.read_image()
+    assert done[1] == 0 and int(img.sum()) + over == n
+    sim.close()
