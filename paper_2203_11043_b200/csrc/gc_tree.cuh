@@ -33,7 +33,7 @@ constexpr uint32_t kFan = 8;               // children per node
 constexpr uint32_t kTreeMaxLevels = 9;     // 8 * 8^8 = 2^27 > 2^26
 constexpr uint32_t kGroup = 256;           // targets per traversal group = one level-1 node
 constexpr int kTreeTPB = 128;              // threads of k_tree_field: one packed pair of targets each
-constexpr uint32_t kFarCap = 2048, kNearCap = 1024, kFrontCap = 1024;
+constexpr uint32_t kFarCap = 1024, kNearCap = 768, kFrontCap = 2048;
 constexpr int kCPT = 2;                    // candidates per thread and batch of the walk
 constexpr uint32_t kBatch = kCPT * kTreeTPB;
 constexpr uint32_t kTopNodes = 64;         // the walk starts at the lowest level with at most this many nodes
