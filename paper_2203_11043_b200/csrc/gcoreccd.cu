@@ -471,6 +471,7 @@ int gcoreccd_reset(gcoreccd_t* h) {
   GC_CUDA(h, cudaMemsetAsync(h->ctrl, 0, sizeof(Ctrl), h->stream));
   GC_CUDA(h, cudaMemsetAsync(h->image, 0, (size_t)h->p.img_nx * h->p.img_ny * 4, h->stream));
   GC_CUDA(h, cudaMemsetAsync(h->fin, 0xff, (size_t)h->L.cap_pad * 16, h->stream));     // NaN / all-ones = still drifting
+  if (h->ff_on) GC_CUDA(h, cudaMemsetAsync(h->tree.tc, 0, sizeof(TreeCtrl), h->stream)); // far-field counters restart too
   GC_CUDA(h, cudaStreamSynchronize(h->stream));
   drop_events(h);
   h->n_loaded = 0;
@@ -839,6 +840,7 @@ int gcoreccd_debug_normals(gcoreccd_t* h, const uint32_t* id, const uint64_t* st
 // ---------------------------------------------------------------------------- batched independent events
 int gcoreccd_load_events(gcoreccd_t* h, const float* xyz, const uint64_t* offsets, uint64_t n_events, int on_device) {
   if (!h || !offsets || n_events == 0 || n_events > 0x7fffffffull) return GCORECCD_ERR_INVALID;
+  if (h->shard_world > 1) return fail(h, GCORECCD_ERR_STATE, "load_events: the handle is sharded (independent events shard as replicas)");
   const uint64_t n = offsets[n_events];
   if (offsets[0] != 0 || (!xyz && n)) return fail(h, GCORECCD_ERR_INVALID, "load_events: offsets[0] must be 0");
   for (uint64_t e = 0; e < n_events; ++e) {
