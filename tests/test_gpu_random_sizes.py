@@ -1,0 +1,70 @@
+"""Randomised sizes for the two widened paths (treecode, target sharding): ragged tails, sizes around the tile / leaf /
+group / variant boundaries, more ranks than tiles.  The reference here is the exact single-GPU CUDA path, itself pinned
+to the oracle elsewhere, so many cases stay cheap; seeds are fixed (the cases are the same every run)."""
+import numpy as np
+import pytest
+
+from paper_2203_11043_b200 import workloads
+from util import gpu_sim
+
+pytestmark = pytest.mark.gpu
+
+_rng = np.random.default_rng(20220322)
+_EDGE = [7, 8, 9, 63, 64, 65, 255, 256, 257, 511, 513, 2047, 2049, 3071, 3073, 12287, 12289, 24575, 24577]
+CASES = [(int(c), int(n)) for c, n in zip(_rng.integers(0, 4, size=len(_EDGE)), _EDGE)] + \
+        [(int(c), int(n)) for c, n in zip(_rng.integers(0, 4, size=10), _rng.integers(1, 70000, size=10))]
+
+
+@pytest.mark.parametrize("cfg,n", CASES)
+def test_treecode_theta_zero_equals_the_all_pairs_kernel(cfg, n):
+    w = workloads.make(cfg, n=n)
+    n = len(w["xyz"])                                       # multi-cloud configs round n down to whole clouds
+    sim = gpu_sim(w)
+    sim.load_carriers(w["xyz"])
+    E0 = sim.eval_field()
+    _, ids0 = sim.read_carriers()
+    sim.set_farfield(0.0, 1, 1)
+    E1 = sim.eval_field()
+    _, ids1 = sim.read_carriers()
+    assert np.array_equal(np.sort(ids1), ids0)
+    a = E1[np.argsort(ids1)].astype(np.float64)
+    b = E0.astype(np.float64)
+    scale = np.maximum(np.linalg.norm(b, axis=1), 1e-3 * np.sqrt((b ** 2).sum(axis=1).mean()) + 1e-30)
+    assert (np.linalg.norm(a - b, axis=1) / scale).max() <= 5e-5        # two FP32 summation orders of the same terms
+    # and the approximation never breaks conservation or finiteness over a few steps
+    sim.set_farfield(0.5, 2, 1)
+    sim.step(5)
+    st = sim.state()
+    img, over = sim.read_image()
+    assert int(img.sum()) + over + st["n_active"] == n
+    assert np.isfinite(sim.read_carriers()[0]).all()
+    sim.close()
+
+
+@pytest.mark.parametrize("cfg,n,G", [(c, n, int(g_)) for (c, n), g_ in zip(CASES[::2], _rng.integers(2, 9, size=len(CASES[::2])))])
+def test_sharded_steps_equal_the_single_gpu_steps(cfg, n, G):
+    import torch
+    from paper_2203_11043_b200 import binding, sharded
+    w = workloads.make(cfg, n=n)
+    n = len(w["xyz"])
+    stream = torch.cuda.Stream()
+    es = [binding.from_workload(w, stream=stream) for _ in range(G)]
+    vr = sharded.VirtualRanks(es, lambda nb: torch.empty(nb, dtype=torch.uint8, device="cuda"))
+    vr.load_carriers(w["xyz"])
+    vr.step(3)
+    ref = gpu_sim(w)
+    ref.load_carriers(w["xyz"])
+    ref.step(3)
+    a, ia = es[G - 1].read_carriers()
+    b, ib = ref.read_carriers()
+    tot, rst = vr.totals(), ref.state()
+    assert tot["step"] == rst["step"] and tot["pair_interactions"] == rst["pair_interactions"]
+    if np.array_equal(ia, ib):
+        d = np.abs(a.astype(np.float64) - b).max(axis=1)
+        assert np.median(d) <= 1e-4 and (d > 1e-3).mean() <= 0.02       # same terms, another FP32 summation split
+    else:                                                               # a hole within an ulp of the collection plane
+        assert len(np.setxor1d(ia, ib)) <= 2
+    assert tot["n_active"] + tot["n_collected"] == n
+    ref.close()
+    for e in es:
+        e.close()
