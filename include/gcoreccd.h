@@ -229,9 +229,10 @@ int gcoreccd_shard_commit(gcoreccd_t* h, const void* const* msgs_host, uint32_t 
 /* ---- Far-field approximation of eq. 6 — a VARIANT, off by default --------------------------
  * The exact path sums all N_a^2 ordered pairs.  With set_farfield(theta >= 0) step a1 is replaced by
  * a treecode: the active holes are kept in Hilbert-curve order (re-sorted every resort_every field evaluations; 0 => 4), an
- * implicit 8-ary tree of runs of 32*8^l consecutive holes carries, per node, its hole count m, centre of charge c and
- * bounding radius a; every group of 256 consecutive targets (ball (c_T, r_T)) replaces a node by ONE pseudo-hole of
- * charge m at c when  a <= theta * (|c - c_T| - r_T)  and sums all other holes exactly.  a2..a8 are unchanged.
+ * implicit 8-ary tree of runs of 8*8^l consecutive holes carries, per node, its hole count m, centre of charge c and the
+ * radius a of the ball about c holding its members; every group of 256 consecutive targets replaces a node by ONE
+ * pseudo-hole of charge m at c when  a <= theta * |x_t - c|  holds for every target t of the group, and sums all other
+ * holes exactly.  a2..a8 are unchanged.
  * Stated bound (monopole about the centre of charge; the dipole vanishes): for every target j
  *     |E_approx,j - E_exact,j|  <=  B(theta) * sum_{accepted nodes} m K' / d_j^2 ,   B = theta^2 (3 - 2 theta)/(1 - theta)^2,
  * d_j the distance from j to the node's centre; the near field is exact; theta = 0 accepts no node (exact sum in

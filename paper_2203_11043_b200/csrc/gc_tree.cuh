@@ -8,11 +8,11 @@
 //      carriers starting at k*8*8^l; a node stores its hole count m, its centre of charge c (the dipole about c
 //      vanishes) and the radius a of the smallest ball about c holding its members (computed from the CURRENT
 //      positions, so the nodes stay valid between re-sorts, only less compact);
-//   3. every 256 consecutive targets (= one level-1 node; Q_T = the union of the axis-aligned boxes of its 8 leaves) walk
-//      the tree level by level: a node is
-//      ACCEPTED when  a <= theta * D,  D = dist(c, Q_T) > 0  (every target then sees it under a/d <= theta) and
-//      enters the group's far list as one pseudo-hole of charge m at c; otherwise it is opened (its 8 children join
-//      the next level's frontier) or, at the leaf level, its 8 holes enter the near list and are summed exactly;
+//   3. every 256 consecutive targets (a "group") walk the tree level by level from the lowest level with <= 64 nodes: a
+//      node is ACCEPTED when  a <= theta * |x_t - c|  for EVERY target t of the group (decided exactly, through boxes of
+//      256 / 32 / 8 targets and then the targets themselves: tree_accept) and enters the group's far list as one
+//      pseudo-hole of charge m at c; otherwise it is opened (it joins the frontier whose children are the next level's
+//      candidates) or, at the leaf level, its 8 holes enter the near list and are summed exactly;
 //   4. the lists are consumed by the same packed FP32x2 inner loop as k_field (weighted by m for pseudo-holes).
 //
 // Error bound (stated, and checked against the FP64 oracle in tests/test_gpu_farfield.py): for one accepted node,
