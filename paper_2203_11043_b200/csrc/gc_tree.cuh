@@ -44,6 +44,7 @@ struct TreeCtrl {                          // device resident, next to the tree 
   uint32_t next_group;                     // dynamic work counter of k_tree_field
   uint32_t pad_;
   unsigned long long far_evals, near_evals;  // interactions actually evaluated (pseudo-hole and exact)
+  uint32_t tot[6][256];                    // radix sort: global digit totals of each pass (order-independent)
 };
 
 struct Tree {                              // device pointers carved from the workspace
@@ -52,7 +53,7 @@ struct Tree {                              // device pointers carved from the wo
   float* node_r;
   unsigned long long* key[2];              // radix sort double buffers: 48-bit curve keys ...
   uint32_t* val[2];                        // ... and the carrier index they came from
-  uint32_t* counts;                        // [256][blocks] digit histograms
+  uint32_t* counts;                        // [blocks][256] digit histograms
 };
 
 __host__ __device__ inline uint32_t level_size(uint32_t l) { return kLeaf << (3u * l); }
@@ -81,6 +82,8 @@ __global__ void k_tree_reset(TreeCtrl* __restrict__ tc, int reset_box) {
       for (int c = 0; c < 3; ++c) { tc->lo[c] = 0xffffffffu; tc->hi[c] = 0u; }
     }
   }
+  if (reset_box)                                            // a re-sort follows: clear the digit totals
+    for (uint32_t k = threadIdx.x; k < 6u * 256u; k += blockDim.x) (&tc->tot[0][0])[k] = 0u;
 }
 
 __global__ void __launch_bounds__(kTPB)
@@ -93,6 +96,7 @@ k_tree_bbox(const float* __restrict__ px, const float* __restrict__ py, const fl
 #pragma unroll
     for (int c = 0; c < 3; ++c) { lo[c] = min(lo[c], v[c]); hi[c] = max(hi[c], v[c]); }
   }
+  __shared__ uint32_t s_lo[3][kTPB / 32], s_hi[3][kTPB / 32];
 #pragma unroll
   for (int c = 0; c < 3; ++c) {
     lo[c] = __reduce_min_sync(0xffffffffu, lo[c]);
@@ -100,7 +104,13 @@ k_tree_bbox(const float* __restrict__ px, const float* __restrict__ py, const fl
   }
   if ((threadIdx.x & 31u) == 0) {
 #pragma unroll
-    for (int c = 0; c < 3; ++c) { atomicMin(&tc->lo[c], lo[c]); atomicMax(&tc->hi[c], hi[c]); }
+    for (int c = 0; c < 3; ++c) { s_lo[c][threadIdx.x >> 5] = lo[c]; s_hi[c][threadIdx.x >> 5] = hi[c]; }
+  }
+  __syncthreads();
+  if (threadIdx.x < 3) {                                    // one atomic pair per coordinate and CTA, not per warp
+    uint32_t a = s_lo[threadIdx.x][0], b = s_hi[threadIdx.x][0];
+    for (int w = 1; w < kTPB / 32; ++w) { a = min(a, s_lo[threadIdx.x][w]); b = max(b, s_hi[threadIdx.x][w]); }
+    atomicMin(&tc->lo[threadIdx.x], a); atomicMax(&tc->hi[threadIdx.x], b);
   }
 }
 
@@ -152,7 +162,8 @@ k_tree_keys(const float* __restrict__ px, const float* __restrict__ py, const fl
 
 // ---- LSD radix sort, 8 bits per pass, keys + values; stable ------------------------------------------------------
 __global__ void __launch_bounds__(256)
-k_radix_hist(const unsigned long long* __restrict__ key, const Ctrl* __restrict__ ctrl, uint32_t shift, uint32_t* __restrict__ counts) {
+k_radix_hist(const unsigned long long* __restrict__ key, const Ctrl* __restrict__ ctrl, uint32_t shift, uint32_t* __restrict__ counts,
+             uint32_t* __restrict__ tot) {
   __shared__ uint32_t s_h[256];
   const uint32_t n = ctrl->n_active;
   const uint32_t nb = (n + kSortBlock - 1) / kSortBlock;
@@ -165,59 +176,42 @@ k_radix_hist(const unsigned long long* __restrict__ key, const Ctrl* __restrict_
     if (i < n) atomicAdd(&s_h[(uint32_t)(key[i] >> shift) & 255u], 1u);
   }
   __syncthreads();
-  counts[threadIdx.x * nb + blockIdx.x] = s_h[threadIdx.x];
-}
-
-// exclusive scan of counts[256][nb] (digit-major), one block of 32 warps: warp w owns digit rows w, w+32, ...;
-// row sums (coalesced), a scan of the 256 row totals, then the in-row scans
-__global__ void __launch_bounds__(1024)
-k_radix_scan(const Ctrl* __restrict__ ctrl, uint32_t* __restrict__ counts) {
-  __shared__ uint32_t s_tot[256];
-  const uint32_t n = ctrl->n_active;
-  const uint32_t nb = (n + kSortBlock - 1) / kSortBlock;
-  const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
-  for (uint32_t d = warp; d < 256; d += 32) {
-    uint32_t sum = 0;
-    for (uint32_t b = lane; b < nb; b += 32) sum += counts[d * nb + b];
-    sum = __reduce_add_sync(0xffffffffu, sum);
-    if (lane == 0) s_tot[d] = sum;
-  }
-  __syncthreads();
-  if (warp == 0) {
-    uint32_t run = 0;
-    for (uint32_t d0 = 0; d0 < 256; d0 += 32) {
-      const uint32_t v = s_tot[d0 + lane];
-      uint32_t inc = v;
-      for (int o = 1; o < 32; o <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= (uint32_t)o) inc += t; }
-      s_tot[d0 + lane] = run + inc - v;
-      run += __shfl_sync(0xffffffffu, inc, 31);
-    }
-  }
-  __syncthreads();
-  for (uint32_t d = warp; d < 256; d += 32) {
-    uint32_t run = s_tot[d];
-    for (uint32_t b0 = 0; b0 < nb; b0 += 32) {
-      const uint32_t b = b0 + lane;
-      const uint32_t v = b < nb ? counts[d * nb + b] : 0u;
-      uint32_t inc = v;
-      for (int o = 1; o < 32; o <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= (uint32_t)o) inc += t; }
-      if (b < nb) counts[d * nb + b] = run + inc - v;
-      run += __shfl_sync(0xffffffffu, inc, 31);
-    }
-  }
+  counts[blockIdx.x * 256u + threadIdx.x] = s_h[threadIdx.x];             // block-major: [block][digit]
+  if (s_h[threadIdx.x]) atomicAdd(&tot[threadIdx.x], s_h[threadIdx.x]);      // integer: order-independent
 }
 
 __global__ void __launch_bounds__(256)
 k_radix_scatter(const unsigned long long* __restrict__ key_in, const uint32_t* __restrict__ val_in, unsigned long long* __restrict__ key_out,
                 uint32_t* __restrict__ val_out, const Ctrl* __restrict__ ctrl, uint32_t shift,
-                const uint32_t* __restrict__ offsets) {
+                const uint32_t* __restrict__ counts, const uint32_t* __restrict__ tot) {
   __shared__ uint32_t s_wh[8][256];       // per-warp digit counts of the current round
   __shared__ uint32_t s_run[256];         // digits already placed by this block
   const uint32_t n = ctrl->n_active;
   const uint32_t nb = (n + kSortBlock - 1) / kSortBlock;
   if (blockIdx.x >= nb) return;
   const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
-  s_run[tid] = offsets[tid * nb + blockIdx.x];
+  // where this block's keys of digit d go: (keys of smaller digits anywhere) + (keys of digit d in earlier blocks).
+  // No separate scan kernel: the digit totals come from the histogram pass, the prefix over the earlier blocks is summed
+  // here from the block-major count table.
+  {
+    const uint32_t v = tot[tid];
+    uint32_t inc = v;
+    for (int o = 1; o < 32; o <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= (uint32_t)o) inc += t; }
+    if (lane == 31) s_wh[0][warp] = inc;
+    __syncthreads();
+    uint32_t base = inc - v;
+    for (uint32_t w = 0; w < warp; ++w) base += s_wh[0][w];
+    __syncthreads();
+    uint32_t a0 = 0, a1 = 0, a2 = 0, a3 = 0;                 // thread d sums digit d over the earlier blocks: coalesced
+    uint32_t b = 0;                                         // across threads, independent loads along b
+    for (; b + 4 <= blockIdx.x; b += 4) {
+      a0 += counts[(b + 0) * 256u + tid]; a1 += counts[(b + 1) * 256u + tid];
+      a2 += counts[(b + 2) * 256u + tid]; a3 += counts[(b + 3) * 256u + tid];
+    }
+    for (; b < blockIdx.x; ++b) a0 += counts[b * 256u + tid];
+    s_run[tid] = base + a0 + a1 + a2 + a3;
+    __syncthreads();
+  }
   const uint32_t base = blockIdx.x * kSortBlock;
   for (uint32_t r = 0; r < kSortBlock / 256; ++r) {
     for (int w = 0; w < 8; ++w) s_wh[w][tid] = 0;

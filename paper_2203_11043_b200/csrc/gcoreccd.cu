@@ -165,7 +165,7 @@ int launch_tree_field(gcoreccd_t* h) {
   const Tree& T = h->tree;
   const bool sort = h->ff_age % h->ff_resort == 0;
   h->ff_age += 1;
-  k_tree_reset<<<1, 32, 0, h->stream>>>(T.tc, sort ? 1 : 0);
+  k_tree_reset<<<1, 256, 0, h->stream>>>(T.tc, sort ? 1 : 0);
   h->launches += 1;
   if (sort) {
     k_tree_bbox<<<std::min<uint32_t>(tiles, (uint32_t)h->num_sms * 4u), kTPB, 0, h->stream>>>(h->A.x, h->A.y, h->A.z, h->ctrl, T.tc);
@@ -173,14 +173,14 @@ int launch_tree_field(gcoreccd_t* h) {
     const uint32_t sb = (uint32_t)((nb + kSortBlock - 1) / kSortBlock);
     int cur = 0;
     for (uint32_t shift = 0; shift < 8 * kKeyPasses; shift += 8) {
-      k_radix_hist<<<sb, 256, 0, h->stream>>>(T.key[cur], h->ctrl, shift, T.counts);
-      k_radix_scan<<<1, 1024, 0, h->stream>>>(h->ctrl, T.counts);
-      k_radix_scatter<<<sb, 256, 0, h->stream>>>(T.key[cur], T.val[cur], T.key[cur ^ 1], T.val[cur ^ 1], h->ctrl, shift, T.counts);
+      uint32_t* tot = &T.tc->tot[shift / 8][0];
+      k_radix_hist<<<sb, 256, 0, h->stream>>>(T.key[cur], h->ctrl, shift, T.counts, tot);
+      k_radix_scatter<<<sb, 256, 0, h->stream>>>(T.key[cur], T.val[cur], T.key[cur ^ 1], T.val[cur ^ 1], h->ctrl, shift, T.counts, tot);
       cur ^= 1;
     }
     k_tree_permute<<<tiles, kTPB, 0, h->stream>>>(h->A, h->B, T.val[cur], h->ctrl);     // state B is scratch between steps
     k_tree_copy<<<tiles, kTPB, 0, h->stream>>>(h->B, h->A, h->ctrl);
-    h->launches += 4 + 3 * kKeyPasses;
+    h->launches += 4 + 2 * kKeyPasses;
   }
   const uint32_t leaves = nodes_at((uint32_t)nb, 0);
   k_tree_leaves<<<(leaves * kLeaf + kTPB - 1) / kTPB, kTPB, 0, h->stream>>>(h->A.x, h->A.y, h->A.z, h->ctrl, T.node_c, T.node_r);
@@ -432,10 +432,10 @@ int gcoreccd_create(const gcoreccd_params* p, gcoreccd_t** out) {
   if (e != cudaSuccess) { fail(h, GCORECCD_ERR_CUDA, "occupancy query", e); gcoreccd_destroy(h); return GCORECCD_ERR_CUDA; }
   h->grid_tree = h->num_sms * (occ_tree > 0 ? occ_tree : 1);
   {
-    // treecode scratch: the last 8 cap_pad floats of partial plane 0 (free while S = 1; the load paths stage at its start)
-    float* r = h->Ep + (h->L.part_cap - 8 * cp);
+    // treecode scratch: the last 10 cap_pad floats of partial plane 0 (free while S <= 8; the load paths stage at its start)
+    float* r = h->Ep + (h->L.part_cap - 10 * cp);
     Tree& T = h->tree;
-    T.tc = (TreeCtrl*)r;                         r += 64;
+    T.tc = (TreeCtrl*)r;                         r += 2048;                 // 6.2 KB: box, counters, digit totals
     T.node_c = (float4*)r;                       r += cp * 5 / 8 + 64;      // <= cp/7 + 9 nodes of 4 floats
     T.node_r = r;                                r += cp * 3 / 16 + 64;
     T.key[0] = (unsigned long long*)r; r += 2 * cp;  T.key[1] = (unsigned long long*)r; r += 2 * cp;
