@@ -54,6 +54,23 @@ Layout make_layout(uint64_t max_carriers, int32_t nx, int32_t ny) {
 
 }  // namespace
 
+// Batched events: one kernel variant ("tier") per event size, so that the threads of a CTA are mostly busy:
+// tier 0 one WARP per event (k_events_warp), tiers 1..4 one CTA of 32/64/128/256 threads with one packed pair of
+// targets per thread, tier 5 256 threads with four pairs per thread.
+constexpr int kEvTiers = 6;
+constexpr uint32_t kEvTierCap[kEvTiers] = {kEvCapMicro, 64u, kEvCapTiny, 256u, kEvCapSmall, kEvCapLarge};
+constexpr int kEvTierThreads[kEvTiers] = {128, 32, 64, 128, 256, 256};
+using EvKernel = void (*)(SoA, EventTable, const uint32_t*, uint32_t, uint32_t*, Ctrl*, Sink, DevParams, uint64_t, uint32_t);
+inline EvKernel ev_kernel(int tier) {
+  switch (tier) {
+    case 1: return k_events<1, 32, 16>;
+    case 2: return k_events<1, 64, 12>;
+    case 3: return k_events<1, 128, 6>;
+    case 4: return k_events<1, 256, 3>;
+    default: return k_events<4, 256, 1>;
+  }
+}
+
 struct gcoreccd {
   gcoreccd_params p;
   DevParams dp;
@@ -94,15 +111,15 @@ struct gcoreccd {
     bool loaded;
     uint64_t n_events, n_carriers;        // as loaded
     uint64_t events_left, carriers_left;  // after the last run_events
-    uint32_t n_q[4];                      // events per queue: micro, tiny, small, large (order = [micro..., tiny..., ...])
+    uint32_t n_q[kEvTiers];               // events per queue, smallest tier first (order = [tier 0..., tier 1..., ...])
     char* d_buf;                          // one allocation: off | cnt | order | queue | step
     uint32_t *d_off, *d_cnt, *d_order, *d_queue;
     uint64_t* d_step;
     uint32_t *h_off, *h_cnt;              // host mirrors
     uint64_t* h_step;
-    int grid_q[4];
-    cudaStream_t aux[3];                  // the small, tiny and micro queues run beside the large one
-    cudaEvent_t fork, join[3];
+    int grid_q[kEvTiers];
+    cudaStream_t aux[kEvTiers - 1];       // the smaller tiers run beside the largest one
+    cudaEvent_t fork, join[kEvTiers - 1];
   } evb;
 };
 
@@ -308,7 +325,7 @@ int enqueue_steps(gcoreccd_t* h, uint64_t n_steps) {
 
 void drop_events(gcoreccd_t* h) {
   if (h->evb.d_buf) cudaFree(h->evb.d_buf);
-  for (int k = 0; k < 3; ++k) {
+  for (int k = 0; k < kEvTiers - 1; ++k) {
     if (h->evb.aux[k]) cudaStreamDestroy(h->evb.aux[k]);
     if (h->evb.join[k]) cudaEventDestroy(h->evb.join[k]);
   }
@@ -914,7 +931,7 @@ int gcoreccd_load_events(gcoreccd_t* h, const float* xyz, const uint64_t* offset
   if (e == cudaSuccess) e = cudaMemcpyAsync(zmean, B.d_order, ne * 4, cudaMemcpyDeviceToHost, h->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
   if (e != cudaSuccess) { free(order); free(zmean); drop_events(h); return fail(h, GCORECCD_ERR_CUDA, "load_events", e); }
-  // four queues (one per kernel variant), each in longest-processing-time-first order
+  // one queue per tier (kernel variant), each in longest-processing-time-first order
   // estimated work of an event = n^2 x steps, steps ~ the low-field drift time from its mean depth,
   // ln(a2 / (a2 - a1 z)) (eq. 1 with constant mobility); plain z where that is undefined.  Order only: never physics.
   const uint32_t* cnt = B.h_cnt;
@@ -928,12 +945,11 @@ int gcoreccd_load_events(gcoreccd_t* h, const float* xyz, const uint64_t* offset
   }
   const float* cost = zmean;
   auto by_size = [cost](uint32_t a, uint32_t b) { return cost[a] != cost[b] ? cost[a] > cost[b] : a < b; };
-  const uint32_t lim[5] = {0u, kEvCapMicro, kEvCapTiny, kEvCapSmall, kEvCapLarge};
   uint32_t filled = 0;
-  for (int q = 0; q < 4; ++q) {
+  for (int q = 0; q < kEvTiers; ++q) {
     const uint32_t first = filled;
     for (size_t k = 0; k < ne; ++k)
-      if ((q == 0 ? true : B.h_cnt[k] > lim[q]) && B.h_cnt[k] <= lim[q + 1]) order[filled++] = (uint32_t)k;
+      if ((q == 0 ? true : B.h_cnt[k] > kEvTierCap[q - 1]) && B.h_cnt[k] <= kEvTierCap[q]) order[filled++] = (uint32_t)k;
     if (q > 0) std::sort(order + first, order + filled, by_size);
     else if (filled > first) {
       // <= 32-hole events come in tens of thousands: a 64-bucket counting sort by estimated work (O(n)) keeps the
@@ -956,17 +972,15 @@ int gcoreccd_load_events(gcoreccd_t* h, const float* xyz, const uint64_t* offset
   if (e != cudaSuccess) { drop_events(h); return fail(h, GCORECCD_ERR_CUDA, "load_events", e); }
 
   // persistent grids: resident CTAs per SM x SM count
-  const size_t smem[4] = {0, event_smem_bytes(kEvCapTiny), event_smem_bytes(kEvCapSmall), event_smem_bytes(kEvCapLarge)};
-  int occ[4] = {0, 0, 0, 0};
-  e = cudaFuncSetAttribute(k_events<4, 256, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem[3]);
-  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[0], k_events_warp, 128, 0);
-  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[1], k_events<1, 64, 12>, 64, smem[1]);
-  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[2], k_events<1, 256, 3>, 256, smem[2]);
-  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[3], k_events<4, 256, 1>, 256, smem[3]);
+  int occ[kEvTiers] = {0};
+  e = cudaFuncSetAttribute(k_events<4, 256, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)event_smem_bytes(kEvCapLarge));
+  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[0], k_events_warp, kEvTierThreads[0], 0);
+  for (int q = 1; q < kEvTiers && e == cudaSuccess; ++q)
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[q], ev_kernel(q), kEvTierThreads[q], event_smem_bytes(kEvTierCap[q]));
   if (e != cudaSuccess) { drop_events(h); return fail(h, GCORECCD_ERR_CUDA, "load_events: kernel attributes", e); }
-  for (int q = 0; q < 4; ++q) B.grid_q[q] = h->num_sms * (occ[q] > 0 ? occ[q] : 1);
+  for (int q = 0; q < kEvTiers; ++q) B.grid_q[q] = h->num_sms * (occ[q] > 0 ? occ[q] : 1);
   e = cudaEventCreateWithFlags(&B.fork, cudaEventDisableTiming);
-  for (int k = 0; k < 3 && e == cudaSuccess; ++k) {
+  for (int k = 0; k < kEvTiers - 1 && e == cudaSuccess; ++k) {
     e = cudaStreamCreateWithFlags(&B.aux[k], cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&B.join[k], cudaEventDisableTiming);
   }
@@ -986,41 +1000,31 @@ int gcoreccd_run_events(gcoreccd_t* h, uint64_t max_steps, uint64_t* events_left
   int ret = GCORECCD_OK;
   if (B.carriers_left > 0) {
     const EventTable tab{B.d_off, B.d_cnt, B.d_step};
-    GC_CUDA(h, cudaMemsetAsync(B.d_queue, 0, 16, h->stream));
-    // one kernel per queue, forked onto side streams so that the small events fill the SMs the large ones leave
-    const uint32_t first[4] = {0u, B.n_q[0], B.n_q[0] + B.n_q[1], B.n_q[0] + B.n_q[1] + B.n_q[2]};
+    GC_CUDA(h, cudaMemsetAsync(B.d_queue, 0, 4 * kEvTiers, h->stream));
+    // one kernel per tier, the largest on the handle's stream, the others forked onto side streams so that the small
+    // events fill the SMs the large ones leave
+    uint32_t first[kEvTiers];
+    first[0] = 0;
+    for (int q = 1; q < kEvTiers; ++q) first[q] = first[q - 1] + B.n_q[q - 1];
     GC_CUDA(h, cudaEventRecord(B.fork, h->stream));
-    if (B.n_q[3]) {
-      const int g = (int)std::min<uint32_t>(B.n_q[3], (uint32_t)B.grid_q[3]);
-      k_events<4, 256, 1><<<g, 256, event_smem_bytes(kEvCapLarge), h->stream>>>(h->A, tab, B.d_order + first[3], B.n_q[3], B.d_queue + 3,
-                                                                              h->ctrl, h->sink, h->dp, max_steps, kEvCapLarge);
+    for (int q = kEvTiers - 1; q >= 0; --q) {
+      if (!B.n_q[q]) continue;
+      const bool side = q < kEvTiers - 1;
+      cudaStream_t st = side ? B.aux[q] : h->stream;
+      if (side) GC_CUDA(h, cudaStreamWaitEvent(st, B.fork, 0));
+      if (q == 0) {                                           // one warp per event, four events per CTA
+        const int g = (int)std::min<uint32_t>((B.n_q[0] + 3u) / 4u, (uint32_t)B.grid_q[0]);
+        k_events_warp<<<g, kEvTierThreads[0], 0, st>>>(h->A, tab, B.d_order, B.n_q[0], B.d_queue, h->ctrl, h->sink, h->dp, max_steps);
+      } else {
+        const int g = (int)std::min<uint32_t>(B.n_q[q], (uint32_t)B.grid_q[q]);
+        ev_kernel(q)<<<g, kEvTierThreads[q], event_smem_bytes(kEvTierCap[q]), st>>>(h->A, tab, B.d_order + first[q], B.n_q[q], B.d_queue + q,
+                                                                                     h->ctrl, h->sink, h->dp, max_steps, kEvTierCap[q]);
+      }
       h->launches += 1;
-    }
-    if (B.n_q[2]) {
-      GC_CUDA(h, cudaStreamWaitEvent(B.aux[0], B.fork, 0));
-      const int g = (int)std::min<uint32_t>(B.n_q[2], (uint32_t)B.grid_q[2]);
-      k_events<1, 256, 3><<<g, 256, event_smem_bytes(kEvCapSmall), B.aux[0]>>>(h->A, tab, B.d_order + first[2], B.n_q[2], B.d_queue + 2,
-                                                                             h->ctrl, h->sink, h->dp, max_steps, kEvCapSmall);
-      h->launches += 1;
-      GC_CUDA(h, cudaEventRecord(B.join[0], B.aux[0]));
-      GC_CUDA(h, cudaStreamWaitEvent(h->stream, B.join[0], 0));
-    }
-    if (B.n_q[1]) {
-      GC_CUDA(h, cudaStreamWaitEvent(B.aux[1], B.fork, 0));
-      const int g = (int)std::min<uint32_t>(B.n_q[1], (uint32_t)B.grid_q[1]);
-      k_events<1, 64, 12><<<g, 64, event_smem_bytes(kEvCapTiny), B.aux[1]>>>(h->A, tab, B.d_order + first[1], B.n_q[1], B.d_queue + 1,
-                                                                           h->ctrl, h->sink, h->dp, max_steps, kEvCapTiny);
-      h->launches += 1;
-      GC_CUDA(h, cudaEventRecord(B.join[1], B.aux[1]));
-      GC_CUDA(h, cudaStreamWaitEvent(h->stream, B.join[1], 0));
-    }
-    if (B.n_q[0]) {                                          // one warp per event, four events per CTA
-      GC_CUDA(h, cudaStreamWaitEvent(B.aux[2], B.fork, 0));
-      const int g = (int)std::min<uint32_t>((B.n_q[0] + 3u) / 4u, (uint32_t)B.grid_q[0]);
-      k_events_warp<<<g, 128, 0, B.aux[2]>>>(h->A, tab, B.d_order, B.n_q[0], B.d_queue, h->ctrl, h->sink, h->dp, max_steps);
-      h->launches += 1;
-      GC_CUDA(h, cudaEventRecord(B.join[2], B.aux[2]));
-      GC_CUDA(h, cudaStreamWaitEvent(h->stream, B.join[2], 0));
+      if (side) {
+        GC_CUDA(h, cudaEventRecord(B.join[q], st));
+        GC_CUDA(h, cudaStreamWaitEvent(h->stream, B.join[q], 0));
+      }
     }
     GC_CUDA(h, cudaGetLastError());
     GC_CUDA(h, cudaMemcpyAsync(B.h_cnt, B.d_cnt, B.n_events * 4, cudaMemcpyDeviceToHost, h->stream));
