@@ -21,6 +21,7 @@
 #include "gc_common.cuh"
 #include "gc_field.cuh"
 #include "gc_integrate.cuh"
+#include <cooperative_groups.h>
 
 namespace gc {
 
@@ -222,6 +223,142 @@ k_events(SoA A, EventTable ev, const uint32_t* __restrict__ order, uint32_t n_or
   }
   if (nonfinite) atomicOr(&ctrl->nonfinite, 1u);
 }
+
+// FEW LARGE EVENTS: with one CTA per event and about as many events as SMs, the batch takes as long as its deepest
+// event while the SMs of the shallow ones idle (148 x 4,096 holes: 26 % of FP32 peak).  Here a thread-block CLUSTER of
+// CL CTAs (CL SMs) owns one event: every CTA keeps the whole state in its own shared memory (the field loop needs all
+// sources locally), the passes of 2*NPACK*TPB targets are dealt round-robin to the CTAs, and after the update each CTA
+// pulls the other CTAs' new positions through distributed shared memory (two cluster barriers per step).  Collection
+// and compaction are repeated identically in every CTA (O(n), cheap); only rank 0 touches the image, the records and
+// the counters.  Same arithmetic per pair and per hole as k_events.
+template <int NPACK, int TPB, int CL>
+__global__ void __launch_bounds__(TPB, 1)
+k_events_cluster(SoA A, EventTable ev, const uint32_t* __restrict__ order, uint32_t n_order, uint32_t* __restrict__ queue,
+                 Ctrl* __restrict__ ctrl, Sink sink, DevParams P, uint64_t max_steps, uint32_t cap) {
+  namespace cg = cooperative_groups;
+  cg::cluster_group cluster = cg::this_cluster();
+  const uint32_t rank = cluster.block_rank();
+  extern __shared__ __align__(16) unsigned char smem[];
+  float4* s_xy = reinterpret_cast<float4*>(smem);                       // (x,x,y,y), cap + 4 entries
+  float4* s_next = s_xy + (cap + 4);                                    // (x',y',z',id), cap entries
+  float2* s_z = reinterpret_cast<float2*>(s_next + cap);                // (z,z), cap + 4 entries
+  uint32_t* s_id = reinterpret_cast<uint32_t*>(s_z + (cap + 4));        // cap entries
+  __shared__ uint32_t s_warp[TPB / 32];
+  __shared__ uint32_t s_ev, s_coll, s_over;
+
+  const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+  constexpr uint32_t kPass = 2u * NPACK * TPB;                          // targets per pass
+  uint32_t nonfinite = 0;
+
+  for (;;) {
+    cluster.sync();                                                     // previous event fully retired, in every CTA
+    if (tid == 0) {
+      s_coll = 0; s_over = 0;
+      if (rank == 0) {
+        const uint32_t v = atomicAdd(queue, 1u);
+        for (uint32_t r = 0; r < CL; ++r) *cluster.map_shared_rank(&s_ev, r) = v;
+      }
+    }
+    cluster.sync();
+    if (s_ev >= n_order) break;
+    const uint32_t e = order[s_ev];
+    const uint32_t off = ev.off[e];
+    uint32_t n = ev.cnt[e];
+    uint64_t step = ev.step[e];
+    if (n == 0) continue;
+    for (uint32_t i = tid; i < n; i += TPB)
+      s_next[i] = make_float4(A.x[off + i], A.y[off + i], A.z[off + i], __uint_as_float(A.id[off + i]));
+    __syncthreads();
+
+    uint64_t pairs = 0, done = 0;
+    bool first = true;
+    for (;;) {
+      // ---- a7 + a8: bin the holes that crossed z_well, compact the survivors (stable) into the field layout
+      const uint32_t per = (n + TPB - 1) / TPB;
+      const uint32_t lo = min(tid * per, n), hi = min(lo + per, n);
+      uint32_t keep = 0, coll = 0, over = 0;
+      for (uint32_t i = lo; i < hi; ++i) {
+        const float4 c = s_next[i];
+        if ((double)c.z <= P.z_well) { coll += 1; if (rank == 0) collect(c.x, c.y, c.z, __float_as_uint(c.w), step, P, sink, over); }
+        else keep += 1;
+      }
+      uint32_t incl = keep;                                             // block exclusive scan of the survivor counts
+      for (int o = 1; o < 32; o <<= 1) { const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o); if ((int)lane >= o) incl += v; }
+      if (lane == 31) s_warp[warp] = incl;
+      const uint32_t wc = __reduce_add_sync(0xffffffffu, coll), wo = __reduce_add_sync(0xffffffffu, over);
+      if (lane == 0 && wc) { atomicAdd(&s_coll, wc); if (wo) atomicAdd(&s_over, wo); }
+      __syncthreads();
+      uint32_t base = 0, total = 0;
+#pragma unroll
+      for (int w = 0; w < TPB / 32; ++w) { const uint32_t v = s_warp[w]; if (w < (int)warp) base += v; total += v; }
+      uint32_t o = base + incl - keep;
+      for (uint32_t i = lo; i < hi; ++i) {
+        const float4 c = s_next[i];
+        if ((double)c.z > P.z_well) {
+          s_xy[o] = make_float4(c.x, c.x, c.y, c.y); s_z[o] = make_float2(c.z, c.z); s_id[o] = __float_as_uint(c.w);
+          ++o;
+        }
+      }
+      if (tid < 4) {                                                    // sentinels up to the unroll factor
+        const uint32_t k = total + tid;
+        if (k < ((total + 3u) & ~3u)) { s_xy[k] = make_float4(kSentinel, kSentinel, kSentinel, kSentinel); s_z[k] = make_float2(kSentinel, kSentinel); }
+      }
+      if (!first) { step += 1; done += 1; if (!(P.flags & 1u)) pairs += (uint64_t)n * (uint64_t)n; }
+      first = false;
+      n = total;
+      __syncthreads();
+      if (n == 0 || done >= max_steps) break;
+
+      // ---- a1..a6: field of every hole of the event, then its Euler-Maruyama update, into s_next
+      // pass size: an even split of the event over the CTAs, in whole packs of 2 TPB targets, at most kPass
+      const uint32_t pass_sz = min(kPass, max(2u * TPB, (((n + CL - 1u) / CL + 2u * TPB - 1u) / (2u * TPB)) * (2u * TPB)));
+      for (uint32_t base_i = 0, pass = 0; base_i < n; base_i += pass_sz, ++pass) {
+        if (pass % CL != rank) continue;                                  // another CTA of the cluster owns this pass
+        // Pack p covers targets [base_i + p 2TPB, +2TPB): thread t takes t and t + hs of it.  hs = TPB except in the
+        // last live pack, where it shrinks to half the remaining targets (rounded up to a warp), so that both lanes
+        // of the packed arithmetic stay busy and an event of <= 32 holes puts one hole on each thread of one warp.
+        const uint32_t i_first = base_i + tid;
+        const uint32_t m = min(n - base_i, pass_sz);
+        const uint32_t p_last = (m - 1u) / (2u * TPB);
+        const uint32_t m_last = m - p_last * (2u * TPB);
+        const uint32_t hs_last = min((uint32_t)TPB, max(32u, (((m_last + 1u) >> 1) + 31u) & ~31u));
+        const uint32_t np = p_last + ((warp * 32u < hs_last) ? 1u : 0u);   // packs with a live target in this warp (uniform)
+        if (np == 0) continue;
+        if constexpr (NPACK == 1) {
+          event_pass<1, TPB>(s_xy, s_z, s_id, s_next, n, i_first, p_last, hs_last, step, P, nonfinite);
+        } else {
+          if (np == 1) event_pass<1, TPB>(s_xy, s_z, s_id, s_next, n, i_first, p_last, hs_last, step, P, nonfinite);
+          else if (np == 2) event_pass<2, TPB>(s_xy, s_z, s_id, s_next, n, i_first, p_last, hs_last, step, P, nonfinite);
+          else if (np == 3) event_pass<3, TPB>(s_xy, s_z, s_id, s_next, n, i_first, p_last, hs_last, step, P, nonfinite);
+          else event_pass<4, TPB>(s_xy, s_z, s_id, s_next, n, i_first, p_last, hs_last, step, P, nonfinite);
+        }
+      }
+      cluster.sync();                                                     // every CTA's new positions are in its s_next
+      for (uint32_t base_i = 0, pass = 0; base_i < n; base_i += pass_sz, ++pass) {
+        if (pass % CL == rank) continue;
+        const float4* remote = cluster.map_shared_rank(s_next, pass % CL);
+        const uint32_t hi_i = min(base_i + pass_sz, n);
+        for (uint32_t i = base_i + tid; i < hi_i; i += TPB) s_next[i] = remote[i];
+      }
+      cluster.sync();                                                     // all pulls done before any s_next is rewritten
+    }
+
+    // ---- retire (rank 0): survivors (if max_steps stopped the event early) back to the state arrays, counters out
+    if (rank != 0) continue;
+    for (uint32_t i = tid; i < n; i += TPB) {
+      A.x[off + i] = s_xy[i].x; A.y[off + i] = s_xy[i].z; A.z[off + i] = s_z[i].x; A.id[off + i] = s_id[i];
+    }
+    if (tid == 0) {
+      ev.cnt[e] = n;
+      ev.step[e] = step;
+      if (s_coll) atomicAdd((unsigned long long*)&ctrl->n_collected, (unsigned long long)s_coll);
+      if (s_over) atomicAdd((unsigned long long*)&ctrl->n_overflow, (unsigned long long)s_over);
+      if (pairs) atomicAdd((unsigned long long*)&ctrl->pairs, (unsigned long long)pairs);
+    }
+  }
+  if (nonfinite) atomicOr(&ctrl->nonfinite, 1u);
+}
+
 
 // Events of at most 32 holes (a 100 eV deposit is 26 holes): ONE WARP OWNS ONE EVENT, one hole per lane,
 // the state in registers for the event's whole life; a CTA is four such warps that never synchronise with each other.

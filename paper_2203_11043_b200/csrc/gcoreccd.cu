@@ -60,6 +60,7 @@ Layout make_layout(uint64_t max_carriers, int32_t nx, int32_t ny) {
 constexpr int kEvTiers = 6;
 constexpr uint32_t kEvTierCap[kEvTiers] = {kEvCapMicro, 64u, kEvCapTiny, 256u, kEvCapSmall, kEvCapLarge};
 constexpr int kEvTierThreads[kEvTiers] = {128, 32, 64, 128, 256, 256};
+constexpr uint32_t kEvClusterFewFactor = 3;  // "few" = at most this many large events per SM
 using EvKernel = void (*)(SoA, EventTable, const uint32_t*, uint32_t, uint32_t*, Ctrl*, Sink, DevParams, uint64_t, uint32_t);
 inline EvKernel ev_kernel(int tier) {
   switch (tier) {
@@ -974,6 +975,10 @@ int gcoreccd_load_events(gcoreccd_t* h, const float* xyz, const uint64_t* offset
   // persistent grids: resident CTAs per SM x SM count
   int occ[kEvTiers] = {0};
   e = cudaFuncSetAttribute(k_events<4, 256, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)event_smem_bytes(kEvCapLarge));
+  if (e == cudaSuccess)
+    e = cudaFuncSetAttribute(k_events_cluster<4, 256, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)event_smem_bytes(kEvCapLarge));
+  if (e == cudaSuccess)
+    e = cudaFuncSetAttribute(k_events_cluster<4, 256, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)event_smem_bytes(kEvCapLarge));
   if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[0], k_events_warp, kEvTierThreads[0], 0);
   for (int q = 1; q < kEvTiers && e == cudaSuccess; ++q)
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[q], ev_kernel(q), kEvTierThreads[q], event_smem_bytes(kEvTierCap[q]));
@@ -1015,6 +1020,24 @@ int gcoreccd_run_events(gcoreccd_t* h, uint64_t max_steps, uint64_t* events_left
       if (q == 0) {                                           // one warp per event, four events per CTA
         const int g = (int)std::min<uint32_t>((B.n_q[0] + 3u) / 4u, (uint32_t)B.grid_q[0]);
         k_events_warp<<<g, kEvTierThreads[0], 0, st>>>(h->A, tab, B.d_order, B.n_q[0], B.d_queue, h->ctrl, h->sink, h->dp, max_steps);
+      } else if (q == kEvTiers - 1 && B.n_q[q] <= kEvClusterFewFactor * (uint32_t)h->num_sms) {
+        // few large events: a cluster of 2 CTAs per event, 4 when there are not even enough events for that
+        // (gc_events.cuh: k_events_cluster)
+        const uint32_t cl = (B.n_q[q] * 2u <= (uint32_t)h->num_sms) ? 4u : 2u;
+        const uint32_t clusters = std::min<uint32_t>(B.n_q[q], (uint32_t)h->num_sms / cl);
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(clusters * cl); cfg.blockDim = dim3(256);
+        cfg.dynamicSmemBytes = event_smem_bytes(kEvCapLarge); cfg.stream = st;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = cl; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        if (cl == 4)
+          GC_CUDA(h, cudaLaunchKernelEx(&cfg, k_events_cluster<4, 256, 4>, h->A, tab, (const uint32_t*)(B.d_order + first[q]), B.n_q[q],
+                                        B.d_queue + q, h->ctrl, h->sink, h->dp, max_steps, kEvCapLarge));
+        else
+          GC_CUDA(h, cudaLaunchKernelEx(&cfg, k_events_cluster<4, 256, 2>, h->A, tab, (const uint32_t*)(B.d_order + first[q]), B.n_q[q],
+                                        B.d_queue + q, h->ctrl, h->sink, h->dp, max_steps, kEvCapLarge));
       } else {
         const int g = (int)std::min<uint32_t>(B.n_q[q], (uint32_t)B.grid_q[q]);
         ev_kernel(q)<<<g, kEvTierThreads[q], event_smem_bytes(kEvTierCap[q]), st>>>(h->A, tab, B.d_order + first[q], B.n_q[q], B.d_queue + q,

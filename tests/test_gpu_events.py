@@ -301,3 +301,30 @@ def test_every_tier_boundary_follows_the_oracle():
         assert len(ids) == int(act[e]) and np.all(np.diff(ids.astype(np.int64)) > 0)
         _check_event(xyz, ids, o, hist, size, TRAJ_TOL)
     sim.close()
+
+
+def test_cluster_per_event_kernel_follows_the_oracle():
+    """Few large events (at most 3 per SM in the > 512-hole tier) run on k_events_cluster: a thread-block cluster of two
+    CTAs per event, new positions exchanged through distributed shared memory.  Sizes that split into one, two and
+    uneven passes per CTA; 10 steps against the per-event oracle, then to collection with exact conservation."""
+    sizes = [513, 1024, 1025, 2048, 2049, 3000, 4096, 700]
+    w = workloads.make_events(sizes, seed=44)
+    n = len(w["xyz"])
+    sim = gpu_sim(w, max_carriers=n)
+    sim.load_events(w["xyz"], w["offsets"])
+    sim.run_events(3)
+    sim.run_events(7)
+    act, stp = sim.events()
+    for e, size in enumerate(sizes):
+        o, hist = _oracle_event(w, e, 10)
+        assert int(stp[e]) == o.state()["step"], (e, size)
+        xyz, ids = sim.read_event_carriers(e)
+        assert len(ids) == int(act[e]) and np.all(np.diff(ids.astype(np.int64)) > 0)
+        _check_event(xyz, ids, o, hist, size, TRAJ_TOL)
+    ev_left, ca_left, rc = sim.run_events()
+    img, over = sim.read_image()
+    st = sim.state()
+    assert ca_left == 0 and int(img.sum()) + over == n and st["n_collected"] == n
+    xyz_f, step_f = sim.read_collected()
+    assert np.all(step_f != 0xFFFFFFFF) and np.isfinite(xyz_f).all()          # every hole recorded exactly once (rank 0)
+    sim.close()
