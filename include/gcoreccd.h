@@ -138,8 +138,9 @@ int gcoreccd_eval_field(gcoreccd_t* h, float* Exyz_V_per_cm, uint64_t cap, int o
  * holes repel each other only inside their own event, and its GPU is under-utilised below ~1e3 holes
  * (PAPER.md:92).  A batch runs every event exactly as if it had been loaded alone into a fresh handle with the
  * same parameters (same eq. 6 sum over the event's own holes, same a2..a8, same Philox stream keyed by
- * (seed, carrier id, the EVENT's step index)), but all events advance concurrently: one thread block owns one
- * event for its whole life, with the state in shared memory.  All events share the handle's image, counters and
+ * (seed, carrier id, the EVENT's step index)), but all events advance concurrently: one warp (<= 32 holes), one
+ * thread block, or - when there are few large events - one cluster of 2 or 4 thread blocks owns one event for its whole
+ * life, with the state in registers / shared memory.  All events share the handle's image, counters and
  * pair_interactions (sum over events and steps of n_event^2).
  *
  * load_events: event e owns carriers [event_offsets[e], event_offsets[e+1]) of xyz_um (interleaved x,y,z FP32,
