@@ -301,7 +301,8 @@ def run_ours(args):
     if not args.no_event and rank == 0:
         batched = []
         for sizes, what in (([2048] * 592, "592 X-ray events x 2,048 holes (7.5 keV-like clouds, sigma 0.5 um, depth U[10,665] um)"),
-                            ([26] * 44400, "44,400 X-ray events x 26 holes (100 eV, PAPER.md:106)")):
+                            ([26] * 44400, "44,400 X-ray events x 26 holes (100 eV, PAPER.md:106)"),
+                            ([4096] * 148, "148 events x 4,096 holes (few large events: one thread-block cluster per event)")):
             we = workloads.make_events(sizes)
             ne = len(we["xyz"])
             bs = binding.from_workload(we, max_carriers=ne, stream=stream)
