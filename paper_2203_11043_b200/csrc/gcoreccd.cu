@@ -56,10 +56,12 @@ Layout make_layout(uint64_t max_carriers, int32_t nx, int32_t ny) {
 
 // Batched events: one kernel variant ("tier") per event size, so that the threads of a CTA are mostly busy:
 // tier 0 one WARP per event (k_events_warp), tiers 1..4 one CTA of 32/64/128/256 threads with one packed pair of
-// targets per thread, tier 5 256 threads with four pairs per thread.
-constexpr int kEvTiers = 6;
-constexpr uint32_t kEvTierCap[kEvTiers] = {kEvCapMicro, 64u, kEvCapTiny, 256u, kEvCapSmall, kEvCapLarge};
-constexpr int kEvTierThreads[kEvTiers] = {128, 32, 64, 128, 256, 256};
+// targets per thread, tier 5 (<= 768 holes) 256 threads with two pairs per thread and shared memory sized so that two events share
+// an SM (measured: 600-hole events 1,502 -> 1,883 G pairs/s; at 1,000 holes the big tier is faster), tier 6 256
+// threads with four pairs per thread.
+constexpr int kEvTiers = 7;
+constexpr uint32_t kEvTierCap[kEvTiers] = {kEvCapMicro, 64u, kEvCapTiny, 256u, kEvCapSmall, 768u, kEvCapLarge};
+constexpr int kEvTierThreads[kEvTiers] = {128, 32, 64, 128, 256, 256, 256};
 constexpr uint32_t kEvClusterFewFactor = 3;  // "few" = at most this many large events per SM
 using EvKernel = void (*)(SoA, EventTable, const uint32_t*, uint32_t, uint32_t*, Ctrl*, Sink, DevParams, uint64_t, uint32_t);
 inline EvKernel ev_kernel(int tier) {
@@ -68,6 +70,7 @@ inline EvKernel ev_kernel(int tier) {
     case 2: return k_events<1, 64, 12>;
     case 3: return k_events<1, 128, 6>;
     case 4: return k_events<1, 256, 3>;
+    case 5: return k_events<2, 256, 2>;          // <= 768 holes: 34 KB of shared memory, two CTAs per SM (registers)
     default: return k_events<4, 256, 1>;
   }
 }
@@ -975,6 +978,7 @@ int gcoreccd_load_events(gcoreccd_t* h, const float* xyz, const uint64_t* offset
   // persistent grids: resident CTAs per SM x SM count
   int occ[kEvTiers] = {0};
   e = cudaFuncSetAttribute(k_events<4, 256, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)event_smem_bytes(kEvCapLarge));
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_events<2, 256, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)event_smem_bytes(2048u));
   if (e == cudaSuccess)
     e = cudaFuncSetAttribute(k_events_cluster<4, 256, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)event_smem_bytes(kEvCapLarge));
   if (e == cudaSuccess)

@@ -285,16 +285,17 @@ def test_warp_per_event_kernel_follows_the_oracle_to_collection_boundaries():
 
 
 def test_every_tier_boundary_follows_the_oracle():
-    """One event on each side of every tier limit (32 | 64 | 128 | 256 | 512 holes: warp kernel, then CTAs of 32, 64,
-    128, 256 threads, then four pairs per thread), 10 steps against the per-event oracle."""
-    sizes = [32, 33, 64, 65, 128, 129, 256, 257, 512, 513]
+    """One event on each side of every tier limit (32 | 64 | 128 | 256 | 512 | 768 holes: warp kernel, then CTAs of 32,
+    64, 128, 256 threads, then two and four pairs per thread; enough events above 512 holes (> 3 per SM) that the
+    CTA-per-event kernels, not the cluster kernel, take them), 10 steps against the per-event oracle."""
+    sizes = [32, 33, 64, 65, 128, 129, 256, 257, 512, 513, 768, 769] + [520] * 460
     w = workloads.make_events(sizes, seed=33)
     n = len(w["xyz"])
     sim = gpu_sim(w, max_carriers=n)
     sim.load_events(w["xyz"], w["offsets"])
     sim.run_events(10)
     act, stp = sim.events()
-    for e, size in enumerate(sizes):
+    for e, size in enumerate(sizes[:14]):                     # the boundary events and two of the fillers
         o, hist = _oracle_event(w, e, 10)
         assert int(stp[e]) == o.state()["step"], (e, size)
         xyz, ids = sim.read_event_carriers(e)
