@@ -978,7 +978,7 @@ int gcoreccd_load_events(gcoreccd_t* h, const float* xyz, const uint64_t* offset
   // persistent grids: resident CTAs per SM x SM count
   int occ[kEvTiers] = {0};
   e = cudaFuncSetAttribute(k_events<4, 256, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)event_smem_bytes(kEvCapLarge));
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_events<2, 256, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)event_smem_bytes(2048u));
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_events<2, 256, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)event_smem_bytes(768u));
   if (e == cudaSuccess)
     e = cudaFuncSetAttribute(k_events_cluster<4, 256, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)event_smem_bytes(kEvCapLarge));
   if (e == cudaSuccess)
