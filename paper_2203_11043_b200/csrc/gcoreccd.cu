@@ -100,6 +100,8 @@ struct gcoreccd {
   cudaGraphExec_t graph;
   int graph_variant;
   uint32_t graph_tiles;
+  uint32_t graph_parts, graph_steps;  // treecode parts the graph was captured for (0: all-pairs), steps it holds
+  uint64_t graph_launches;            // kernels in the graph
   cudaEvent_t ev[4];
   uint32_t shard_rank, shard_world;   // target sharding (gc_shard.cuh); world 1 = not sharded
   bool ff_on;                         // far-field approximation (gc_tree.cuh)
@@ -275,14 +277,28 @@ void drop_graph(gcoreccd_t* h) {
   if (h->graph) { cudaGraphExecDestroy(h->graph); h->graph = nullptr; }
 }
 
+// Steps per graph: kGraphSteps for the all-pairs path; for the treecode a whole number of re-sort cycles (the graph
+// starts with a re-sort), so that the host-scheduled cadence is baked in.  0 = do not use a graph.
+inline uint32_t graph_steps_for(const gcoreccd_t* h) {
+  if (!h->ff_parts) return kGraphSteps;
+  if (h->ff_resort > 16) return 0;
+  return h->ff_resort * ((kGraphSteps + h->ff_resort - 1) / h->ff_resort);
+}
+
 int ensure_graph(gcoreccd_t* h, uint32_t tiles) {
-  if (h->graph && h->graph_variant == h->variant && h->graph_tiles == tiles) return 0;
+  const uint32_t steps = graph_steps_for(h);
+  if (h->graph && h->graph_variant == h->variant && h->graph_tiles == tiles && h->graph_parts == h->ff_parts &&
+      h->graph_steps == steps)
+    return 0;
   drop_graph(h);
   cudaGraph_t g = nullptr;
   GC_CUDA(h, cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal));
   const uint64_t before = h->launches;
-  for (int k = 0; k < kGraphSteps; ++k) enqueue_step(h, tiles);
-  h->launches = before;                                   // capture does not launch
+  const uint32_t age = h->ff_age;
+  for (uint32_t k = 0; k < steps; ++k) enqueue_step(h, tiles);
+  h->graph_launches = h->launches - before;
+  h->launches = before;                                   // capture does not launch ...
+  h->ff_age = age;                                        // ... nor age the treecode's order
   cudaError_t e = cudaStreamEndCapture(h->stream, &g);
   if (e != cudaSuccess) return fail(h, GCORECCD_ERR_CUDA, "cudaStreamEndCapture", e);
   e = cudaGraphInstantiate(&h->graph, g, 0);
@@ -290,6 +306,8 @@ int ensure_graph(gcoreccd_t* h, uint32_t tiles) {
   if (e != cudaSuccess) { h->graph = nullptr; return fail(h, GCORECCD_ERR_CUDA, "cudaGraphInstantiate", e); }
   h->graph_variant = h->variant;
   h->graph_tiles = tiles;
+  h->graph_parts = h->ff_parts;
+  h->graph_steps = steps;
   return 0;
 }
 
@@ -311,16 +329,18 @@ int enqueue_steps(gcoreccd_t* h, uint64_t n_steps) {
     GC_CUDA(h, cudaGetLastError());
     return 0;
   }
-  const uint32_t per_step = (h->dp.flags & GCORECCD_COULOMB_OFF) ? 2u : 3u;
   // stream capture is not permitted on the legacy / per-thread default streams: plain launches there
-  // (the treecode's re-sort cadence is host-scheduled: plain launches there too)
-  const bool can_graph = h->stream != cudaStreamLegacy && h->stream != cudaStreamPerThread && h->stream != nullptr && !h->ff_parts;
-  while (can_graph && n_steps >= (uint64_t)kGraphSteps) {
+  const uint32_t gsteps = graph_steps_for(h);
+  const bool can_graph = h->stream != cudaStreamLegacy && h->stream != cudaStreamPerThread && h->stream != nullptr && gsteps > 0;
+  // the treecode's graph begins with a re-sort: single steps until the cadence is at that point
+  while (h->ff_parts && can_graph && n_steps > 0 && h->ff_age % h->ff_resort != 0) { enqueue_step(h, tiles); --n_steps; }
+  while (can_graph && n_steps >= (uint64_t)gsteps) {
     rc = ensure_graph(h, tiles);
     if (rc) return rc;
     GC_CUDA(h, cudaGraphLaunch(h->graph, h->stream));
-    h->launches += (uint64_t)kGraphSteps * per_step;
-    n_steps -= kGraphSteps;
+    if (h->ff_parts) h->ff_age += gsteps;
+    h->launches += h->graph_launches;
+    n_steps -= gsteps;
   }
   for (; n_steps > 0; --n_steps) enqueue_step(h, tiles);
   GC_CUDA(h, cudaGetLastError());
