@@ -229,7 +229,8 @@ int gcoreccd_shard_commit(gcoreccd_t* h, const void* const* msgs_host, uint32_t 
 
 /* ---- Far-field approximation of eq. 6 — a VARIANT, off by default --------------------------
  * The exact path sums all N_a^2 ordered pairs.  With set_farfield(theta >= 0) step a1 is replaced by
- * a treecode: the active holes are kept in Hilbert-curve order (re-sorted every resort_every field evaluations; 0 => 4), an
+ * a treecode: the active holes are kept in Hilbert-curve order (re-sorted every resort_every field evaluations; 0 => every
+ * 2nd for the first 192 evaluations after set_farfield / reset, while the cloud is dense, then every 4th), an
  * implicit 8-ary tree of runs of 8*8^l consecutive holes carries, per node, its hole count m, centre of charge c and the
  * radius a of the ball about c holding its members; every group of 256 consecutive targets replaces a node by ONE
  * pseudo-hole of charge m at c when  a <= theta * |x_t - c|  holds for every target t of the group, and sums all other

@@ -102,13 +102,15 @@ struct gcoreccd {
   uint32_t graph_tiles;
   uint32_t graph_parts, graph_steps;  // treecode parts the graph was captured for (0: all-pairs), steps it holds
   uint64_t graph_launches;            // kernels in the graph
+  uint32_t graph_cadence;             // re-sort cadence baked into a treecode graph
   cudaEvent_t ev[4];
   uint32_t shard_rank, shard_world;   // target sharding (gc_shard.cuh); world 1 = not sharded
   bool ff_on;                         // far-field approximation (gc_tree.cuh)
   float ff_theta;
   uint32_t ff_parts;                  // CTAs (= partial chunks) per group of 256 targets; 0 = all-pairs kernel in use
   uint64_t ff_min_active;             // below this many active holes the all-pairs kernel is faster and is used
-  uint32_t ff_resort, ff_age;         // re-sort cadence; field evaluations since the last Hilbert sort
+  uint32_t ff_resort, ff_age;         // re-sort cadence; field evaluations since set_farfield / reset
+  bool ff_auto;                       // default cadence: every 2nd evaluation for the first 192, then every ff_resort-th
   int grid_tree;
   Tree tree;
   char err[256];
@@ -181,12 +183,19 @@ inline uint32_t bucket_tiles(uint32_t t) {                  // power-of-two buck
   return b;
 }
 
-// Far-field variant (gc_tree.cuh): [Hilbert re-sort of the state every ff_resort evaluations] + nodes + walk/evaluate.
+// Re-sort cadence at a given age.  Early in an event the cloud is dense and diffusion (0.55 um per step) scrambles the
+// curve order within a few steps; later it ages slowly, hence the denser cadence at the start.
+constexpr uint32_t kFfEarlyEvals = 192;
+inline uint32_t ff_cadence_at(const gcoreccd_t* h, uint32_t age) {
+  return (h->ff_auto && age < kFfEarlyEvals) ? std::min(2u, h->ff_resort) : h->ff_resort;
+}
+
+// Far-field variant (gc_tree.cuh): [Hilbert re-sort of the state every `cadence` evaluations] + nodes + walk/evaluate.
 int launch_tree_field(gcoreccd_t* h) {
   const uint64_t nb = h->n_bound ? h->n_bound : 1;
   const uint32_t tiles = tiles_for(nb);
   const Tree& T = h->tree;
-  const bool sort = h->ff_age % h->ff_resort == 0;
+  const bool sort = h->ff_age % ff_cadence_at(h, h->ff_age) == 0;
   h->ff_age += 1;
   k_tree_reset<<<1, 256, 0, h->stream>>>(T.tc, sort ? 1 : 0);
   h->launches += 1;
@@ -281,14 +290,17 @@ void drop_graph(gcoreccd_t* h) {
 // starts with a re-sort), so that the host-scheduled cadence is baked in.  0 = do not use a graph.
 inline uint32_t graph_steps_for(const gcoreccd_t* h) {
   if (!h->ff_parts) return kGraphSteps;
-  if (h->ff_resort > 16) return 0;
-  return h->ff_resort * ((kGraphSteps + h->ff_resort - 1) / h->ff_resort);
+  const uint32_t c = ff_cadence_at(h, h->ff_age);
+  if (c > 16) return 0;
+  const uint32_t steps = c * ((kGraphSteps + c - 1) / c);
+  return ff_cadence_at(h, h->ff_age + steps - 1) == c ? steps : 0;          // not across a change of cadence
 }
 
 int ensure_graph(gcoreccd_t* h, uint32_t tiles) {
   const uint32_t steps = graph_steps_for(h);
+  const uint32_t cadence = h->ff_parts ? ff_cadence_at(h, h->ff_age) : 0u;
   if (h->graph && h->graph_variant == h->variant && h->graph_tiles == tiles && h->graph_parts == h->ff_parts &&
-      h->graph_steps == steps)
+      h->graph_steps == steps && h->graph_cadence == cadence)
     return 0;
   drop_graph(h);
   cudaGraph_t g = nullptr;
@@ -308,6 +320,7 @@ int ensure_graph(gcoreccd_t* h, uint32_t tiles) {
   h->graph_tiles = tiles;
   h->graph_parts = h->ff_parts;
   h->graph_steps = steps;
+  h->graph_cadence = cadence;
   return 0;
 }
 
@@ -330,11 +343,12 @@ int enqueue_steps(gcoreccd_t* h, uint64_t n_steps) {
     return 0;
   }
   // stream capture is not permitted on the legacy / per-thread default streams: plain launches there
-  const uint32_t gsteps = graph_steps_for(h);
-  const bool can_graph = h->stream != cudaStreamLegacy && h->stream != cudaStreamPerThread && h->stream != nullptr && gsteps > 0;
-  // the treecode's graph begins with a re-sort: single steps until the cadence is at that point
-  while (h->ff_parts && can_graph && n_steps > 0 && h->ff_age % h->ff_resort != 0) { enqueue_step(h, tiles); --n_steps; }
-  while (can_graph && n_steps >= (uint64_t)gsteps) {
+  const bool stream_ok = h->stream != cudaStreamLegacy && h->stream != cudaStreamPerThread && h->stream != nullptr;
+  while (stream_ok && n_steps > 0) {
+    // the treecode's graph begins with a re-sort: single steps until the cadence is at that point
+    if (h->ff_parts && h->ff_age % ff_cadence_at(h, h->ff_age) != 0) { enqueue_step(h, tiles); --n_steps; continue; }
+    const uint32_t gsteps = graph_steps_for(h);
+    if (gsteps == 0 || n_steps < (uint64_t)gsteps) break;
     rc = ensure_graph(h, tiles);
     if (rc) return rc;
     GC_CUDA(h, cudaGraphLaunch(h->graph, h->stream));
@@ -513,6 +527,7 @@ int gcoreccd_reset(gcoreccd_t* h) {
   GC_CUDA(h, cudaMemsetAsync(h->image, 0, (size_t)h->p.img_nx * h->p.img_ny * 4, h->stream));
   GC_CUDA(h, cudaMemsetAsync(h->fin, 0xff, (size_t)h->L.cap_pad * 16, h->stream));     // NaN / all-ones = still drifting
   if (h->ff_on) GC_CUDA(h, cudaMemsetAsync(h->tree.tc, 0, sizeof(TreeCtrl), h->stream)); // far-field counters restart too
+  h->ff_age = 0;
   GC_CUDA(h, cudaStreamSynchronize(h->stream));
   drop_events(h);
   h->n_loaded = 0;
@@ -828,6 +843,7 @@ int gcoreccd_set_farfield(gcoreccd_t* h, double theta, uint32_t resort_every, ui
   h->ff_on = theta >= 0.0;
   h->ff_theta = (float)(theta >= 0.0 ? theta : 0.0);
   h->ff_resort = resort_every ? resort_every : 4u;
+  h->ff_auto = resort_every == 0;
   h->ff_min_active = min_active ? min_active : 24576u;
   h->ff_parts = 0;
   h->ff_age = 0;
