@@ -244,3 +244,30 @@ def test_sharded_treecode_run_conserves_and_tracks_the_single_gpu_treecode():
     single.close()
     for e in es:
         e.close()
+
+
+def test_farfield_track_image_agrees_with_the_exact_path_pixel_by_pixel():
+    """cfg-3 track, 65,536 holes, to full collection: the far-field image against the exact CUDA path's, R22
+    (sum exact; per pixel |dn| <= max(1 % n_ref, 5 sqrt(n_ref + 1)): two realisations of a chaotic system differ by
+    counting noise, not by more)."""
+    from util import image_moments
+    w = workloads.make(3, n=65536)
+    P = w["params"]
+    imgs = []
+    for theta in (-1.0, 0.5):
+        sim = gpu_sim(w)
+        if theta >= 0:
+            sim.set_farfield(theta)
+        sim.load_carriers(w["xyz"])
+        done, left, _ = sim.run_to_collection()
+        img, over = sim.read_image()
+        assert left == 0 and int(img.sum()) + over == 65536
+        imgs.append((img.astype(np.int64), over, done))
+        sim.close()
+    (a, oa, da), (b, ob, db) = imgs
+    assert abs(da - db) <= 8 and abs(oa - ob) <= 5 * np.sqrt(oa + 1)
+    tol = np.maximum(0.01 * a, 5.0 * np.sqrt(a + 1.0))
+    assert np.all(np.abs(a - b) <= tol), int((np.abs(a - b) > tol).sum())
+    ma, mb = image_moments(a, P["img_x0_um"], P["img_y0_um"], P["pixel_pitch_um"]), image_moments(b, P["img_x0_um"], P["img_y0_um"], P["pixel_pitch_um"])
+    assert abs(ma[0] - mb[0]) <= 0.05 and abs(ma[1] - mb[1]) <= 0.05              # centroids, um
+    assert abs(ma[2] / mb[2] - 1.0) <= 0.01 and abs(ma[3] / mb[3] - 1.0) <= 0.01    # second moments within 1 %
