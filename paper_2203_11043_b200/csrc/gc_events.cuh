@@ -378,7 +378,6 @@ k_events_warp(SoA A, EventTable ev, const uint32_t* __restrict__ order, uint32_t
   float* sx = s_pos[warp][0];
   float* sy = s_pos[warp][1];
   float* sz = s_pos[warp][2];
-  const uint32_t lt = (1u << lane) - 1u;
   const float2 eps2v = make_float2(P.eps2, P.eps2);
   uint32_t nonfinite = 0;
 
