@@ -168,7 +168,9 @@ inline PlanArgs plan_args(const gcoreccd_t* h, int v) {
   PlanArgs a;
   a.IB = variant_ib(v);
   a.grid = (uint32_t)h->grid_field[v];
-  a.part_cap_entries = (uint32_t)h->L.part_cap;
+  // with the far-field variant on, the tail of the partial plane is the treecode's scratch (counters included): the
+  // all-pairs kernel, which takes over below min_active holes, must not plan its chunks into it
+  a.part_cap_entries = (uint32_t)(h->ff_on ? h->L.part_cap - 10 * h->L.cap_pad : h->L.part_cap);
   a.rank = h->shard_rank;
   a.world = h->shard_world;
   a.force_S = h->ff_parts;

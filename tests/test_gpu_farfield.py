@@ -271,3 +271,21 @@ def test_farfield_track_image_agrees_with_the_exact_path_pixel_by_pixel():
     ma, mb = image_moments(a, P["img_x0_um"], P["img_y0_um"], P["pixel_pitch_um"]), image_moments(b, P["img_x0_um"], P["img_y0_um"], P["pixel_pitch_um"])
     assert abs(ma[0] - mb[0]) <= 0.05 and abs(ma[1] - mb[1]) <= 0.05              # centroids, um
     assert abs(ma[2] / mb[2] - 1.0) <= 0.01 and abs(ma[3] / mb[3] - 1.0) <= 0.01    # second moments within 1 %
+
+
+def test_farfield_counters_survive_the_switch_to_the_all_pairs_kernel():
+    """Below min_active the all-pairs kernel takes over; its partial sums must stay out of the treecode's scratch (the
+    counters live there): small capacity, many chunks."""
+    w = workloads.make(2, n=30000)
+    sim = gpu_sim(w)
+    sim.set_farfield(0.5, 0, 1)
+    sim.load_carriers(w["xyz"])
+    sim.step(4)
+    before = sim.farfield_stats()
+    assert before["far_evals"] > 0
+    sim.set_farfield(0.5, 0, 10 ** 9)                     # min_active above the population: all-pairs from now on
+    sim.step(6)
+    after = sim.farfield_stats()
+    assert after["far_evals"] == 0 and after["near_evals"] == 0      # set_farfield restarts them; nothing tramples them
+    assert sim.state()["step"] == 10
+    sim.close()
