@@ -259,17 +259,21 @@ def run_ours(args):
     # ---- seconds per 131k-hole event (second half of BASELINE.json's metric): load -> full collection
     event = None
     if not args.no_event:
-        sim.reset()
-        barrier()
-        t0 = time.perf_counter()
-        sim.load_carriers_ptr(host_in.data_ptr(), n)
-        done, left, rc = sim.run_to_collection(10 ** 7)
-        img, over = sim.read_image()
-        torch.cuda.synchronize()
-        ev_s = time.perf_counter() - t0
-        st2 = sim.state()
-        assert left == 0 and int(img.sum()) + over == n, "hole count not conserved"
-        event = {"seconds": ev_s, "steps": done, "pair_interactions": st2["pair_interactions"],
+        runs = []
+        for _ in range(3):                                  # best of 3 plus median
+            sim.reset()
+            barrier()
+            t0 = time.perf_counter()
+            sim.load_carriers_ptr(host_in.data_ptr(), n)
+            done, left, rc = sim.run_to_collection(10 ** 7)
+            img, over = sim.read_image()
+            torch.cuda.synchronize()
+            runs.append(time.perf_counter() - t0)
+            st2 = sim.state()
+            assert left == 0 and int(img.sum()) + over == n, "hole count not conserved"
+        ev_s = min(runs)
+        event = {"seconds": ev_s, "seconds_median": float(np.median(runs)), "runs": 3, "steps": done,
+                 "pair_interactions": st2["pair_interactions"],
                  "avg_G_pairs_per_s": st2["pair_interactions"] / ev_s / 1e9, "holes": n, "collected_in_window": int(img.sum())}
 
     # ---- far-field VARIANT (reported separately, never part of `value`): same event, treecode
