@@ -120,7 +120,8 @@ struct gcoreccd {
     uint64_t n_events, n_carriers;        // as loaded
     uint64_t events_left, carriers_left;  // after the last run_events
     uint32_t n_q[kEvTiers];               // events per queue, smallest tier first (order = [tier 0..., tier 1..., ...])
-    char* d_buf;                          // one allocation: off | cnt | order | queue | step
+    char* d_buf;                          // one allocation: off | cnt | order | queue | step (kept across batches)
+    size_t d_buf_bytes, h_cap_events;     // capacities of d_buf and of the host mirrors
     uint32_t *d_off, *d_cnt, *d_order, *d_queue;
     uint64_t* d_step;
     uint32_t *h_off, *h_cnt;              // host mirrors
@@ -363,7 +364,16 @@ int enqueue_steps(gcoreccd_t* h, uint64_t n_steps) {
   return 0;
 }
 
-void drop_events(gcoreccd_t* h) {
+// A batch's device buffer, host mirrors, side streams and events are kept from one batch to the next (a production
+// run loads batch after batch): clear_events forgets the batch, free_events releases everything.
+void clear_events(gcoreccd_t* h) {
+  auto& B = h->evb;
+  B.loaded = false;
+  B.n_events = B.n_carriers = B.events_left = B.carriers_left = 0;
+  for (int q = 0; q < kEvTiers; ++q) B.n_q[q] = 0;
+}
+
+void free_events(gcoreccd_t* h) {
   if (h->evb.d_buf) cudaFree(h->evb.d_buf);
   for (int k = 0; k < kEvTiers - 1; ++k) {
     if (h->evb.aux[k]) cudaStreamDestroy(h->evb.aux[k]);
@@ -513,7 +523,7 @@ int gcoreccd_destroy(gcoreccd_t* h) {
   DeviceGuard guard(h->device);
   if (h->stream) cudaStreamSynchronize(h->stream);
   drop_graph(h);
-  drop_events(h);
+  free_events(h);
   for (int k = 0; k < 4; ++k) if (h->ev[k]) cudaEventDestroy(h->ev[k]);
   if (h->h_ctrl) cudaFreeHost(h->h_ctrl);
   if (h->own_stream && h->stream) cudaStreamDestroy(h->stream);
@@ -531,7 +541,7 @@ int gcoreccd_reset(gcoreccd_t* h) {
   if (h->ff_on) GC_CUDA(h, cudaMemsetAsync(h->tree.tc, 0, sizeof(TreeCtrl), h->stream)); // far-field counters restart too
   h->ff_age = 0;
   GC_CUDA(h, cudaStreamSynchronize(h->stream));
-  drop_events(h);
+  clear_events(h);
   h->n_loaded = 0;
   h->n_bound = 0;
   h->variant = -1;
@@ -928,23 +938,34 @@ int gcoreccd_load_events(gcoreccd_t* h, const float* xyz, const uint64_t* offset
     if (h->h_ctrl->invalid) return fail(h, GCORECCD_ERR_INVALID, "load_events: non-finite coordinate or z > thickness");
   }
 
-  drop_events(h);
+  clear_events(h);
   auto& B = h->evb;
   const size_t ne = (size_t)n_events;
   const size_t b_off = align_up((ne + 1) * 4, 256), b_cnt = align_up(ne * 4, 256), b_ord = align_up(ne * 4, 256), b_q = 256,
                b_step = align_up(ne * 8, 256);
-  cudaError_t e = cudaMalloc((void**)&B.d_buf, b_off + b_cnt + b_ord + b_q + b_step);
-  if (e != cudaSuccess) { B.d_buf = nullptr; return fail(h, e == cudaErrorMemoryAllocation ? GCORECCD_ERR_NOMEM : GCORECCD_ERR_CUDA, "load_events: cudaMalloc", e); }
+  cudaError_t e = cudaSuccess;
+  if (b_off + b_cnt + b_ord + b_q + b_step > B.d_buf_bytes) {
+    if (B.d_buf) cudaFree(B.d_buf);
+    B.d_buf = nullptr; B.d_buf_bytes = 0;
+    e = cudaMalloc((void**)&B.d_buf, b_off + b_cnt + b_ord + b_q + b_step);
+    if (e != cudaSuccess) { B.d_buf = nullptr; return fail(h, e == cudaErrorMemoryAllocation ? GCORECCD_ERR_NOMEM : GCORECCD_ERR_CUDA, "load_events: cudaMalloc", e); }
+    B.d_buf_bytes = b_off + b_cnt + b_ord + b_q + b_step;
+  }
   B.d_off = (uint32_t*)B.d_buf;
   B.d_cnt = (uint32_t*)(B.d_buf + b_off);
   B.d_order = (uint32_t*)(B.d_buf + b_off + b_cnt);
   B.d_queue = (uint32_t*)(B.d_buf + b_off + b_cnt + b_ord);
   B.d_step = (uint64_t*)(B.d_buf + b_off + b_cnt + b_ord + b_q);
-  B.h_off = (uint32_t*)malloc((ne + 1) * 4);
-  B.h_cnt = (uint32_t*)malloc(ne * 4 + 4);
-  B.h_step = (uint64_t*)calloc(ne + 1, 8);
+  if (ne > B.h_cap_events) {
+    free(B.h_off); free(B.h_cnt); free(B.h_step);
+    B.h_off = (uint32_t*)malloc((ne + 1) * 4);
+    B.h_cnt = (uint32_t*)malloc(ne * 4 + 4);
+    B.h_step = (uint64_t*)malloc((ne + 1) * 8);
+    B.h_cap_events = (B.h_off && B.h_cnt && B.h_step) ? ne : 0;
+  }
+  if (B.h_step) memset(B.h_step, 0, (ne + 1) * 8);
   uint32_t* order = (uint32_t*)malloc(ne * 4 + 4);
-  if (!B.h_off || !B.h_cnt || !B.h_step || !order) { free(order); drop_events(h); return fail(h, GCORECCD_ERR_NOMEM, "load_events: host memory"); }
+  if (!B.h_off || !B.h_cnt || !B.h_step || !order) { free(order); clear_events(h); return fail(h, GCORECCD_ERR_NOMEM, "load_events: host memory"); }
   uint64_t left_events = 0;
   for (size_t k = 0; k < ne; ++k) {
     B.h_off[k] = (uint32_t)offsets[k];
@@ -964,7 +985,7 @@ int gcoreccd_load_events(gcoreccd_t* h, const float* xyz, const uint64_t* offset
   if (e == cudaSuccess) e = cudaMemcpyAsync(&h->ctrl->n_loaded, &total_loaded, 8, cudaMemcpyHostToDevice, h->stream);
   // scheduling hint: mean depth per event (d_order doubles as the float scratch until the order is uploaded)
   float* zmean = (float*)malloc(ne * 4 + 4);
-  if (!zmean) { free(order); drop_events(h); return fail(h, GCORECCD_ERR_NOMEM, "load_events: host memory"); }
+  if (!zmean) { free(order); clear_events(h); return fail(h, GCORECCD_ERR_NOMEM, "load_events: host memory"); }
   if (e == cudaSuccess) {
     k_event_depth<<<(unsigned)((ne * 32 + kTPB - 1) / kTPB), kTPB, 0, h->stream>>>(h->A, B.d_off, B.d_cnt, (uint32_t)ne, (float*)B.d_order);
     h->launches += 1;
@@ -972,7 +993,7 @@ int gcoreccd_load_events(gcoreccd_t* h, const float* xyz, const uint64_t* offset
   }
   if (e == cudaSuccess) e = cudaMemcpyAsync(zmean, B.d_order, ne * 4, cudaMemcpyDeviceToHost, h->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
-  if (e != cudaSuccess) { free(order); free(zmean); drop_events(h); return fail(h, GCORECCD_ERR_CUDA, "load_events", e); }
+  if (e != cudaSuccess) { free(order); free(zmean); clear_events(h); return fail(h, GCORECCD_ERR_CUDA, "load_events", e); }
   // one queue per tier (kernel variant), each in longest-processing-time-first order
   // estimated work of an event = n^2 x steps, steps ~ the low-field drift time from its mean depth,
   // ln(a2 / (a2 - a1 z)) (eq. 1 with constant mobility); plain z where that is undefined.  Order only: never physics.
@@ -1011,27 +1032,29 @@ int gcoreccd_load_events(gcoreccd_t* h, const float* xyz, const uint64_t* offset
   e = cudaMemcpyAsync(B.d_order, order, ne * 4, cudaMemcpyHostToDevice, h->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
   free(order);
-  if (e != cudaSuccess) { drop_events(h); return fail(h, GCORECCD_ERR_CUDA, "load_events", e); }
+  if (e != cudaSuccess) { clear_events(h); return fail(h, GCORECCD_ERR_CUDA, "load_events", e); }
 
-  // persistent grids: resident CTAs per SM x SM count
-  int occ[kEvTiers] = {0};
-  e = cudaFuncSetAttribute(k_events<4, 256, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)event_smem_bytes(kEvCapLarge));
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_events<2, 256, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)event_smem_bytes(768u));
-  if (e == cudaSuccess)
-    e = cudaFuncSetAttribute(k_events_cluster<4, 256, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)event_smem_bytes(kEvCapLarge));
-  if (e == cudaSuccess)
-    e = cudaFuncSetAttribute(k_events_cluster<4, 256, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)event_smem_bytes(kEvCapLarge));
-  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[0], k_events_warp, kEvTierThreads[0], 0);
-  for (int q = 1; q < kEvTiers && e == cudaSuccess; ++q)
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[q], ev_kernel(q), kEvTierThreads[q], event_smem_bytes(kEvTierCap[q]));
-  if (e != cudaSuccess) { drop_events(h); return fail(h, GCORECCD_ERR_CUDA, "load_events: kernel attributes", e); }
-  for (int q = 0; q < kEvTiers; ++q) B.grid_q[q] = h->num_sms * (occ[q] > 0 ? occ[q] : 1);
-  e = cudaEventCreateWithFlags(&B.fork, cudaEventDisableTiming);
-  for (int k = 0; k < kEvTiers - 1 && e == cudaSuccess; ++k) {
-    e = cudaStreamCreateWithFlags(&B.aux[k], cudaStreamNonBlocking);
-    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&B.join[k], cudaEventDisableTiming);
+  // persistent grids (resident CTAs per SM x SM count), side streams and events: once per handle
+  if (!B.fork) {
+    int occ[kEvTiers] = {0};
+    e = cudaFuncSetAttribute(k_events<4, 256, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)event_smem_bytes(kEvCapLarge));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_events<2, 256, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)event_smem_bytes(768u));
+    if (e == cudaSuccess)
+      e = cudaFuncSetAttribute(k_events_cluster<4, 256, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)event_smem_bytes(kEvCapLarge));
+    if (e == cudaSuccess)
+      e = cudaFuncSetAttribute(k_events_cluster<4, 256, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)event_smem_bytes(kEvCapLarge));
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[0], k_events_warp, kEvTierThreads[0], 0);
+    for (int q = 1; q < kEvTiers && e == cudaSuccess; ++q)
+      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[q], ev_kernel(q), kEvTierThreads[q], event_smem_bytes(kEvTierCap[q]));
+    if (e != cudaSuccess) { clear_events(h); return fail(h, GCORECCD_ERR_CUDA, "load_events: kernel attributes", e); }
+    for (int q = 0; q < kEvTiers; ++q) B.grid_q[q] = h->num_sms * (occ[q] > 0 ? occ[q] : 1);
+    for (int k = 0; k < kEvTiers - 1 && e == cudaSuccess; ++k) {
+      e = cudaStreamCreateWithFlags(&B.aux[k], cudaStreamNonBlocking);
+      if (e == cudaSuccess) e = cudaEventCreateWithFlags(&B.join[k], cudaEventDisableTiming);
+    }
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&B.fork, cudaEventDisableTiming);
+    if (e != cudaSuccess) { free_events(h); return fail(h, GCORECCD_ERR_CUDA, "load_events: streams", e); }
   }
-  if (e != cudaSuccess) { drop_events(h); return fail(h, GCORECCD_ERR_CUDA, "load_events: streams", e); }
   B.loaded = true;
   B.n_events = n_events; B.n_carriers = n;
   B.events_left = left_events; B.carriers_left = n;
