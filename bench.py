@@ -134,7 +134,7 @@ def run_reference(args):
     if rank != 0:
         return 0
     from oracle import goracle as g
-    from paper_2203_11043_b200 import workloads
+    import workloads
     g.build()
     w = workloads.make(WORKLOAD_CFG)
     P, xyz = w["params"], w["xyz"]
@@ -163,7 +163,8 @@ def run_reference(args):
 def run_ours(args):
     import torch
     import torch.distributed as dist
-    from paper_2203_11043_b200 import binding, replicas, workloads
+    import workloads
+    from paper_2203_11043_b200 import binding, replicas
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -367,7 +368,8 @@ def run_sweep(args):
     """N sweep at fixed geometry (cfg-2 cloud), Coulomb on and off, 16 steps each through the graph path: the shape of
     the paper's Fig. 4 experiment.  One JSON line per size; not the headline number."""
     import torch
-    from paper_2203_11043_b200 import binding, workloads
+    import workloads
+    from paper_2203_11043_b200 import binding
     peaks, _ = measured_peaks()
     peak_pairs = SM_COUNT * LANES * 2.0 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / FLOP_PER_PAIR
     sizes = [int(t) for t in args.sweep.split(",")]
@@ -403,7 +405,8 @@ def run_sharded(args):
     (shard_local + shard_commit, CUDA events) — the exchange over NVLink is NOT in that number."""
     import torch
     import torch.distributed as dist
-    from paper_2203_11043_b200 import binding, replicas, sharded, workloads
+    import workloads
+    from paper_2203_11043_b200 import binding, replicas, sharded
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))

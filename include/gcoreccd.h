@@ -96,7 +96,9 @@ int gcoreccd_reset(gcoreccd_t* h);
 int gcoreccd_load_carriers(gcoreccd_t* h, const float* xyz_um, uint64_t n, int on_device);
 
 /* Restart from an exported snapshot (replaces the active set): positions, ids (must be unique) and the step
- * index the next step will use.  The image and counters are kept.  Host pointers. */
+ * index the next step will use.  The image and counters are kept; n_loaded becomes max(n_loaded, max id + 1).
+ * Validated like load_carriers (INVALID on a non-finite coordinate, z > thickness, or z <= z_well: a snapshot holds
+ * ACTIVE carriers only).  On a sharded handle every rank loads the same snapshot.  Host pointers. */
 int gcoreccd_load_snapshot(gcoreccd_t* h, const float* xyz_um_host, const uint32_t* id_host, uint64_t n,
                            uint64_t step);
 

@@ -3,4 +3,4 @@
 Importing the package is cheap and loads no native code; `paper_2203_11043_b200.binding`
 loads the C-ABI library (include/gcoreccd.h) on first use and fails loudly if it is missing.
 """
-__all__ = ["binding", "workloads", "build"]
+__all__ = ["binding", "build"]

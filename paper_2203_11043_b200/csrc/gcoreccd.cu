@@ -314,8 +314,14 @@ int ensure_graph(gcoreccd_t* h, uint32_t tiles) {
   h->graph_launches = h->launches - before;
   h->launches = before;                                   // capture does not launch ...
   h->ff_age = age;                                        // ... nor age the treecode's order
-  cudaError_t e = cudaStreamEndCapture(h->stream, &g);
-  if (e != cudaSuccess) return fail(h, GCORECCD_ERR_CUDA, "cudaStreamEndCapture", e);
+  const cudaError_t e_launch = cudaGetLastError();        // a launch refused during capture (bad configuration)
+  cudaError_t e = cudaStreamEndCapture(h->stream, &g);    // always end the capture: the caller's stream must not stay in it
+  if (e == cudaSuccess && e_launch != cudaSuccess) e = e_launch;
+  if (e != cudaSuccess) {
+    if (g) cudaGraphDestroy(g);
+    cudaGetLastError();                                   // clear the sticky capture-invalidated status
+    return fail(h, GCORECCD_ERR_CUDA, "CUDA graph capture of a batch of steps", e);
+  }
   e = cudaGraphInstantiate(&h->graph, g, 0);
   cudaGraphDestroy(g);
   if (e != cudaSuccess) { h->graph = nullptr; return fail(h, GCORECCD_ERR_CUDA, "cudaGraphInstantiate", e); }
@@ -541,6 +547,7 @@ int gcoreccd_reset(gcoreccd_t* h) {
   if (h->ff_on) GC_CUDA(h, cudaMemsetAsync(h->tree.tc, 0, sizeof(TreeCtrl), h->stream)); // far-field counters restart too
   h->ff_age = 0;
   GC_CUDA(h, cudaStreamSynchronize(h->stream));
+  drop_graph(h);                                           // its grids were sized for the previous population
   clear_events(h);
   h->n_loaded = 0;
   h->n_bound = 0;
@@ -558,6 +565,7 @@ int gcoreccd_load_carriers(gcoreccd_t* h, const float* xyz, uint64_t n, int on_d
   if (rc) return rc;
   const uint64_t n_act = h->h_ctrl->n_active;
   if (n_act + n > h->p.max_carriers || h->n_loaded + n > 0xffffffffull) return fail(h, GCORECCD_ERR_CAPACITY, "load_carriers: capacity");
+  drop_graph(h);                                           // the population grows: a cached graph's grids may be too small
   const float* src = xyz;
   if (!on_device) {
     GC_CUDA(h, cudaMemcpyAsync(h->Ep, xyz, n * 12, cudaMemcpyHostToDevice, h->stream));
@@ -591,24 +599,39 @@ int gcoreccd_load_snapshot(gcoreccd_t* h, const float* xyz, const uint32_t* id, 
   if (n > h->p.max_carriers) return fail(h, GCORECCD_ERR_CAPACITY, "load_snapshot: capacity");
   if (events_busy(h)) return fail(h, GCORECCD_ERR_STATE, "load_snapshot: a batch of events is still drifting");
   DeviceGuard guard(h->device);
+  drop_graph(h);
   float* st_xyz = h->Ep;
   uint32_t* st_id = (uint32_t*)(h->Ep + 3 * h->L.cap_pad);
   if (n) {
     GC_CUDA(h, cudaMemcpyAsync(st_xyz, xyz, n * 12, cudaMemcpyHostToDevice, h->stream));
     GC_CUDA(h, cudaMemcpyAsync(st_id, id, n * 4, cudaMemcpyHostToDevice, h->stream));
+    // same validation as load_carriers; in addition an ACTIVE carrier must be above the collection plane
+    GC_CUDA(h, cudaMemsetAsync(&h->ctrl->invalid, 0, 4, h->stream));
+    k_validate<<<tiles_for(n), kTPB, 0, h->stream>>>(st_xyz, (uint32_t)n, h->ctrl, h->dp.thickness);
+    h->launches += 1;
+    int rc = sync_ctrl(h);
+    if (rc) return rc;
+    if (h->h_ctrl->invalid) return fail(h, GCORECCD_ERR_INVALID, "load_snapshot: non-finite coordinate or z > thickness");
+    for (uint64_t k = 0; k < n; ++k)
+      if (!((double)xyz[3 * k + 2] > h->p.z_well_um)) return fail(h, GCORECCD_ERR_INVALID, "load_snapshot: an active carrier must have z > z_well");
     k_set_snapshot<<<tiles_for(n), kTPB, 0, h->stream>>>(st_xyz, st_id, (uint32_t)n, h->A);
     h->launches += 1;
   }
-  const int v = pick_variant(n);
+  // sharded handles: every rank loads the same snapshot; the plan below is this rank's share of it
+  const int v = pick_variant(h->shard_world > 1 ? (n + h->shard_world - 1) / h->shard_world : n);
   h->variant = v;
+  h->ff_parts = 0;
   k_replan<<<1, 32, 0, h->stream>>>(h->ctrl, plan_args(h, v), 1, (uint32_t)n, 1, step);
   h->launches += 1;
   GC_CUDA(h, cudaGetLastError());
-  int rc = sync_ctrl(h);
-  if (rc) return rc;
   uint64_t max_id = 0;
   for (uint64_t k = 0; k < n; ++k) if (id[k] > max_id) max_id = id[k];
   if (n && h->n_loaded < max_id + 1) h->n_loaded = max_id + 1;
+  // keep the device copy in step with the host's: get_state's invariant is stated on n_loaded
+  GC_CUDA(h, cudaMemcpyAsync(&h->ctrl->n_loaded, &h->n_loaded, 8, cudaMemcpyHostToDevice, h->stream));
+  int rc = sync_ctrl(h);
+  if (rc) return rc;
+  h->variant = -1;                                         // the next step re-picks (far-field parts included)
   return GCORECCD_OK;
 }
 

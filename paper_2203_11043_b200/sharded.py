@@ -96,9 +96,10 @@ class ShardedEvent:
         self.nbytes = self.e.shard_message_bytes()
         if self.nbytes > self.max_bytes:
             self.max_bytes = self.nbytes
-            self.x = self._xf(self.max_bytes)
-            if not hasattr(self.x, "message"):
-                self.msgs = [self._alloc(self.max_bytes), self._alloc(self.max_bytes)]
+            with self._on_engine_stream():   # buffers allocated by torch belong to the stream that uses them
+                self.x = self._xf(self.max_bytes)
+                if not hasattr(self.x, "message"):
+                    self.msgs = [self._alloc(self.max_bytes), self._alloc(self.max_bytes)]
 
     def load_carriers(self, xyz):
         """Every rank loads the same holes in the same order."""
@@ -110,16 +111,27 @@ class ShardedEvent:
         self._prepare()
         return st
 
+    def _on_engine_stream(self):
+        """The exchange (an NCCL all-gather, a symmetric-memory barrier) is enqueued on torch's CURRENT stream, the
+        library's kernels on the handle's stream: make them the same stream for the duration of a step, so that
+        shard_local -> gather -> shard_commit are ordered by the stream and nothing else."""
+        st = getattr(self.e, "_stream", None)
+        if st is None:                       # an engine without a CUDA stream (the CPU test engine)
+            import contextlib
+            return contextlib.nullcontext()
+        return self.e._torch.cuda.stream(st)
+
     def step(self, n=1):
         if self.x is None:
             self._prepare()
-        for _ in range(int(n)):
-            msg = self.x.message() if hasattr(self.x, "message") else self.msgs[self.k & 1]
-            self.k += 1
-            self.e.shard_local(msg.data_ptr(), self.nbytes)
-            ptrs = self.x.gather(msg, self.nbytes)
-            self.e.shard_commit(ptrs, self.nbytes)
-            self.x.after_commit()
+        with self._on_engine_stream():
+            for _ in range(int(n)):
+                msg = self.x.message() if hasattr(self.x, "message") else self.msgs[self.k & 1]
+                self.k += 1
+                self.e.shard_local(msg.data_ptr(), self.nbytes)
+                ptrs = self.x.gather(msg, self.nbytes)
+                self.e.shard_commit(ptrs, self.nbytes)
+                self.x.after_commit()
 
     def run_to_collection(self, max_steps=10 ** 9):
         st = self.refresh()

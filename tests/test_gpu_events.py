@@ -5,7 +5,8 @@ import numpy as np
 import pytest
 
 from oracle import goracle as g
-from paper_2203_11043_b200 import binding, workloads
+import workloads
+from paper_2203_11043_b200 import binding
 from util import gpu_sim, oracle_sim
 
 pytestmark = pytest.mark.gpu

@@ -7,7 +7,7 @@ import numpy as np
 import pytest
 
 from oracle import goracle as g
-from paper_2203_11043_b200 import workloads
+import workloads
 from util import field_rel_err, gpu_sim, oracle_sim, traj_assert
 
 pytestmark = pytest.mark.gpu

@@ -4,7 +4,7 @@ to the oracle elsewhere, so many cases stay cheap; seeds are fixed (the cases ar
 import numpy as np
 import pytest
 
-from paper_2203_11043_b200 import workloads
+import workloads
 from util import gpu_sim
 
 pytestmark = pytest.mark.gpu

@@ -24,7 +24,8 @@ def _free_port():
 
 def _worker(rank, world, port, q):
     sys.path.insert(0, ROOT)
-    from paper_2203_11043_b200 import replicas, workloads
+    import workloads
+    from paper_2203_11043_b200 import replicas
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:

@@ -25,7 +25,7 @@ def _free_port():
 
 
 def _workload():
-    from paper_2203_11043_b200 import workloads
+    import workloads
     w = workloads.make(3, n=N_HOLES)               # a track: holes retire from the first step on, shares move
     return w
 
