@@ -53,6 +53,11 @@ enum {                            /* gcoreccd_params.flags */
   GCORECCD_DEPLETION_OFF = 4u     /* test hook: a1 = a2 = 0                          */
 };
 
+/* Largest capacity of one handle: 2^24 holes (32 B of state + 192 B of partial-sum planes + 16 B of collection record per
+ * hole of capacity: 4.0 GB at 2^24).  Tested up to 4,194,304 holes (tests/test_gpu_full_runs.py); one all-pairs step at 2^24
+ * holes is 2.8e14 interactions (~100 s on a B200), beyond which the far-field variant or target sharding is the tool. */
+#define GCORECCD_MAX_CARRIERS (1ull << 24)
+
 typedef struct {
   uint32_t struct_size;           /* = sizeof(gcoreccd_params); ABI versioning                            */
   uint32_t flags;                 /* bits above; 0 = full physics                                          */
@@ -75,7 +80,7 @@ typedef struct {
   void*    workspace;             /* optional caller-owned device memory (e.g. a torch uint8 tensor),
                                      256-byte aligned, alive until destroy; NULL => the library allocates */
   uint64_t workspace_bytes;       /* >= gcoreccd_workspace_size(max_carriers, img_nx, img_ny)              */
-  uint64_t max_carriers;          /* capacity, 1 .. 2^26                                                   */
+  uint64_t max_carriers;          /* capacity, 1 .. GCORECCD_MAX_CARRIERS                                  */
 } gcoreccd_params;
 
 /* Bytes of device memory a handle needs (state ping-pong, field partials, image, counters). */
@@ -254,9 +259,18 @@ int gcoreccd_shard_commit(gcoreccd_t* h, const void* const* msgs_host, uint32_t 
 int gcoreccd_set_farfield(gcoreccd_t* h, double theta, uint32_t resort_every, uint64_t min_active);
 int gcoreccd_farfield_stats(gcoreccd_t* h, uint64_t* far_evals, uint64_t* near_evals, double* bound_B);
 
-/* Run ONE step with CUDA events between its kernels (on the handle's stream) and return the device time of
- * each in milliseconds: ms[0] field, ms[1] integrate+collect, ms[2] compact, ms[3] whole step.  Synchronous. */
+/* Run ONE step as two launches with CUDA events between them (on the handle's stream) and return the device time of
+ * each in milliseconds: ms[0] field (a1), ms[1] advance (a2..a8: update, collection, in-place compaction), ms[2] = 0
+ * (compaction was a kernel of its own in version 0.1), ms[3] whole step.  Synchronous. */
 int gcoreccd_profile_step(gcoreccd_t* h, float ms_host[4]);
+
+/* Small populations (below ~1e3 charges "the GPU is subutilised"): while the handle's upper bound on
+ * n_active is <= max_active, gcoreccd_step / run_to_collection run all their steps in ONE cooperative launch of a
+ * persistent kernel (field -> grid barrier -> a2..a8 -> grid barrier per step) instead of two launches per step.
+ * on = 0 turns that off (tuning / test hook); max_active = 0 keeps the default (24,576).  Same physics, same Philox
+ * counters; the FP32 summation order of eq. 6 differs between the two paths, nothing else.  All-pairs, unsharded
+ * handles only (otherwise ignored). */
+int gcoreccd_set_persistent(gcoreccd_t* h, int on, uint64_t max_active);
 
 /* Number of kernels this handle has launched so far (bench.py's gpu_launches). */
 uint64_t gcoreccd_kernel_launches(gcoreccd_t* h);

@@ -24,7 +24,7 @@ EXPORTS = ["gcoreccd_workspace_size", "gcoreccd_create", "gcoreccd_destroy", "gc
            "gcoreccd_load_carriers_file", "gcoreccd_save_collected_file",
            "gcoreccd_set_farfield", "gcoreccd_farfield_stats",
            "gcoreccd_set_shard", "gcoreccd_shard_message_bytes", "gcoreccd_shard_local", "gcoreccd_shard_commit",
-           "gcoreccd_profile_step", "gcoreccd_kernel_launches", "gcoreccd_debug_normals", "gcoreccd_strerror",
+           "gcoreccd_profile_step", "gcoreccd_set_persistent", "gcoreccd_kernel_launches", "gcoreccd_debug_normals", "gcoreccd_strerror",
            "gcoreccd_last_error", "gcoreccd_version"]
 
 
@@ -121,6 +121,8 @@ def lib():
     L.gcoreccd_farfield_stats.argtypes = [vp, u64p, u64p, C.POINTER(C.c_double)]
     L.gcoreccd_profile_step.restype = C.c_int
     L.gcoreccd_profile_step.argtypes = [vp, fp]
+    L.gcoreccd_set_persistent.restype = C.c_int
+    L.gcoreccd_set_persistent.argtypes = [vp, C.c_int, C.c_uint64]
     L.gcoreccd_kernel_launches.restype = C.c_uint64
     L.gcoreccd_kernel_launches.argtypes = [vp]
     L.gcoreccd_debug_normals.restype = C.c_int
@@ -414,7 +416,10 @@ class Gcoreccd:
     def profile_step(self):
         ms = (C.c_float * 4)()
         self._check(lib().gcoreccd_profile_step(self._h, ms), "gcoreccd_profile_step")
-        return dict(field=float(ms[0]), integrate=float(ms[1]), compact=float(ms[2]), step=float(ms[3]))
+        return dict(field=float(ms[0]), advance=float(ms[1]), step=float(ms[3]))
+
+    def set_persistent(self, on=True, max_active=0):
+        self._check(lib().gcoreccd_set_persistent(self._h, int(bool(on)), int(max_active)), "gcoreccd_set_persistent")
 
     def kernel_launches(self):
         return int(lib().gcoreccd_kernel_launches(self._h))

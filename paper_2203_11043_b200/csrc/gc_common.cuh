@@ -12,7 +12,7 @@ namespace gc {
 
 constexpr int kTPB        = 256;          // threads per CTA of every kernel
 constexpr int kTile       = 256;          // sources per shared-memory tile == carriers per compaction tile
-constexpr uint32_t kPartFactor = 40;      // partial-sum slots per carrier of capacity (upper bound on j-splits)
+constexpr uint32_t kPartFactor = 16;      // partial-sum chunks a handle can hold at full capacity (gcoreccd.cu make_layout)
 constexpr float kSentinel = 1.0e18f;      // padding source: (1e18)^-3 underflows to 0, contribution exactly 0
 
 // Work plan of the field kernel: the N_a x N_a interaction matrix is cut into nIB row blocks
@@ -45,8 +45,16 @@ struct Ctrl {                 // lives in device memory; only kernels write it (
   uint32_t multi_steps;       // scratch of the Coulomb-off multi-step kernel: steps the longest-lived carrier took
   FieldPlan plan;             // valid for (n_active, current field variant, shard)
   uint32_t diverged;          // sticky: a shard message disagreed with this rank's (n_active, step) (gc_shard.cuh)
-  uint32_t pad2_;
+  uint32_t ticket;            // tile tickets of k_advance (look-back needs tiles in start order); 0 between launches
+  uint32_t scan_seq;          // executed look-back scans: the stamp that tells this step's status words from stale ones
+  uint32_t pad2_[5];
+  // second 128-byte line: polled by the persistent kernel's grid barrier, kept away from the line everybody reads
+  uint32_t bar;               // arrivals since the launch began; 0 between launches
+  uint32_t bar_exit;          // CTAs that left the persistent kernel; 0 between launches
+  uint32_t bar_gen;           // grid barriers executed since the last reset (the value the per-CTA flags hold)
+  uint32_t pad3_[29];
 };
+static_assert(sizeof(Ctrl) == 256, "Ctrl is two 128-byte lines");
 
 struct SoA {                  // one state set
   float* x; float* y; float* z; uint32_t* id;

@@ -62,18 +62,16 @@ struct FieldCfg {
 
 // Partial sums: Ep is three planes (x,y,z) of part_cap floats each; plane c, chunk s, target i at
 // Ep[c*part_cap + s*stride + (i - t0)], [t0, t0+nt) being the targets this rank owns (all of them if unsharded).  The value stored is sum (r_s - r_t) w = -S_t (sign folded by the consumer).
-template <int NPACK, int TPB, int MINB, int UNROLL = 4>
-__global__ void __launch_bounds__(TPB, MINB)
-k_field(const float* __restrict__ px, const float* __restrict__ py, const float* __restrict__ pz,
-        const Ctrl* __restrict__ ctrl, float* __restrict__ Ep, uint32_t part_cap, float eps2) {
+//
+// field_items: the work items of `plan` dealt round-robin to this CTA.  Called by k_field (one launch per evaluation)
+// and by the persistent multi-step kernel (gc_persist.cuh), in which the state changes between two calls inside ONE
+// launch: every load of the state goes to L2 (ld.global.cg), never through the non-coherent path.
+template <int NPACK, int TPB, int UNROLL>
+__device__ __forceinline__ void field_items(const float* px, const float* py, const float* pz, const FieldPlan& plan, float* Ep,
+                                            uint32_t part_cap, float eps2, float4 (&s_xy)[2][TPB], float2 (&s_z)[2][TPB]) {
   constexpr int IB = FieldCfg<NPACK, TPB>::kIB;
   constexpr int kTile = TPB;                            // sources per shared-memory tile: one per thread
-  __shared__ float4 s_xy[2][kTile];   // (x,x,y,y) per source
-  __shared__ float2 s_z[2][kTile];    // (z,z)
-
-  const FieldPlan plan = ctrl->plan;
   const uint32_t n = plan.n;
-  if (n == 0) return;
   const uint32_t tid = threadIdx.x;
   const uint32_t items = plan.nIB * plan.S;
   const float2 eps2v = make_float2(eps2, eps2);
@@ -85,6 +83,15 @@ k_field(const float* __restrict__ px, const float* __restrict__ py, const float*
     const uint32_t j0 = sc * plan.JC;
     const uint32_t j1 = min(j0 + plan.JC, n);
 
+    // first source tile: issued before the target loads so that both L2 round trips overlap
+    uint32_t jt = j0;
+    float sx, sy, sz;
+    {
+      const uint32_t j = jt + tid;
+      const bool ok = j < j1;
+      sx = ok ? __ldcg(px + j) : kSentinel; sy = ok ? __ldcg(py + j) : kSentinel; sz = ok ? __ldcg(pz + j) : kSentinel;
+    }
+
     // this thread's targets, negated: d = r_s + (-r_t)
     float2 ntx[NPACK], nty[NPACK], ntz[NPACK];
     float2 tx[NPACK], ty[NPACK], tz[NPACK];          // per-chunk totals
@@ -93,24 +100,17 @@ k_field(const float* __restrict__ px, const float* __restrict__ py, const float*
       const uint32_t i0 = i_base + (p * TPB + tid) * 2u;
       float2 vx = make_float2(0.f, 0.f), vy = vx, vz = vx;
       if (i0 + 1 < i_end) {                           // arrays are padded, but keep padding out of the math
-        vx = *reinterpret_cast<const float2*>(px + i0);
-        vy = *reinterpret_cast<const float2*>(py + i0);
-        vz = *reinterpret_cast<const float2*>(pz + i0);
+        vx = __ldcg(reinterpret_cast<const float2*>(px + i0));
+        vy = __ldcg(reinterpret_cast<const float2*>(py + i0));
+        vz = __ldcg(reinterpret_cast<const float2*>(pz + i0));
       } else if (i0 < i_end) {
-        vx.x = px[i0]; vy.x = py[i0]; vz.x = pz[i0];
+        vx.x = __ldcg(px + i0); vy.x = __ldcg(py + i0); vz.x = __ldcg(pz + i0);
       }
       ntx[p] = make_float2(-vx.x, -vx.y); nty[p] = make_float2(-vy.x, -vy.y); ntz[p] = make_float2(-vz.x, -vz.y);
       tx[p] = make_float2(0.f, 0.f); ty[p] = tx[p]; tz[p] = tx[p];
     }
 
     // software pipeline: registers hold tile k+1 while tile k is consumed from shared memory
-    uint32_t jt = j0;
-    float sx, sy, sz;
-    {
-      const uint32_t j = jt + tid;
-      const bool ok = j < j1;
-      sx = ok ? px[j] : kSentinel; sy = ok ? py[j] : kSentinel; sz = ok ? pz[j] : kSentinel;
-    }
     int buf = 0;
     __syncthreads();                                  // previous item's readers are done with both buffers
     s_xy[buf][tid] = make_float4(sx, sx, sy, sy);
@@ -122,7 +122,7 @@ k_field(const float* __restrict__ px, const float* __restrict__ py, const float*
       if (jn < j1) {                                  // prefetch the next tile into registers
         const uint32_t j = jn + tid;
         const bool ok = j < j1;
-        sx = ok ? px[j] : kSentinel; sy = ok ? py[j] : kSentinel; sz = ok ? pz[j] : kSentinel;
+        sx = ok ? __ldcg(px + j) : kSentinel; sy = ok ? __ldcg(py + j) : kSentinel; sz = ok ? __ldcg(pz + j) : kSentinel;
       }
       const int len = (int)min((uint32_t)kTile, (j1 - jt + 3u) & ~3u);   // padded to the unroll factor with sentinels
 
@@ -161,6 +161,17 @@ k_field(const float* __restrict__ px, const float* __restrict__ py, const float*
       }
     }
   }
+}
+
+template <int NPACK, int TPB, int MINB, int UNROLL = 4>
+__global__ void __launch_bounds__(TPB, MINB)
+k_field(const float* __restrict__ px, const float* __restrict__ py, const float* __restrict__ pz,
+        const Ctrl* __restrict__ ctrl, float* __restrict__ Ep, uint32_t part_cap, float eps2) {
+  __shared__ float4 s_xy[2][TPB];   // (x,x,y,y) per source
+  __shared__ float2 s_z[2][TPB];    // (z,z)
+  const FieldPlan plan = ctrl->plan;
+  if (plan.n == 0) return;
+  field_items<NPACK, TPB, UNROLL>(px, py, pz, plan, Ep, part_cap, eps2, s_xy, s_z);
 }
 
 }  // namespace gc

@@ -28,17 +28,29 @@ __device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint2 k) {
 
 // u = ((w>>9)+0.5) 2^-23 in (0,1); f = (w>>8) 2^-24 in [0,1): exactly representable in FP32 and FP64.
 // n = (R_a cos 2 pi f_a, R_a sin 2 pi f_a, R_b cos 2 pi f_b), R = sqrt(-2 ln u).
+// The draw is written as four independent chains (R_a | sin, cos | R_b | cos) so that the small-population kernel
+// (gc_persist.cuh) can give each to a thread of its own; one thread running all four computes the same bits.
+struct BoxMuller { double Ra, sa, ca, Rb, cb; };
+__device__ __forceinline__ uint4 philox_words(uint32_t seed_lo, uint32_t seed_hi, uint32_t id, uint64_t step) {
+  return philox4x32_10(make_uint4(id, 0u, (uint32_t)step, (uint32_t)(step >> 32)), make_uint2(seed_lo, seed_hi));
+}
+__device__ __forceinline__ double bm_radius(uint32_t w) {
+  const double u = ((double)(w >> 9) + 0.5) * (1.0 / 8388608.0);
+  return sqrt(-2.0 * log(u));
+}
+__device__ __forceinline__ double bm_fraction(uint32_t w) { return (double)(w >> 8) * (1.0 / 16777216.0); }
+__device__ __forceinline__ void bm_chain(const uint4 w, int chain, BoxMuller& b) {   // chain 0..3, or -1 = all
+  if (chain == 0 || chain < 0) b.Ra = bm_radius(w.x);
+  if (chain == 1 || chain < 0) sincospi(2.0 * bm_fraction(w.y), &b.sa, &b.ca);
+  if (chain == 2 || chain < 0) b.Rb = bm_radius(w.z);
+  if (chain == 3 || chain < 0) b.cb = cospi(2.0 * bm_fraction(w.w));
+}
 __device__ __forceinline__ void philox_normals(uint32_t seed_lo, uint32_t seed_hi, uint32_t id, uint64_t step,
                                                double n[3], uint4* words) {
-  const uint4 w = philox4x32_10(make_uint4(id, 0u, (uint32_t)step, (uint32_t)(step >> 32)), make_uint2(seed_lo, seed_hi));
-  const double ua = ((double)(w.x >> 9) + 0.5) * (1.0 / 8388608.0);
-  const double fa = (double)(w.y >> 8) * (1.0 / 16777216.0);
-  const double ub = ((double)(w.z >> 9) + 0.5) * (1.0 / 8388608.0);
-  const double fb = (double)(w.w >> 8) * (1.0 / 16777216.0);
-  const double Ra = sqrt(-2.0 * log(ua)), Rb = sqrt(-2.0 * log(ub));
-  double sa, ca;
-  sincospi(2.0 * fa, &sa, &ca);
-  n[0] = Ra * ca; n[1] = Ra * sa; n[2] = Rb * cospi(2.0 * fb);
+  const uint4 w = philox_words(seed_lo, seed_hi, id, step);
+  BoxMuller b;
+  bm_chain(w, -1, b);
+  n[0] = b.Ra * b.ca; n[1] = b.Ra * b.sa; n[2] = b.Rb * b.cb;
   if (words) *words = w;
 }
 
@@ -85,18 +97,17 @@ __device__ __forceinline__ void reduce_partials(const float* __restrict__ e, uin
   }
 }
 
-// a2..a6 for one carrier: (Ex,Ey,Ez) is its Coulomb field in V/cm (eq. 6); returns the new FP32 position, i.e. the
-// correctly rounded value of the FP64 expression the oracle evaluates.  False if the result is not finite.
-__device__ __forceinline__ bool advance_carrier(float x, float y, float z, uint32_t id, uint64_t step, double Ex, double Ey,
-                                                double Ez, const DevParams& P, float& xf, float& yf, float& zf) {
+// a2..a6 for one carrier: (Ex,Ey,Ez) is its Coulomb field in V/cm (eq. 6), nrm its normal triple (unused with
+// DIFFUSION_OFF); returns the new FP32 position, i.e. the correctly rounded value of the FP64 expression the oracle
+// evaluates.  False if the result is not finite.
+__device__ __forceinline__ bool advance_with_normals(float x, float y, float z, double Ex, double Ey, double Ez, const double nrm[3],
+                                                     const DevParams& P, float& xf, float& yf, float& zf) {
   if (!(P.flags & 4u)) Ez += P.a1_um * (double)z - P.a2;     // eq. 1
   const double Emag = sqrt(Ex * Ex + Ey * Ey + Ez * Ez);
   const double mu = mobility(Emag, P);                       // eq. 2
   const double kd = P.drift_k * mu;                          // 1e-5 mu dt
   double dx = kd * Ex, dy = kd * Ey, dz = kd * Ez;
   if (!(P.flags & 2u)) {                                     // eqs. 3-4
-    double nrm[3];
-    philox_normals(P.seed_lo, P.seed_hi, id, step, nrm, nullptr);
     const double sigma = sqrt(P.sigma_k * mu);
     dx += sigma * nrm[0]; dy += sigma * nrm[1]; dz += sigma * nrm[2];
   }
@@ -105,6 +116,13 @@ __device__ __forceinline__ bool advance_carrier(float x, float y, float z, uint3
   if (zn > P.thickness) zn = 2.0 * P.thickness - zn;         // specular back surface
   xf = (float)xn; yf = (float)yn; zf = (float)zn;
   return isfinite(xf) && isfinite(yf) && isfinite(zf);
+}
+
+__device__ __forceinline__ bool advance_carrier(float x, float y, float z, uint32_t id, uint64_t step, double Ex, double Ey,
+                                                double Ez, const DevParams& P, float& xf, float& yf, float& zf) {
+  double nrm[3] = {0.0, 0.0, 0.0};
+  if (!(P.flags & 2u)) philox_normals(P.seed_lo, P.seed_hi, id, step, nrm, nullptr);
+  return advance_with_normals(x, y, z, Ex, Ey, Ez, nrm, P, xf, yf, zf);
 }
 
 // Block-level tally of (collected, overflow) and the survivor count of this tile.

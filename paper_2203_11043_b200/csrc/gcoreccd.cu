@@ -12,11 +12,13 @@
 #include <vector>
 
 #include "gc_common.cuh"
+#include "gc_advance.cuh"
 #include "gc_compact.cuh"
 #include "gc_events.cuh"
 #include "gc_field.cuh"
 #include "gc_frontend.cuh"
 #include "gc_integrate.cuh"
+#include "gc_persist.cuh"
 #include "gc_shard.cuh"
 #include "gc_tree.cuh"
 
@@ -24,13 +26,17 @@ using namespace gc;
 
 namespace {
 
-constexpr uint64_t kMaxCarriers = 1ull << 26;
-constexpr int kNumVariants = 3;                       // field kernel register-blocking variants
+constexpr uint64_t kMaxCarriers = GCORECCD_MAX_CARRIERS;
+constexpr uint64_t kBarFlags = 1024;                       // >= the largest cooperative grid (4 CTAs x 148 SMs)
+constexpr uint64_t kPersistMaxDefault = 24576;          // populations up to this run many steps per launch (gc_persist.cuh)
+constexpr uint64_t kPersistMaxLimit = 37888;            // 148 CTAs x 256: beyond, the one-step kernels are as fast
+constexpr int kNumVariants = 6;                       // 0-2: one-step field kernels (2/4/8 targets per thread); 3-4: persistent
+                                                      // multi-step kernels (4/8 targets per thread), 5: 2 targets per thread on 96 SMs for < 3,072 holes, gc_persist.cuh
 constexpr int kGraphSteps = 8;                        // steps per CUDA-graph launch
 
 struct Layout {
-  uint64_t cap_pad, part_cap, n_tiles;
-  uint64_t off_ctrl, off_A, off_B, off_Ep, off_tiles, off_image, off_fin, total;
+  uint64_t cap_pad, part_cap, n_tiles, scan_entries, tree_scratch;
+  uint64_t off_ctrl, off_A, off_B, off_Ep, off_tiles, off_scan, off_flags, off_image, off_fin, total;
 };
 
 inline uint64_t align_up(uint64_t v, uint64_t a) { return (v + a - 1) / a * a; }
@@ -38,14 +44,21 @@ inline uint64_t align_up(uint64_t v, uint64_t a) { return (v + a - 1) / a * a; }
 Layout make_layout(uint64_t max_carriers, int32_t nx, int32_t ny) {
   Layout L;
   L.cap_pad = align_up(max_carriers, 1024);
-  L.part_cap = (uint64_t)kPartFactor * L.cap_pad;
+  // Partial planes: S chunks x stride (= n_active rounded to 256) entries each.  A large population is balanced over
+  // the SMs with few chunks (64+ row blocks x 16 chunks = 7+ rounds of 148 CTAs, <= 1.5 % idle), a small one needs many
+  // (8 row blocks at 4,096 holes): 16 chunks at capacity, and never fewer entries than 64 chunks of 32,768 holes.
+  L.part_cap = std::max<uint64_t>((uint64_t)kPartFactor * L.cap_pad, 64ull * std::min<uint64_t>(L.cap_pad, 32768));
+  L.tree_scratch = 8 * L.cap_pad + 4096;                  // far-field variant: tail of plane x (see gcoreccd_create)
   L.n_tiles = L.cap_pad / kTPB;
+  L.scan_entries = std::max<uint64_t>(L.n_tiles, 1024);   // look-back status words: 256-carrier tiles, or 64-carrier tiles of <= 65,536 holes
   uint64_t o = 0;
   L.off_ctrl = o;  o += align_up(sizeof(Ctrl), 256);
   L.off_A = o;     o += align_up(4 * L.cap_pad * 4, 256);
   L.off_B = o;     o += align_up(4 * L.cap_pad * 4, 256);
   L.off_Ep = o;    o += align_up(3 * L.part_cap * 4, 256);
   L.off_tiles = o; o += align_up(L.n_tiles * 4, 256);
+  L.off_scan = o;  o += align_up(L.scan_entries * 8, 256);
+  L.off_flags = o; o += kBarFlags * 128;                  // one 128-byte line per CTA of the persistent kernel's grid barrier
   L.off_image = o; o += align_up((uint64_t)nx * (uint64_t)ny * 4, 256);
   L.off_fin = o;   o += align_up(L.cap_pad * 16, 256);
   L.total = o;
@@ -89,13 +102,15 @@ struct gcoreccd {
   SoA A, B;
   float* Ep;
   uint32_t* tile_count;
+  unsigned long long* scan;     // look-back status words (gc_advance.cuh)
+  uint32_t* bar_flags;          // per-CTA flags of the persistent kernel's grid barrier (gc_persist.cuh)
   uint32_t* image;
   float4* fin;                  // per-id collection records
   Sink sink;
   uint64_t n_loaded;            // host copy (ids continue)
   uint64_t n_bound;             // host upper bound on n_active
   int variant;                  // current field variant (-1 = none yet)
-  int grid_field[kNumVariants];
+  int grid_field[kNumVariants];       // persistent grid of each variant (3-4: co-resident CTAs of k_steps<>, cooperative launch)
   uint64_t launches;
   cudaGraphExec_t graph;
   int graph_variant;
@@ -104,6 +119,8 @@ struct gcoreccd {
   uint64_t graph_launches;            // kernels in the graph
   uint32_t graph_cadence;             // re-sort cadence baked into a treecode graph
   cudaEvent_t ev[4];
+  uint64_t persist_max;
+  bool persist_on;                    // many-steps-per-launch path for small populations (gc_persist.cuh); test hook turns it off
   uint32_t shard_rank, shard_world;   // target sharding (gc_shard.cuh); world 1 = not sharded
   bool ff_on;                         // far-field approximation (gc_tree.cuh)
   float ff_theta;
@@ -157,11 +174,20 @@ int fail(gcoreccd_t* h, int code, const char* what, cudaError_t e = cudaSuccess)
     if (e__ != cudaSuccess) return fail((h), GCORECCD_ERR_CUDA, #call, e__);   \
   } while (0)
 
-inline uint32_t variant_ib(int v) { return (uint32_t)kTPB * (2u << v); }     // 512, 1024, 2048 targets per row block
+inline int variant_npack(int v) { return (v == 0 || v == 5) ? 1 : (v == 1 || v == 3) ? 2 : 4; }
+inline uint32_t variant_ib(int v) { return (uint32_t)kTPB * 2u * (uint32_t)variant_npack(v); }   // targets per row block
+inline bool variant_persistent(int v) { return v >= 3; }
 
-inline int pick_variant(uint64_t n_bound) {
-  if (n_bound >= 12288) return 2;      // 8 targets/thread, 1 CTA/SM: highest FMA-pipe utilisation (76 %)
-  if (n_bound >= 3072) return 1;       // 4 targets/thread, 3 CTAs/SM: more row blocks for balance
+// Small populations run many steps per cooperative launch (gc_persist.cuh): all-pairs, unsharded handles only.
+inline bool persist_eligible(const gcoreccd_t* h, uint64_t n) {
+  return h->persist_on && !(h->dp.flags & GCORECCD_COULOMB_OFF) && h->shard_world == 1 && n <= h->persist_max &&
+         !(h->ff_on && n >= h->ff_min_active) && h->grid_field[3] > 0 && h->grid_field[4] > 0;
+}
+
+inline int pick_variant(const gcoreccd_t* h, uint64_t n) {
+  if (persist_eligible(h, n)) return n >= 12288 ? 4 : n >= 3072 ? 3 : 5;
+  if (n >= 12288) return 2;            // 8 targets/thread, 1 CTA/SM: highest FMA-pipe utilisation (76 %)
+  if (n >= 3072) return 1;             // 4 targets/thread, 3 CTAs/SM: more row blocks for balance
   return 0;                            // 2 targets/thread, 4 CTAs/SM
 }
 
@@ -171,7 +197,7 @@ inline PlanArgs plan_args(const gcoreccd_t* h, int v) {
   a.grid = (uint32_t)h->grid_field[v];
   // with the far-field variant on, the tail of the partial plane is the treecode's scratch (counters included): the
   // all-pairs kernel, which takes over below min_active holes, must not plan its chunks into it
-  a.part_cap_entries = (uint32_t)(h->ff_on ? h->L.part_cap - 10 * h->L.cap_pad : h->L.part_cap);
+  a.part_cap_entries = (uint32_t)(h->ff_on ? h->L.part_cap - h->L.tree_scratch : h->L.part_cap);
   a.rank = h->shard_rank;
   a.world = h->shard_world;
   a.force_S = h->ff_parts;
@@ -237,24 +263,35 @@ int launch_field(gcoreccd_t* h, int v) {
   if (h->ff_parts) return launch_tree_field(h);
   const int g = h->grid_field[v];
   const uint32_t pc = (uint32_t)h->L.part_cap;
-  switch (v) {
-    case 0: k_field<1, 256, 4><<<g, kTPB, 0, h->stream>>>(h->A.x, h->A.y, h->A.z, h->ctrl, h->Ep, pc, h->dp.eps2); break;
-    case 1: k_field<2, 256, 3><<<g, kTPB, 0, h->stream>>>(h->A.x, h->A.y, h->A.z, h->ctrl, h->Ep, pc, h->dp.eps2); break;
+  switch (variant_npack(v)) {            // the plan was made for this variant's grid g (persistent variants included)
+    case 1: k_field<1, 256, 4><<<g, kTPB, 0, h->stream>>>(h->A.x, h->A.y, h->A.z, h->ctrl, h->Ep, pc, h->dp.eps2); break;
+    case 2: k_field<2, 256, 3><<<g, kTPB, 0, h->stream>>>(h->A.x, h->A.y, h->A.z, h->ctrl, h->Ep, pc, h->dp.eps2); break;
     default: k_field<4, 256, 1><<<g, kTPB, 0, h->stream>>>(h->A.x, h->A.y, h->A.z, h->ctrl, h->Ep, pc, h->dp.eps2); break;
   }
   h->launches += 1;
   return 0;
 }
 
-// one time step = field + integrate + compact, all reading n_active / plan from device memory
+// one time step = field (a1) + advance (a2..a8: update, collection, in-place compaction), both reading n_active / the
+// plan from device memory
 void enqueue_step(gcoreccd_t* h, uint32_t tiles) {
   const bool coulomb = !(h->dp.flags & GCORECCD_COULOMB_OFF);
   if (coulomb) launch_field(h, h->variant);
-  k_integrate<<<tiles, kTPB, 0, h->stream>>>(h->A, h->B, h->ctrl, h->Ep, (uint32_t)h->L.part_cap, h->sink,
-                                             h->tile_count, h->dp);
-  k_compact<<<tiles, kTPB, 0, h->stream>>>(h->B, h->A, h->ctrl, h->tile_count, 0u, 0u, 0, h->dp.z_well,
-                                           coulomb ? 1u : 0u, plan_args(h, h->variant));
-  h->launches += 2;
+  k_advance<<<tiles, kTPB, 0, h->stream>>>(h->A, h->ctrl, h->Ep, (uint32_t)h->L.part_cap, h->sink, h->scan, h->dp,
+                                           plan_args(h, h->variant), coulomb ? 1u : 0u);
+  h->launches += 1;
+}
+
+// Small populations: up to 2^20 steps in ONE cooperative launch (gc_persist.cuh).
+int launch_persistent(gcoreccd_t* h, uint32_t n_steps) {
+  const int v = h->variant;
+  SoA A = h->A; SoA B = h->B; Ctrl* ctrl = h->ctrl; float* Ep = h->Ep; uint32_t pc = (uint32_t)h->L.part_cap; Sink sink = h->sink;
+  unsigned long long* scan = h->scan; uint32_t* flags = h->bar_flags; DevParams dp = h->dp; PlanArgs pa = plan_args(h, v);
+  void* args[] = {&A, &B, &ctrl, &Ep, &pc, &sink, &scan, &flags, &dp, &pa, &n_steps};
+  const void* fn = v == 4 ? (const void*)k_steps<4, 1> : v == 3 ? (const void*)k_steps<2, 2> : (const void*)k_steps<1, 2>;
+  GC_CUDA(h, cudaLaunchCooperativeKernel(fn, dim3((unsigned)h->grid_field[v]), dim3(kTPB), args, 0, h->stream));
+  h->launches += 1;
+  return 0;
 }
 
 // parts per treecode group: enough work items for ~1.5 per resident CTA, power of two, at most 8 (workspace layout)
@@ -266,7 +303,7 @@ inline uint32_t pick_parts(const gcoreccd_t* h) {
 }
 
 int ensure_variant(gcoreccd_t* h) {
-  const int v = pick_variant(h->n_bound);
+  const int v = pick_variant(h, h->n_bound);
   const uint32_t parts = h->ff_on && h->n_bound >= h->ff_min_active ? pick_parts(h) : 0u;
   if (v != h->variant || parts != h->ff_parts) {
     h->ff_parts = parts;
@@ -343,12 +380,21 @@ int enqueue_steps(gcoreccd_t* h, uint64_t n_steps) {
     while (n_steps > 0) {
       const uint32_t chunk = (uint32_t)std::min<uint64_t>(n_steps, 1u << 30);
       k_drift_multi<<<tiles, kTPB, 0, h->stream>>>(h->A, h->B, h->ctrl, h->sink, h->tile_count, h->dp, chunk);
-      k_compact<<<tiles, kTPB, 0, h->stream>>>(h->B, h->A, h->ctrl, h->tile_count, 0u, 0u, 2, h->dp.z_well, 0u,
+      k_compact<<<tiles, kTPB, 0, h->stream>>>(h->B, h->A, h->ctrl, h->tile_count, h->scan, 0u, 0u, 2, h->dp.z_well, 0u,
                                                plan_args(h, h->variant));
       h->launches += 2;
       n_steps -= chunk;
     }
     GC_CUDA(h, cudaGetLastError());
+    return 0;
+  }
+  if (variant_persistent(h->variant)) {
+    while (n_steps > 0) {
+      const uint32_t chunk = (uint32_t)std::min<uint64_t>(n_steps, 1u << 20);
+      rc = launch_persistent(h, chunk);
+      if (rc) return rc;
+      n_steps -= chunk;
+    }
     return 0;
   }
   // stream capture is not permitted on the legacy / per-thread default streams: plain launches there
@@ -428,6 +474,8 @@ int gcoreccd_create(const gcoreccd_params* p, gcoreccd_t** out) {
   h->num_sms = prop.multiProcessorCount;
   h->variant = -1;
   h->shard_world = 1;
+  h->persist_on = true;
+  h->persist_max = kPersistMaxDefault;
   DeviceGuard guard(dev);
 
   h->L = make_layout(p->max_carriers, p->img_nx, p->img_ny);
@@ -466,6 +514,8 @@ int gcoreccd_create(const gcoreccd_params* p, gcoreccd_t** out) {
   h->B = SoA{b, b + cp, b + 2 * cp, (uint32_t*)(b + 3 * cp)};
   h->Ep = (float*)(h->ws + h->L.off_Ep);
   h->tile_count = (uint32_t*)(h->ws + h->L.off_tiles);
+  h->scan = (unsigned long long*)(h->ws + h->L.off_scan);
+  h->bar_flags = (uint32_t*)(h->ws + h->L.off_flags);
   h->image = (uint32_t*)(h->ws + h->L.off_image);
   h->fin = (float4*)(h->ws + h->L.off_fin);
   h->sink = Sink{h->image, h->fin, (uint32_t)std::min<uint64_t>(p->max_carriers, 0xffffffffull)};
@@ -494,19 +544,29 @@ int gcoreccd_create(const gcoreccd_params* p, gcoreccd_t** out) {
   d.nx = p->img_nx; d.ny = p->img_ny;
 
   // persistent grid of the field kernel: resident CTAs per SM x SM count
-  int occ[kNumVariants] = {0, 0, 0};
+  int occ[kNumVariants] = {0, 0, 0, 0, 0, 0};
   e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[0], k_field<1, 256, 4>, kTPB, 0);
   if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[1], k_field<2, 256, 3>, kTPB, 0);
   if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[2], k_field<4, 256, 1>, kTPB, 0);
+  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[3], k_steps<2, 2>, kTPB, 0);
+  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[4], k_steps<4, 1>, kTPB, 0);
+  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[5], k_steps<1, 2>, kTPB, 0);
   if (e != cudaSuccess) { fail(h, GCORECCD_ERR_CUDA, "occupancy query", e); gcoreccd_destroy(h); return GCORECCD_ERR_CUDA; }
-  for (int v = 0; v < kNumVariants; ++v) h->grid_field[v] = h->num_sms * (occ[v] > 0 ? occ[v] : 1);
+  for (int v = 0; v < 3; ++v) h->grid_field[v] = h->num_sms * (occ[v] > 0 ? occ[v] : 1);
+  int coop = 0;
+  cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+  for (int v = 3; v < 5; ++v) h->grid_field[v] = coop ? h->num_sms * std::min(occ[v], v == 3 ? 2 : 1) : 0;   // 0: no persistent path
+  // < 3,072 holes: 96 tiles of 32 carriers at most; every CTA that only waits at the grid barriers makes them slower
+  h->grid_field[5] = coop && occ[5] > 0 ? std::min(h->num_sms, 96) : 0;
   int occ_tree = 0;
   e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_tree, k_tree_field, kTreeTPB, 0);
   if (e != cudaSuccess) { fail(h, GCORECCD_ERR_CUDA, "occupancy query", e); gcoreccd_destroy(h); return GCORECCD_ERR_CUDA; }
   h->grid_tree = h->num_sms * (occ_tree > 0 ? occ_tree : 1);
   {
-    // treecode scratch: the last 10 cap_pad floats of partial plane 0 (free while S <= 8; the load paths stage at its start)
-    float* r = h->Ep + (h->L.part_cap - 10 * cp);
+    // treecode scratch: the last 8 cap_pad + 4,096 floats of partial plane x.  The treecode writes P <= 8 chunks, and
+    // P > 1 only below ~35k holes (pick_parts), so its chunks end far below; with the variant on, the all-pairs plan is
+    // confined to the entries in front of the scratch (plan_args); the load paths stage in the first 4 cap_pad floats.
+    float* r = h->Ep + (h->L.part_cap - h->L.tree_scratch);
     Tree& T = h->tree;
     T.tc = (TreeCtrl*)r;                         r += 2048;                 // 6.2 KB: box, counters, digit totals
     T.node_c = (float4*)r;                       r += cp * 5 / 8 + 64;      // <= cp/7 + 9 nodes of 4 floats
@@ -542,6 +602,8 @@ int gcoreccd_reset(gcoreccd_t* h) {
   if (!h) return GCORECCD_ERR_INVALID;
   DeviceGuard guard(h->device);
   GC_CUDA(h, cudaMemsetAsync(h->ctrl, 0, sizeof(Ctrl), h->stream));
+  GC_CUDA(h, cudaMemsetAsync(h->scan, 0, (size_t)h->L.scan_entries * 8, h->stream));   // scan_seq restarts: no stale stamps
+  GC_CUDA(h, cudaMemsetAsync(h->bar_flags, 0, kBarFlags * 128, h->stream));            // bar_gen restarts likewise
   GC_CUDA(h, cudaMemsetAsync(h->image, 0, (size_t)h->p.img_nx * h->p.img_ny * 4, h->stream));
   GC_CUDA(h, cudaMemsetAsync(h->fin, 0xff, (size_t)h->L.cap_pad * 16, h->stream));     // NaN / all-ones = still drifting
   if (h->ff_on) GC_CUDA(h, cudaMemsetAsync(h->tree.tc, 0, sizeof(TreeCtrl), h->stream)); // far-field counters restart too
@@ -579,11 +641,11 @@ int gcoreccd_load_carriers(gcoreccd_t* h, const float* xyz, uint64_t n, int on_d
   if (rc) return rc;
   if (h->h_ctrl->invalid) return fail(h, GCORECCD_ERR_INVALID, "load_carriers: non-finite coordinate or z > thickness");
   // the plan stored with the new n_active must match the variant the next step will use
-  const int v = pick_variant(n_act + n);
+  const int v = pick_variant(h, n_act + n);
   h->variant = v;
   k_unpack<<<tiles, kTPB, 0, h->stream>>>(src, (uint32_t)n, h->B, h->ctrl, (uint32_t)h->n_loaded, h->sink,
                                           h->tile_count, h->dp, h->shard_rank == 0 ? 1u : 0u);
-  k_compact<<<tiles, kTPB, 0, h->stream>>>(h->B, h->A, h->ctrl, h->tile_count, (uint32_t)n, (uint32_t)n_act, 1,
+  k_compact<<<tiles, kTPB, 0, h->stream>>>(h->B, h->A, h->ctrl, h->tile_count, h->scan, (uint32_t)n, (uint32_t)n_act, 1,
                                            h->dp.z_well, 0u, plan_args(h, v));
   h->launches += 2;
   GC_CUDA(h, cudaGetLastError());
@@ -618,7 +680,7 @@ int gcoreccd_load_snapshot(gcoreccd_t* h, const float* xyz, const uint32_t* id, 
     h->launches += 1;
   }
   // sharded handles: every rank loads the same snapshot; the plan below is this rank's share of it
-  const int v = pick_variant(h->shard_world > 1 ? (n + h->shard_world - 1) / h->shard_world : n);
+  const int v = pick_variant(h, h->shard_world > 1 ? (n + h->shard_world - 1) / h->shard_world : n);
   h->variant = v;
   h->ff_parts = 0;
   k_replan<<<1, 32, 0, h->stream>>>(h->ctrl, plan_args(h, v), 1, (uint32_t)n, 1, step);
@@ -772,13 +834,11 @@ int gcoreccd_profile_step(gcoreccd_t* h, float ms[4]) {
   GC_CUDA(h, cudaEventRecord(h->ev[0], h->stream));
   if (coulomb) launch_field(h, h->variant);
   GC_CUDA(h, cudaEventRecord(h->ev[1], h->stream));
-  k_integrate<<<tiles, kTPB, 0, h->stream>>>(h->A, h->B, h->ctrl, h->Ep, (uint32_t)h->L.part_cap, h->sink,
-                                             h->tile_count, h->dp);
+  k_advance<<<tiles, kTPB, 0, h->stream>>>(h->A, h->ctrl, h->Ep, (uint32_t)h->L.part_cap, h->sink, h->scan, h->dp,
+                                           plan_args(h, h->variant), coulomb ? 1u : 0u);
   GC_CUDA(h, cudaEventRecord(h->ev[2], h->stream));
-  k_compact<<<tiles, kTPB, 0, h->stream>>>(h->B, h->A, h->ctrl, h->tile_count, 0u, 0u, 0, h->dp.z_well,
-                                           coulomb ? 1u : 0u, plan_args(h, h->variant));
   GC_CUDA(h, cudaEventRecord(h->ev[3], h->stream));
-  h->launches += 2;
+  h->launches += 1;
   GC_CUDA(h, cudaGetLastError());
   rc = sync_ctrl(h);
   if (rc) return rc;
@@ -786,6 +846,14 @@ int gcoreccd_profile_step(gcoreccd_t* h, float ms[4]) {
   GC_CUDA(h, cudaEventElapsedTime(&ms[1], h->ev[1], h->ev[2]));
   GC_CUDA(h, cudaEventElapsedTime(&ms[2], h->ev[2], h->ev[3]));
   GC_CUDA(h, cudaEventElapsedTime(&ms[3], h->ev[0], h->ev[3]));
+  return GCORECCD_OK;
+}
+
+int gcoreccd_set_persistent(gcoreccd_t* h, int on, uint64_t max_active) {
+  if (!h || max_active > kPersistMaxLimit) return GCORECCD_ERR_INVALID;
+  h->persist_on = on != 0;
+  h->persist_max = max_active ? max_active : kPersistMaxDefault;
+  h->variant = -1;                                         // re-pick the kernel variant (and re-plan) at the next step
   return GCORECCD_OK;
 }
 
@@ -830,7 +898,7 @@ int gcoreccd_shard_local(gcoreccd_t* h, void* msg_dev, uint64_t msg_bytes) {
   if ((uintptr_t)msg_dev & 15u) return fail(h, GCORECCD_ERR_INVALID, "shard_local: message buffer must be 16-byte aligned");
   DeviceGuard guard(h->device);
   // the share shrinks with n_active: pick the field variant from the share, not from the whole population
-  const int v = pick_variant((h->n_bound + h->shard_world - 1) / h->shard_world);
+  const int v = pick_variant(h, (h->n_bound + h->shard_world - 1) / h->shard_world);
   const uint32_t parts = h->ff_on && h->n_bound >= h->ff_min_active ? pick_parts(h) : 0u;   // treecode walk of the share
   if (v != h->variant || parts != h->ff_parts) {
     h->variant = v;
@@ -1307,6 +1375,12 @@ int gcoreccd_save_collected_file(gcoreccd_t* h, const char* path, uint64_t* n_wr
   if (n_written) *n_written = w;
   return ok ? GCORECCD_OK : fail(h, GCORECCD_ERR_INVALID, "save_collected_file: write failed");
 }
+
+#ifdef GC_TIMING
+int gcoreccd_debug_timing(long long* out) {      // development builds only (-DGC_TIMING): phase timestamps of k_steps
+  return cudaMemcpyFromSymbol(out, gc::g_dbg, sizeof(gc::g_dbg)) == cudaSuccess ? 0 : -5;
+}
+#endif
 
 const char* gcoreccd_strerror(int code) {
   switch (code) {

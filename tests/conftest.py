@@ -28,3 +28,23 @@ def read_golden(name):
 @pytest.fixture(scope="session")
 def golden():
     return read_golden
+
+
+def pytest_terminal_summary(terminalreporter):
+    """DESIGN.md R21: how many carriers used the close-encounter excuse, over all trajectory checks of the session."""
+    try:
+        from util import EXCUSED
+    except Exception:
+        return
+    if not EXCUSED:
+        return
+    log = os.environ.get("GCORECCD_EXCUSE_LOG")
+    if log:
+        with open(log, "w") as f:
+            for lab, n, k, rs in EXCUSED:
+                f.write("%d %d %s %s\n" % (k, n, lab, rs))
+    tot = sum(e[1] for e in EXCUSED)
+    exc = sum(e[2] for e in EXCUSED)
+    terminalreporter.write_line("R21 excuse clause: %d trajectory checks, %d carriers compared, %d excused (%.4f %%); "
+                                "largest single check: %d" % (len(EXCUSED), tot, exc, 100.0 * exc / max(tot, 1),
+                                                                max(e[2] for e in EXCUSED)))

@@ -289,3 +289,24 @@ def test_farfield_counters_survive_the_switch_to_the_all_pairs_kernel():
     assert after["far_evals"] == 0 and after["near_evals"] == 0      # set_farfield restarts them; nothing tramples them
     assert sim.state()["step"] == 10
     sim.close()
+
+
+def test_a_cached_graph_is_not_replayed_on_a_larger_population():
+    """Far-field steps are captured into CUDA graphs whose grids follow the population at capture time; a reset or a
+    further load must drop them (same tile bucket, same parts, same cadence: the graph key alone cannot tell)."""
+    wa, wb = workloads.make(3, n=25000), workloads.make(3, n=30000)
+    sim = gpu_sim(wb, max_carriers=30000)
+    sim.set_farfield(0.4, min_active=1000)
+    sim.load_carriers(wa["xyz"])
+    sim.step(16)                                                              # graphs captured for <= 25,000 holes
+    sim.reset()
+    sim.load_carriers(wb["xyz"])
+    sim.step(16)
+    fresh = gpu_sim(wb, max_carriers=30000)
+    fresh.set_farfield(0.4, min_active=1000)
+    fresh.load_carriers(wb["xyz"])
+    fresh.step(16)
+    (xa, ia), (xb, ib) = sim.read_carriers(), fresh.read_carriers()
+    assert np.array_equal(ia, ib) and np.array_equal(xa, xb)
+    assert sim.state() == fresh.state()
+    sim.close(); fresh.close()

@@ -1,0 +1,233 @@
+"""GPU parity (-m gpu) of WHOLE EVENTS and of full-size 10-step windows against stored oracle results.
+
+The oracle cannot run configs 1-4 in full inside a GPU test, so committed oracle-only scripts did it once on CPU:
+  tests/golden/make_full_run_goldens.py  -> full_run_cfg{1,2}.txt   (load -> full collection: image, per-cloud moments,
+                                                                    population decay, step count, sum N_a^2)
+  tests/golden/make_trajectory_goldens.py -> traj10_cfg{2,3,4}.txt  (first 10 steps at full size, sampled holes)
+Nothing in those files comes from the CUDA path.  BASELINE.json:north_star: "the collected image exactly conserving the
+hole count, with per-pixel charge and cloud second moments within 1%" and "trajectories within 1e-3 um after 10
+steps"; the system is chaotic (R16), so whole events are compared statistically (R22), never bit for bit.
+
+Also here: snapshot-restart parity at full size for configs 3 and 4 at steps {0, 10, 100, 500}.
+"""
+import os
+
+import numpy as np
+import pytest
+
+from conftest import GOLDEN, read_golden
+from oracle import goracle as g
+import workloads
+from util import field_rel_err, gpu_sim, oracle_params
+
+pytestmark = pytest.mark.gpu
+
+
+def _parse_full_run(name):
+    G = dict(decay=[], groups=[], px=[])
+    for r in read_golden(name):
+        if r[0] == "decay":
+            G["decay"].append((int(r[1]), int(r[2])))
+        elif r[0] == "group":
+            G["groups"].append((r[1], int(r[2]), int(r[3])) + tuple(float(v) for v in r[4:10]))
+        elif r[0] == "px":
+            G["px"].append((int(r[1]), int(r[2]), int(r[3])))
+        elif r[0] == "image_shape":
+            G["shape"] = (int(r[1]), int(r[2]))
+        else:
+            G[r[0]] = int(r[1])
+    img = np.zeros(G["shape"], dtype=np.int64)
+    for iy, ix, c in G["px"]:
+        img[iy, ix] = c
+    G["image"] = img
+    return G
+
+
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_whole_event_against_the_oracle_full_run(cfg):
+    name = "full_run_cfg%d.txt" % cfg
+    assert os.path.exists(os.path.join(GOLDEN, name)), "run tests/golden/make_full_run_goldens.py %d" % cfg
+    G = _parse_full_run(name)
+    w = workloads.make(cfg)
+    n0 = len(w["xyz"])
+    assert n0 == G["n_loaded"]
+    sim = gpu_sim(w)
+    sim.load_carriers(w["xyz"])
+    # population decay, sampled at the oracle's cadence (the loop runs until every charge has arrived)
+    every = G["decay"][1][0] - G["decay"][0][0]
+    worst_decay = 0.0
+    for s_ref, n_ref in G["decay"]:
+        st = sim.state()
+        if st["step"] < s_ref and st["n_active"] > 0:
+            sim.step(min(every, s_ref - st["step"]))
+            st = sim.state()
+        if st["step"] == s_ref:
+            dn = abs(st["n_active"] - n_ref)
+            worst_decay = max(worst_decay, dn / max(1.0, 4.0 * np.sqrt(min(n_ref, n0 - n_ref) + 1.0)))
+            assert dn <= max(0.01 * (n0 - n_ref), 4.0 * np.sqrt(min(n_ref, n0 - n_ref) + 1.0)), (s_ref, st["n_active"], n_ref)
+        img, over = sim.read_image()
+        assert int(img.sum()) + over + st["n_active"] == n0                 # conservation, every batch
+    done, left, rc = sim.run_to_collection(100000)
+    st = sim.state()
+    assert left == 0 and st["n_active"] == 0
+    img, over = sim.read_image()
+    # totals exact; step count and interaction count follow the oracle's
+    assert int(img.sum()) + over == n0 == int(G["image"].sum()) + G["out_of_window"]
+    assert abs(st["step"] - G["steps"]) <= 3, (st["step"], G["steps"])
+    assert st["pair_interactions"] == pytest.approx(G["pair_interactions"], rel=5e-3)
+    assert abs(over - G["out_of_window"]) <= max(0.01 * G["out_of_window"], 4.0 * np.sqrt(G["out_of_window"] + 1.0))
+    # per pixel, R22: |dn| <= max(1 % n_ref, 4 sqrt(n_ref + 1))
+    ref = G["image"]
+    dn = np.abs(img.astype(np.int64) - ref)
+    lim = np.maximum(0.01 * ref, 4.0 * np.sqrt(ref + 1.0))
+    assert np.all(dn <= lim), (int((dn > lim).sum()), int(dn.max()))
+    n_pct = int((0.01 * ref >= 4.0 * np.sqrt(ref + 1.0)).sum())             # pixels judged by the 1 % branch
+    big = ref >= 1000
+    rel_big = float((dn[big] / ref[big]).max()) if big.any() else 0.0
+    # per cloud: centroid and second moments of the collected (x, y) within 1 % (north_star)
+    fin, fstep = sim.read_collected()
+    assert np.isfinite(fin).all() and np.all(fstep != 0xFFFFFFFF)
+    worst_var = 0.0
+    for gname, lo, hi, mx, my, vx, vy, cxy, mstep in G["groups"]:
+        x, y = fin[lo:hi, 0].astype(np.float64), fin[lo:hi, 1].astype(np.float64)
+        sx, sy = np.sqrt(vx), np.sqrt(vy)
+        assert abs(x.mean() - mx) <= 0.01 * sx and abs(y.mean() - my) <= 0.01 * sy, gname
+        gvx, gvy = ((x - x.mean()) ** 2).mean(), ((y - y.mean()) ** 2).mean()
+        gcxy = ((x - x.mean()) * (y - y.mean())).mean()
+        worst_var = max(worst_var, abs(gvx / vx - 1.0), abs(gvy / vy - 1.0))
+        assert gvx == pytest.approx(vx, rel=0.01) and gvy == pytest.approx(vy, rel=0.01), gname
+        assert abs(gcxy - cxy) <= 0.01 * sx * sy, gname
+        assert fstep[lo:hi].astype(np.float64).mean() == pytest.approx(mstep, abs=0.5), gname
+    print("cfg%d whole event vs oracle: steps %d/%d, pixels lit %d, judged by the 1%% branch %d, max |dn| %d, "
+          "max rel. diff on pixels >= 1000 holes %.4f, worst decay/limit %.2f, worst cloud variance diff %.4f %%"
+          % (cfg, st["step"], G["steps"], int((ref > 0).sum()), n_pct, int(dn.max()), rel_big, worst_decay,
+             100.0 * worst_var))
+    sim.close()
+
+
+def _parse_traj(name):
+    T = dict(holes=[])
+    for r in read_golden(name):
+        if r[0] == "hole":
+            T["holes"].append((int(r[1]), float(r[2]), float(r[3]), float(r[4]), float(r[5])))
+        elif r[0] in ("n_active", "retired"):
+            T[r[0]] = [int(v) for v in r[1:]]
+        else:
+            T[r[0]] = int(r[1])
+    T.setdefault("retired", [])
+    return T
+
+
+@pytest.mark.parametrize("cfg", [2, 3, 4])
+def test_ten_step_trajectories_at_full_size_against_the_oracle(cfg):
+    name = "traj10_cfg%d.txt" % cfg
+    assert os.path.exists(os.path.join(GOLDEN, name)), "run tests/golden/make_trajectory_goldens.py %d" % cfg
+    T = _parse_traj(name)
+    w = workloads.make(cfg)
+    assert len(w["xyz"]) == T["n_loaded"]
+    sim = gpu_sim(w)
+    sim.load_carriers(w["xyz"])
+    assert sim.state()["n_active"] == T["n_active"][0]
+    mism = 0
+    for s in range(T["steps"]):
+        sim.step(1)
+        mism = max(mism, abs(sim.state()["n_active"] - T["n_active"][s + 1]))
+    assert mism <= 2 + 1e-5 * T["n_loaded"], mism                          # retire decisions at the plane (R21)
+    xyz, ids = sim.read_carriers()
+    hid = np.array([h[0] for h in T["holes"]], dtype=np.int64)
+    ref = np.array([h[1:4] for h in T["holes"]])
+    close = np.array([h[4] for h in T["holes"]])
+    k = np.searchsorted(ids, hid)
+    found = (k < len(ids))
+    found[found] &= ids[k[found]] == hid[found]
+    d = np.full(len(hid), np.inf)
+    d[found] = np.abs(xyz[k[found]].astype(np.float64) - ref[found]).max(axis=1)
+    suspects = d > 1e-3
+    # DESIGN.md R21: beyond 1e-3 um only after an oracle-side encounter closer than 0.1 um, and at most 2 % (+2)
+    assert suspects.sum() <= 0.02 * len(hid) + 2, int(suspects.sum())
+    assert np.all(close[suspects] < 0.1), (d[suspects], close[suspects])
+    gone = np.isin(np.array(T["retired"], dtype=np.int64), ids)
+    assert gone.sum() <= 1
+    from util import EXCUSED
+    EXCUSED.append(("cfg%d full size, %d sampled holes" % (cfg, len(hid)), len(hid), int(suspects.sum()),
+                    sorted(round(float(r), 4) for r in close[suspects])))
+    print("cfg%d 10 steps at full size: %d sampled holes, median %.2e um, p99 %.2e um, max (unexcused) %.2e um, excused %d"
+          % (cfg, len(hid), np.median(d[found]), np.quantile(d[found], 0.99), d[~suspects].max(), int(suspects.sum())))
+    sim.close()
+
+
+# ---------------------------------------------------------------- snapshot-restart at full size, configs 3 and 4
+def _restart_window(sim, w, rng, m, n_restarts):
+    """n_restarts consecutive one-step checks: the oracle advances m sampled carriers one step from the exported GPU
+    snapshot (needs only their fields: m targets x all sources) and is compared with the GPU's next step."""
+    P = w["params"]
+    op = oracle_params(w, flags=g.FP32_STATE)
+    worst, worst_field, mism = 0.0, 0.0, 0
+    for _ in range(n_restarts):
+        st = sim.state()
+        if st["n_active"] == 0:
+            break
+        xyz, ids = sim.read_carriers()
+        t = np.sort(rng.choice(len(xyz), size=min(m, len(xyz)), replace=False)).astype(np.uint64)
+        Eref = g.coulomb_field(xyz.astype(np.float64), eps_um=P["softening_um"], Kp=g.coulomb_constant(P["eps_si"]), targets=t)
+        E = sim.eval_field()
+        unfl, _ = field_rel_err(E[t.astype(np.int64)], Eref)
+        worst_field = max(worst_field, unfl)
+        sim.step(1)
+        xyz1, ids1 = sim.read_carriers()
+        order = np.argsort(ids1, kind="stable")                               # curve order after a far-field stretch
+        srt = ids1[order]
+        q = np.searchsorted(srt, ids[t.astype(np.int64)])
+        pos = order[np.minimum(q, len(srt) - 1)] if len(srt) else q
+        for k, j in enumerate(t.astype(np.int64)):
+            r_new, collected = g.advance(op, st["step"], int(ids[j]), xyz[j].astype(np.float64), Eref[k])
+            alive = len(srt) > 0 and ids1[pos[k]] == ids[j]
+            if alive != (not collected):
+                mism += 1
+                assert abs(r_new[2]) < 1e-3                                  # only at the collection plane
+            elif alive:
+                worst = max(worst, float(np.abs(xyz1[pos[k]].astype(np.float64) - r_new).max()))
+    return worst, worst_field, mism
+
+
+@pytest.mark.parametrize("cfg,m", [(3, 512), (4, 256)])
+def test_snapshot_restart_at_steps_0_10_100_500_full_size(cfg, m):
+    """at full size the oracle checks the field on sampled targets and ONE step of sampled
+    carriers from the GPU's own snapshot, in windows of 10 consecutive steps starting at steps 0, 10, 100 and 500 —
+    the last two on a track that has lost its front end (population decayed, state compacted many times).
+    Between windows config 3 advances with the exact path; config 4 (0.38 s per exact step at 1M holes) advances with
+    the far-field variant, which is only a way to reach a realistic late state quickly: every checked step is an exact
+    all-pairs step."""
+    w = workloads.make(cfg)
+    n0 = len(w["xyz"])
+    rng = np.random.default_rng(100 + cfg)
+    sim = gpu_sim(w)
+    sim.load_carriers(w["xyz"])
+    n_start = sim.state()["n_active"]
+    report = []
+    for start in (0, 10, 100, 500):
+        st = sim.state()
+        if st["step"] < start:
+            if cfg == 4 and start - st["step"] > 20:
+                sim.set_farfield(0.5)
+                sim.step(start - st["step"])
+                sim.set_farfield(-1.0)                                        # back to the exact O(N^2) path
+            else:
+                sim.step(start - st["step"])
+        st = sim.state()
+        assert st["step"] == start
+        worst, worst_field, mism = _restart_window(sim, w, rng, m, 10)
+        assert worst <= 2e-4, (start, worst)          # one step: FP32 field error x drift + one FP32 rounding of the position
+        assert worst_field <= 1e-4, (start, worst_field)
+        assert mism <= 2
+        st2 = sim.state()
+        img, over = sim.read_image()
+        assert int(img.sum()) + over + st2["n_active"] == n0
+        xyz, ids = sim.read_carriers()
+        if cfg == 3:
+            assert np.all(np.diff(ids.astype(np.int64)) > 0)                 # stable load order (the treecode keeps curve order)
+        assert np.all(xyz[:, 2] > 0) and np.all(xyz[:, 2] <= 675.0)
+        report.append((start, st["n_active"], worst, worst_field))
+    assert report[-1][1] < 0.75 * n_start                                    # the track really lost its front end by step 500
+    print("cfg%d restart windows (step, n_active, worst |dr| um, worst field err): %s" % (cfg, report))
+    sim.close()

@@ -389,3 +389,112 @@ def test_coulomb_off_multi_step_launch_is_bit_identical_to_single_steps():
     assert np.abs(o.image().astype(np.int64) - multi.read_image()[0].astype(np.int64)).sum() <= 4
     multi.close()
     single.close()
+
+
+# ------------------------------------------------------------------ failure detection: non-finite state
+@pytest.mark.parametrize("flags", [0, 1])                                     # all-pairs path and the Coulomb-off multi-step path
+def test_non_finite_state_is_reported_by_run_to_collection_and_get_state(flags):
+    from paper_2203_11043_b200 import binding as b
+    w = workloads.make(0, n=700)
+    sim = gpu_sim(w, flags=flags, dt_ns=1e300)                                # one drift step of 1e295 x mu E overflows FP32
+    sim.load_carriers(w["xyz"])
+    with pytest.raises(b.GcoreccdError) as e:
+        sim.run_to_collection(100)
+    assert e.value.code == b.ERR_NONFINITE
+    with pytest.raises(b.GcoreccdError) as e:                                 # sticky: get_state keeps reporting it
+        sim.state()
+    assert e.value.code == b.ERR_NONFINITE
+    sim.reset()                                                               # a reset clears it
+    assert sim.state()["n_active"] == 0
+    sim.close()
+
+
+def test_non_finite_state_is_reported_by_run_events():
+    from paper_2203_11043_b200 import binding as b
+    w = workloads.make_events([26, 300, 2048])
+    sim = gpu_sim(w, max_carriers=len(w["xyz"]), dt_ns=1e300)
+    sim.load_events(w["xyz"], w["offsets"])
+    with pytest.raises(b.GcoreccdError) as e:
+        sim.run_events(100)
+    assert e.value.code == b.ERR_NONFINITE
+    sim.close()
+
+
+def test_snapshot_is_validated_and_keeps_the_count_invariant():
+    from paper_2203_11043_b200 import binding as b
+    w = workloads.make(0, n=64)
+    sim = gpu_sim(w, max_carriers=128)
+    ids = np.arange(100, 164, dtype=np.uint32)
+    bad = w["xyz"].copy(); bad[3, 0] = np.nan
+    with pytest.raises(b.GcoreccdError) as e:
+        sim.load_snapshot(bad, ids, 5)
+    assert e.value.code == b.ERR_INVALID
+    bad = w["xyz"].copy(); bad[3, 2] = 676.0
+    with pytest.raises(b.GcoreccdError):
+        sim.load_snapshot(bad, ids, 5)
+    bad = w["xyz"].copy(); bad[3, 2] = 0.0                                    # an ACTIVE carrier cannot sit at the plane
+    with pytest.raises(b.GcoreccdError):
+        sim.load_snapshot(bad, ids, 5)
+    sim.load_snapshot(w["xyz"], ids, 5)
+    st = sim.state()
+    assert st["n_loaded"] == 164 and st["n_active"] == 64 and st["step"] == 5  # device copy of n_loaded follows the host's
+    sim.close()
+
+
+# ------------------------------------------------------------------ many steps per launch (gc_persist.cuh)
+@pytest.mark.parametrize("cfg,n", [(0, 1024), (0, 37), (1, 4096), (1, 16384), (3, 20000), (0, 1), (0, 65), (2, 24576)])
+def test_persistent_multi_step_kernel_equals_the_two_launch_path(cfg, n):
+    """Small populations run K steps in one cooperative launch (field -> grid barrier -> a2..a8 -> grid barrier).  Same
+    physics and Philox counters as the two-launch path; only the FP32/FP64 summation order of the chunk partials of
+    eq. 6 differs, so after 12 steps positions agree far inside the trajectory tolerance and every integer agrees
+    except for retire decisions at the plane."""
+    w = workloads.make(cfg, n=n)
+    a, b = gpu_sim(w), gpu_sim(w)
+    b.set_persistent(False)
+    a.load_carriers(w["xyz"]); b.load_carriers(w["xyz"])
+    la = a.kernel_launches()
+    a.step(12); b.step(12)
+    sa, sb = a.state(), b.state()
+    assert a.kernel_launches() - la <= 2                                       # ONE launch for the 12 steps (+ a re-plan)
+    assert sa["step"] == sb["step"] == 12 and abs(sa["n_active"] - sb["n_active"]) <= 2
+    (xa, ia), (xb, ib) = a.read_carriers(), b.read_carriers()
+    assert np.all(np.diff(ia.astype(np.int64)) > 0)                            # stable in-place compaction
+    common = np.intersect1d(ia, ib)
+    d = np.abs(xa[np.isin(ia, common)].astype(np.float64) - xb[np.isin(ib, common)]).max(axis=1)
+    assert len(common) >= len(ia) - 2 and np.quantile(d, 0.98) <= 2e-4 and (d > 1e-3).mean() <= 0.02, d.max()
+    ima, ova = a.read_image(); imb, ovb = b.read_image()
+    assert int(ima.sum()) + ova + sa["n_active"] == len(w["xyz"]) == int(imb.sum()) + ovb + sb["n_active"]
+    assert abs(sa["pair_interactions"] - sb["pair_interactions"]) <= 1e-3 * max(1, sb["pair_interactions"])
+    a.close(); b.close()
+
+
+def test_persistent_kernel_is_bit_reproducible_and_independent_of_the_batching():
+    w = workloads.make(3, n=12000)                                             # a track: holes retire every step
+    runs = []
+    for chunks in ((40,), (1, 7, 32), (13, 27)):
+        s = gpu_sim(w)
+        s.load_carriers(w["xyz"])
+        for c in chunks:
+            s.step(c)
+        runs.append((s.read_carriers(), s.state(), s.read_image()[0]))
+        s.close()
+    for (x, i), st, img in runs[1:]:
+        assert np.array_equal(i, runs[0][0][1]) and np.array_equal(x, runs[0][0][0])
+        assert st == runs[0][1] and np.array_equal(img, runs[0][2])
+    assert runs[0][1]["n_active"] < 12000 and runs[0][1]["step"] == 40
+
+
+def test_persistent_kernel_runs_an_event_to_collection_and_stops_at_zero():
+    w = workloads.make(0, n=2000)
+    s = gpu_sim(w)
+    s.load_carriers(w["xyz"])
+    s.step(100000)                                                             # one launch; the loop ends when nobody drifts
+    st = s.state()
+    img, over = s.read_image()
+    assert st["n_active"] == 0 and int(img.sum()) + over == 2000 and 100 < st["step"] < 200
+    o = oracle_sim(w, flags=g.FP32_STATE)
+    o.load(w["xyz"])
+    o.run(100000)
+    assert abs(st["step"] - o.state()["step"]) <= 3
+    assert st["pair_interactions"] == pytest.approx(o.state()["pair_interactions"], rel=0.02)
+    s.close()

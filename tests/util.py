@@ -1,4 +1,6 @@
 """Helpers shared by the GPU parity tests: the same workload handed to the oracle and to the CUDA path."""
+import os
+
 import numpy as np
 
 from oracle import goracle as g
@@ -50,25 +52,39 @@ def image_moments(img, x0, y0, pitch):
     return mx, my, vx, vy
 
 
-def traj_assert(xyz, ids, oxyz, oids, history, n_total, tol):
+R_ENC = 0.1          # um: DESIGN.md R21 excuse radius (an ORACLE-side encounter closer than this inside the window)
+EXCUSED = []         # (label, n_carriers, n_suspects) of every trajectory check of the session; printed by conftest
+
+
+def closest_encounters(history, suspects):
+    """Smallest distance to any other drifting hole that each suspect id saw at the start of a step of the oracle's
+    window.  history = [(xyz, ids) before each step]."""
+    closest = {int(i): np.inf for i in suspects}
+    for hx, hid in history:
+        for i in closest:
+            k = np.searchsorted(hid, i)
+            if k < len(hid) and hid[k] == i:
+                r = np.linalg.norm(hx - hx[k], axis=1)
+                r[k] = np.inf
+                closest[i] = min(closest[i], float(r.min()))
+    return closest
+
+
+def traj_assert(xyz, ids, oxyz, oids, history, n_total, tol, r_enc=R_ENC, max_frac=0.02, label=""):
     """GPU (xyz, ids) vs FP32-state oracle (oxyz, oids) after some steps; `history` = the oracle's (xyz, ids) before
-    each of those steps.  DESIGN.md R21: a carrier may exceed `tol` only if the ORACLE's trajectory shows a neighbour
-    closer than 0.1 um inside the window, and at most 2 % may do so.  Returns the per-carrier max-coordinate error."""
+    each of those steps.  DESIGN.md R21: a carrier may exceed `tol` (or differ in its retire flag) only if the ORACLE's
+    trajectory shows a neighbour closer than r_enc = 0.1 um inside the window, and at most max_frac = 2 % (+2) may do
+    so.  The number of excused carriers is recorded (EXCUSED) and bounded here, so the clause cannot silently absorb a
+    regression.  Returns the per-carrier max-coordinate error."""
     common = np.intersect1d(ids, oids)
     xyz_c, oxyz_c = xyz[np.isin(ids, common)], oxyz[np.isin(oids, common)]
-    d = np.abs(xyz_c.astype(np.float64) - oxyz_c).max(axis=1)
-    suspects = set(common[d > tol].tolist()) | set(np.setxor1d(ids, oids).tolist())   # incl. retire-flag mismatches
-    if suspects:
-        assert len(suspects) <= 0.02 * n_total + 2, len(suspects)
-        closest = {i: np.inf for i in suspects}
-        for hx, hid in history:
-            for i in suspects:
-                k = np.searchsorted(hid, i)
-                if k < len(hid) and hid[k] == i:
-                    r = np.linalg.norm(hx - hx[k], axis=1)
-                    r[k] = np.inf
-                    closest[i] = min(closest[i], r.min())
-        # retire-flag mismatches must sit at the collection plane, or come from a close encounter like the rest
-        for i, r in closest.items():
-            assert r < 0.1, (i, r, "exceeds %g um without a close encounter" % tol)
+    d = np.abs(xyz_c.astype(np.float64) - oxyz_c).max(axis=1) if len(common) else np.zeros(0)
+    suspects = sorted(set(common[d > tol].tolist()) | set(np.setxor1d(ids, oids).tolist()))   # incl. retire-flag mismatches
+    closest = closest_encounters(history, suspects) if suspects else {}
+    EXCUSED.append((label, int(n_total), len(suspects), sorted(round(r, 4) for r in closest.values())))
+    if os.environ.get("GCORECCD_TRAJ_DIAG"):                 # survey mode: record every suspect, assert nothing
+        return d
+    assert len(suspects) <= max_frac * n_total + 2, (label, len(suspects), n_total)
+    bad = {i: r for i, r in closest.items() if not r < r_enc}
+    assert not bad, (label, bad, "exceeds %g um without an oracle-side encounter inside %g um" % (tol, r_enc))
     return d
