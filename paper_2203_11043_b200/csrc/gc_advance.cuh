@@ -16,6 +16,13 @@
 
 namespace gc {
 
+#ifdef GC_TIMING
+__device__ long long g_pp[1024][16];              // per CTA: clock64 at probe points of the last step (development builds)
+#define GC_P(slot) do { if (threadIdx.x == 0) g_pp[blockIdx.x & 1023][slot] = clock64(); } while (0)
+#else
+#define GC_P(slot) do { } while (0)
+#endif
+
 // status word of a tile: [63:34] stamp of the step | [33:32] kind (1 = count of this tile, 2 = inclusive prefix) | [31:0] value
 __device__ __forceinline__ unsigned long long scan_pack(uint32_t stamp, uint32_t kind, uint32_t v) {
   return ((unsigned long long)stamp << 34) | ((unsigned long long)kind << 32) | (unsigned long long)v;
@@ -45,8 +52,13 @@ __device__ __forceinline__ unsigned long long ld_relaxed_u64(const unsigned long
   asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
   return v;
 }
+// Publishing a word other CTAs spin on: an atomic exchange executes AT the L2, so the word is visible one trip later.
+// A plain (even st.relaxed.gpu) store may sit in the SM's write path: measured 2x longer look-backs than with
+// st.release, whose fence drains it at the price of a MEMBAR.
 __device__ __forceinline__ void st_relaxed_u64(unsigned long long* p, unsigned long long v) {
-  asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+  unsigned long long old;
+  asm volatile("atom.relaxed.gpu.global.exch.b64 %0, [%1], %2;" : "=l"(old) : "l"(p), "l"(v) : "memory");
+  (void)old;
 }
 __device__ __forceinline__ uint32_t scan_stamp(uint32_t seq) { return (seq % 0x3ffffffeu) + 1u; }   // 30 bits, never 0
 
@@ -88,10 +100,34 @@ __device__ __forceinline__ uint32_t scan_lookback(unsigned long long* status, ui
   return excl;
 }
 
+// Two-level scan for a grid whose tiles all run at the same time (the persistent kernel: <= 592 tiles, one per resident
+// CTA).  When every tile publishes at once, the look-back above resolves in t / 32 DEPENDENT rounds (only tile 0 knows
+// its inclusive prefix at first): measured 7,400 cycles at 256 tiles.  Here tile t = 32 g + r sums the counts of the r
+// tiles before it in its group (one round), the last tile of each group publishes the group's total, and every tile adds
+// the totals of the g groups before its own (second round): two rounds at any tile count.  Group totals live behind
+// the tile words (status[kScanGroupBase + g]).  Executed by one full warp.
+constexpr uint32_t kScanGroupBase = 768;                    // tiles < 768; scan_entries >= 1,024 (gcoreccd.cu make_layout)
+__device__ __forceinline__ uint32_t scan_two_level(unsigned long long* status, uint32_t t, uint32_t stamp, uint32_t count) {
+  const uint32_t lane = threadIdx.x & 31u;
+  const uint32_t g = t >> 5, r = t & 31u;
+  if (lane == 0) st_relaxed_u64(status + t, scan_pack(stamp, 1u, count));
+  // both rounds' loads are issued at once; each lane then spins on its own word until it carries this step's stamp
+  const unsigned long long* pa = status + (g << 5) + lane;
+  const unsigned long long* pg = status + kScanGroupBase + lane;
+  unsigned long long a = lane < r ? ld_relaxed_u64(pa) : scan_pack(stamp, 1u, 0u);
+  unsigned long long b = lane < g ? ld_relaxed_u64(pg) : scan_pack(stamp, 1u, 0u);
+  while ((uint32_t)(a >> 34) != stamp) a = ld_relaxed_u64(pa);
+  const uint32_t in_group = __reduce_add_sync(0xffffffffu, (uint32_t)a);
+  if (r == 31u && lane == 0) st_relaxed_u64(status + kScanGroupBase + g, scan_pack(stamp, 1u, in_group + count));
+  while ((uint32_t)(b >> 34) != stamp) b = ld_relaxed_u64(pg);
+  return in_group + __reduce_add_sync(0xffffffffu, (uint32_t)b);
+}
+
 // a7..a8 for tile t = carriers [t TQ, t TQ + TQ) of the state, by the first TQ threads of the CTA (TQ <= 256, a multiple of 32;
 // ALL threads of the CTA must call): (xf, yf, zf) = this thread's updated carrier, `mine` = it has one, `finite` = the
 // update produced finite numbers.  Collection + histogram, survivor ranks, look-back, compacted write into A — the
-// buffer the carriers were read from if INPLACE, another one otherwise.  Returns whether t is the last tile; thread 0 of
+// buffer the carriers were read from if INPLACE (k_advance: any number of tiles, ticket order), another one otherwise
+// (the persistent kernel: all tiles resident).  Returns whether t is the last tile; thread 0 of
 // that CTA then holds the new n_active in n_new_out.
 template <bool INPLACE>
 __device__ __forceinline__ bool commit_tile(const uint32_t TQ, SoA A, uint32_t t, uint32_t n, uint64_t step, uint32_t stamp, bool mine, bool finite,
@@ -106,8 +142,10 @@ __device__ __forceinline__ bool commit_tile(const uint32_t TQ, SoA A, uint32_t t
     else keep = true;
   }
   // s_w: [0, TQ/32) survivors per warp, [8] exclusive prefix of the tile, [9] collected, [10] out of window
+  GC_P(4);
   if (tid < 16) s_w[tid] = 0;
   __syncthreads();
+  GC_P(5);
   uint32_t rank_in_warp = 0;
   if (tid < TQ) {                                            // whole warps: TQ is a multiple of 32
     const uint32_t bal = __ballot_sync(0xffffffffu, keep);
@@ -120,11 +158,12 @@ __device__ __forceinline__ bool commit_tile(const uint32_t TQ, SoA A, uint32_t t
     }
   }
   __syncthreads();
+  GC_P(6);
   if (warp == 0) {
     uint32_t count = 0;
 #pragma unroll
     for (int w = 0; w < 8; ++w) count += s_w[w];             // warps beyond TQ / 32 hold 0
-    const uint32_t excl = scan_lookback<INPLACE>(status, t, stamp, count);
+    const uint32_t excl = INPLACE ? scan_lookback<true>(status, t, stamp, count) : scan_two_level(status, t, stamp, count);
     if (lane == 0) {
       s_w[8] = excl;
       if (s_w[9]) atomicAdd((unsigned long long*)&ctrl->n_collected, (unsigned long long)s_w[9]);
@@ -133,6 +172,7 @@ __device__ __forceinline__ bool commit_tile(const uint32_t TQ, SoA A, uint32_t t
     }
   }
   __syncthreads();
+  GC_P(7);
   if (keep) {
     uint32_t off = s_w[8] + rank_in_warp;
     for (uint32_t w = 0; w < warp; ++w) off += s_w[w];

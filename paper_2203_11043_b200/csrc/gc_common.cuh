@@ -51,8 +51,7 @@ struct Ctrl {                 // lives in device memory; only kernels write it (
   // second 128-byte line: polled by the persistent kernel's grid barrier, kept away from the line everybody reads
   uint32_t bar;               // arrivals since the launch began; 0 between launches
   uint32_t bar_exit;          // CTAs that left the persistent kernel; 0 between launches
-  uint32_t bar_gen;           // grid barriers executed since the last reset (the value the per-CTA flags hold)
-  uint32_t pad3_[29];
+  uint32_t pad3_[30];
 };
 static_assert(sizeof(Ctrl) == 256, "Ctrl is two 128-byte lines");
 

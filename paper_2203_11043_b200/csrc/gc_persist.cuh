@@ -18,35 +18,18 @@
 namespace gc {
 
 // Grid barrier of a cooperative grid, split into ARRIVE and WAIT so that work which does not depend on the other CTAs
-// fills the gap.  Arrivals are counted in ONE word (atom.acq_rel: releases this CTA's writes — they precede the
-// __syncthreads — and lets the last arriver acquire everybody's); the last arriver then raises one flag PER CTA, 128
-// bytes apart, and each CTA polls only its own flag.  With everybody polling the arrival word itself, the polls of
-// the early CTAs queue in front of the late arrivals at one L2 slice: measured 19 cycles per CTA per barrier (296 CTAs:
-// 5,600 cycles).  `gen` = value the flags take at this barrier (increases by one per barrier, never reused between
-// resets); `target` = arrivals expected since the launch began.  Data that crosses the barrier is read with L2-coherent
-// loads (ld.global.cg) only.
-constexpr uint32_t kFlagStride = 32;                        // uint32 per flag: one 128-byte line each
-__device__ __forceinline__ void grid_arrive(uint32_t* bar, uint32_t* flags, uint32_t target, uint32_t gen) {
+// fills the gap.  `target` = arrivals expected since the launch began (barriers so far x gridDim.x).  One release
+// reduction per CTA to arrive (it orders the whole CTA's writes: they precede the __syncthreads), relaxed polling of the
+// same word, one fence after the wait; data that crosses the barrier is read with L2-coherent loads (ld.global.cg) only.
+// (Tried: one flag line per CTA raised by the last arriver, so that nobody polls the arrival word — slower at every
+// size: 10.1 -> 10.6 us per step at 1,024 holes, 18.6 -> 20.2 at 4,096; the second hop costs more than the polls.)
+__device__ __forceinline__ void grid_arrive(uint32_t* bar) {
   __syncthreads();
-  if (threadIdx.x < 32) {
-    uint32_t last = 0;
-    if (threadIdx.x == 0) {
-      uint32_t old;
-      asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], 1;" : "=r"(old) : "l"(bar) : "memory");
-      last = (old + 1u == target) ? 1u : 0u;
-    }
-    last = __shfl_sync(0xffffffffu, last, 0);
-    if (last) {
-      asm volatile("fence.acq_rel.gpu;" ::: "memory");
-      for (uint32_t c = threadIdx.x; c < gridDim.x; c += 32)
-        asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(flags + (size_t)c * kFlagStride), "r"(gen) : "memory");
-    }
-  }
+  if (threadIdx.x == 0) asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(bar) : "memory");
 }
-__device__ __forceinline__ void grid_wait(const uint32_t* flags, uint32_t gen) {
+__device__ __forceinline__ void grid_wait(const uint32_t* bar, uint32_t target) {
   if (threadIdx.x == 0) {
-    const uint32_t* f = flags + (size_t)blockIdx.x * kFlagStride;
-    while ((int32_t)(ld_relaxed_u32(f) - gen) < 0) { }
+    while (ld_relaxed_u32(bar) < target) { }
     asm volatile("fence.acq_rel.gpu;" ::: "memory");
   }
   __syncthreads();
@@ -96,13 +79,14 @@ struct Tile {
   __device__ __forceinline__ bool post(SoA dst, uint32_t t, uint32_t n, uint64_t step, uint32_t stamp, const FieldPlan& plan,
                                        const float* Ep, uint32_t part_cap, Ctrl* ctrl, Sink sink, unsigned long long* status,
                                        const DevParams& P, PersistShared& sh, uint32_t& n_new) {
+    GC_P(0);
     {
       double ex = 0.0, ey = 0.0, ez = 0.0;
       if (have && !(P.flags & 1u)) {
         const uint32_t per = (plan.S + R - 1) / R;
         const uint32_t s0 = min(q * per, plan.S), s1 = min(s0 + per, plan.S);
         const float* e = Ep + i;
-        for (uint32_t s = s0; s < s1; s += 4) {
+        for (uint32_t s = s0; s < s1; s += 4) {              // 12 loads in flight per round trip; 24 measured slower (3,100 -> 5,900 cycles)
           float vx[4], vy[4], vz[4];
 #pragma unroll
           for (int u = 0; u < 4; ++u) {
@@ -117,7 +101,9 @@ struct Tile {
       }
       sh.e[0][q * TQ + c] = ex; sh.e[1][q * TQ + c] = ey; sh.e[2][q * TQ + c] = ez;
     }
+    GC_P(1);
     __syncthreads();                                         // partial ranges and Box-Muller chains are in shared memory
+    GC_P(2);
     float xf = 0.f, yf = 0.f, zf = 0.f;
     bool finite = true;
     const bool mine = have && q == 0;
@@ -133,12 +119,20 @@ struct Tile {
       if (!(P.flags & 2u)) { nrm[0] = sh.bm[0][c] * sh.bm[2][c]; nrm[1] = sh.bm[0][c] * sh.bm[1][c]; nrm[2] = sh.bm[3][c] * sh.bm[4][c]; }
       finite = advance_with_normals(x, y, z, E[0], E[1], E[2], nrm, P, xf, yf, zf);
     }
+    GC_P(3);
     return commit_tile<false>(TQ, dst, t, n, step, stamp, mine, finite, xf, yf, zf, id, ctrl, sink, status, P, sh.w, n_new);
   }
 };
 
 #ifdef GC_TIMING
 __device__ long long g_dbg[2][64][16];
+__device__ unsigned long long g_gt[1024][8];      // per CTA: globaltimer (ns) at the phase boundaries of step 8
+__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
+#define GC_G(slot) do { if (tid == 0 && k == 8) g_gt[blockIdx.x][slot] = gtime(); } while (0)
+#else
+#define GC_G(slot) do { } while (0)
+#endif
+#ifdef GC_TIMING
 #define GC_T(slot) do { if (tid == 0 && k < 64 && (blockIdx.x == 0 || blockIdx.x == gridDim.x - 1)) g_dbg[blockIdx.x ? 1 : 0][k][slot] = clock64(); } while (0)
 #else
 #define GC_T(slot) do { } while (0)
@@ -146,8 +140,8 @@ __device__ long long g_dbg[2][64][16];
 
 template <int NPACK, int MINB>
 __global__ void __launch_bounds__(kTPB, MINB)
-k_steps(SoA A, SoA B, Ctrl* ctrl, float* Ep, uint32_t part_cap, Sink sink, unsigned long long* status, uint32_t* flags,
-        DevParams P, PlanArgs pa, uint32_t n_steps) {
+k_steps(SoA A, SoA B, Ctrl* ctrl, float* Ep, uint32_t part_cap, Sink sink, unsigned long long* status, DevParams P, PlanArgs pa,
+        uint32_t n_steps) {
   __shared__ float4 s_xy[2][kTPB];
   __shared__ float2 s_z[2][kTPB];
   __shared__ PersistShared sh;
@@ -155,8 +149,7 @@ k_steps(SoA A, SoA B, Ctrl* ctrl, float* Ep, uint32_t part_cap, Sink sink, unsig
   __shared__ unsigned long long s_step;
   const uint32_t tid = threadIdx.x;
   const uint32_t seq0 = ld_acquire_u32(&ctrl->scan_seq);
-  const uint32_t gen0 = ld_acquire_u32(&ctrl->bar_gen);      // written by the previous launch's last CTA
-  uint32_t arrivals = 0, gen = gen0;
+  uint32_t arrivals = 0;
   uint32_t k = 0;
   // the state ping-pongs between A and B (step k reads one, writes the compacted survivors to the other): no slot is
   // ever overwritten while another CTA may still read it, so the look-back needs no release/acquire ordering
@@ -184,18 +177,18 @@ k_steps(SoA A, SoA B, Ctrl* ctrl, float* Ep, uint32_t part_cap, Sink sink, unsig
     const uint32_t t = blockIdx.x;
     const bool owner = t < (n + (uint32_t)tq - 1u) / (uint32_t)tq;     // the host keeps n <= 256 G (persist_max)
 
-    GC_T(0);
+    GC_T(0); GC_G(0);
     field_items<NPACK, kTPB, 4>(cur.x, cur.y, cur.z, plan, Ep, part_cap, P.eps2, s_xy, s_z);
-    GC_T(1);
-    arrivals += G; gen += 1;
-    grid_arrive(&ctrl->bar, flags, arrivals, gen);
+    GC_T(1); GC_G(1);
+    arrivals += G;
+    grid_arrive(&ctrl->bar);
     GC_T(2);
 
     Tile tile;
     if (owner) tile.pre((uint32_t)tq, cur, t, n, step, P, sh);
-    GC_T(3);
-    grid_wait(flags, gen);
-    GC_T(4);
+    GC_T(3); GC_G(2);
+    grid_wait(&ctrl->bar, arrivals);
+    GC_T(4); GC_G(3);
     if (owner) {
       uint32_t n_new = 0;
       const bool last = tile.post(nxt, t, n, step, stamp, plan, Ep, part_cap, ctrl, sink, status, P, sh, n_new);
@@ -211,12 +204,12 @@ k_steps(SoA A, SoA B, Ctrl* ctrl, float* Ep, uint32_t part_cap, Sink sink, unsig
         }
       }
     }
-    GC_T(5);
-    arrivals += G; gen += 1;
-    grid_arrive(&ctrl->bar, flags, arrivals, gen);
+    GC_T(5); GC_G(4);
+    arrivals += G;
+    grid_arrive(&ctrl->bar);
     GC_T(6);
-    grid_wait(flags, gen);
-    GC_T(7);
+    grid_wait(&ctrl->bar, arrivals);
+    GC_T(7); GC_G(5);
   }
   // an odd number of steps leaves the state in B: bring it home (every CTA is past the last barrier; B is complete)
   if (k & 1u) {
@@ -234,7 +227,6 @@ k_steps(SoA A, SoA B, Ctrl* ctrl, float* Ep, uint32_t part_cap, Sink sink, unsig
     if (out == gridDim.x - 1) {
       ctrl->bar = 0;
       ctrl->bar_exit = 0;
-      ctrl->bar_gen = gen;
       ctrl->scan_seq = seq0 + k;
     }
   }

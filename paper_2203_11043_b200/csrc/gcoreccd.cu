@@ -27,7 +27,6 @@ using namespace gc;
 namespace {
 
 constexpr uint64_t kMaxCarriers = GCORECCD_MAX_CARRIERS;
-constexpr uint64_t kBarFlags = 1024;                       // >= the largest cooperative grid (4 CTAs x 148 SMs)
 constexpr uint64_t kPersistMaxDefault = 24576;          // populations up to this run many steps per launch (gc_persist.cuh)
 constexpr uint64_t kPersistMaxLimit = 37888;            // 148 CTAs x 256: beyond, the one-step kernels are as fast
 constexpr int kNumVariants = 6;                       // 0-2: one-step field kernels (2/4/8 targets per thread); 3-4: persistent
@@ -36,7 +35,7 @@ constexpr int kGraphSteps = 8;                        // steps per CUDA-graph la
 
 struct Layout {
   uint64_t cap_pad, part_cap, n_tiles, scan_entries, tree_scratch;
-  uint64_t off_ctrl, off_A, off_B, off_Ep, off_tiles, off_scan, off_flags, off_image, off_fin, total;
+  uint64_t off_ctrl, off_A, off_B, off_Ep, off_tiles, off_scan, off_image, off_fin, total;
 };
 
 inline uint64_t align_up(uint64_t v, uint64_t a) { return (v + a - 1) / a * a; }
@@ -46,8 +45,8 @@ Layout make_layout(uint64_t max_carriers, int32_t nx, int32_t ny) {
   L.cap_pad = align_up(max_carriers, 1024);
   // Partial planes: S chunks x stride (= n_active rounded to 256) entries each.  A large population is balanced over
   // the SMs with few chunks (64+ row blocks x 16 chunks = 7+ rounds of 148 CTAs, <= 1.5 % idle), a small one needs many
-  // (8 row blocks at 4,096 holes): 16 chunks at capacity, and never fewer entries than 64 chunks of 32,768 holes.
-  L.part_cap = std::max<uint64_t>((uint64_t)kPartFactor * L.cap_pad, 64ull * std::min<uint64_t>(L.cap_pad, 32768));
+  // (4 row blocks at 4,096 holes over 296 CTAs): 16 chunks at capacity, and never fewer entries than 128 chunks of 16,384 holes.
+  L.part_cap = std::max<uint64_t>((uint64_t)kPartFactor * L.cap_pad, 128ull * std::min<uint64_t>(L.cap_pad, 16384));
   L.tree_scratch = 8 * L.cap_pad + 4096;                  // far-field variant: tail of plane x (see gcoreccd_create)
   L.n_tiles = L.cap_pad / kTPB;
   L.scan_entries = std::max<uint64_t>(L.n_tiles, 1024);   // look-back status words: 256-carrier tiles, or 64-carrier tiles of <= 65,536 holes
@@ -58,7 +57,6 @@ Layout make_layout(uint64_t max_carriers, int32_t nx, int32_t ny) {
   L.off_Ep = o;    o += align_up(3 * L.part_cap * 4, 256);
   L.off_tiles = o; o += align_up(L.n_tiles * 4, 256);
   L.off_scan = o;  o += align_up(L.scan_entries * 8, 256);
-  L.off_flags = o; o += kBarFlags * 128;                  // one 128-byte line per CTA of the persistent kernel's grid barrier
   L.off_image = o; o += align_up((uint64_t)nx * (uint64_t)ny * 4, 256);
   L.off_fin = o;   o += align_up(L.cap_pad * 16, 256);
   L.total = o;
@@ -103,7 +101,6 @@ struct gcoreccd {
   float* Ep;
   uint32_t* tile_count;
   unsigned long long* scan;     // look-back status words (gc_advance.cuh)
-  uint32_t* bar_flags;          // per-CTA flags of the persistent kernel's grid barrier (gc_persist.cuh)
   uint32_t* image;
   float4* fin;                  // per-id collection records
   Sink sink;
@@ -286,8 +283,8 @@ void enqueue_step(gcoreccd_t* h, uint32_t tiles) {
 int launch_persistent(gcoreccd_t* h, uint32_t n_steps) {
   const int v = h->variant;
   SoA A = h->A; SoA B = h->B; Ctrl* ctrl = h->ctrl; float* Ep = h->Ep; uint32_t pc = (uint32_t)h->L.part_cap; Sink sink = h->sink;
-  unsigned long long* scan = h->scan; uint32_t* flags = h->bar_flags; DevParams dp = h->dp; PlanArgs pa = plan_args(h, v);
-  void* args[] = {&A, &B, &ctrl, &Ep, &pc, &sink, &scan, &flags, &dp, &pa, &n_steps};
+  unsigned long long* scan = h->scan; DevParams dp = h->dp; PlanArgs pa = plan_args(h, v);
+  void* args[] = {&A, &B, &ctrl, &Ep, &pc, &sink, &scan, &dp, &pa, &n_steps};
   const void* fn = v == 4 ? (const void*)k_steps<4, 1> : v == 3 ? (const void*)k_steps<2, 2> : (const void*)k_steps<1, 2>;
   GC_CUDA(h, cudaLaunchCooperativeKernel(fn, dim3((unsigned)h->grid_field[v]), dim3(kTPB), args, 0, h->stream));
   h->launches += 1;
@@ -515,7 +512,6 @@ int gcoreccd_create(const gcoreccd_params* p, gcoreccd_t** out) {
   h->Ep = (float*)(h->ws + h->L.off_Ep);
   h->tile_count = (uint32_t*)(h->ws + h->L.off_tiles);
   h->scan = (unsigned long long*)(h->ws + h->L.off_scan);
-  h->bar_flags = (uint32_t*)(h->ws + h->L.off_flags);
   h->image = (uint32_t*)(h->ws + h->L.off_image);
   h->fin = (float4*)(h->ws + h->L.off_fin);
   h->sink = Sink{h->image, h->fin, (uint32_t)std::min<uint64_t>(p->max_carriers, 0xffffffffull)};
@@ -603,7 +599,6 @@ int gcoreccd_reset(gcoreccd_t* h) {
   DeviceGuard guard(h->device);
   GC_CUDA(h, cudaMemsetAsync(h->ctrl, 0, sizeof(Ctrl), h->stream));
   GC_CUDA(h, cudaMemsetAsync(h->scan, 0, (size_t)h->L.scan_entries * 8, h->stream));   // scan_seq restarts: no stale stamps
-  GC_CUDA(h, cudaMemsetAsync(h->bar_flags, 0, kBarFlags * 128, h->stream));            // bar_gen restarts likewise
   GC_CUDA(h, cudaMemsetAsync(h->image, 0, (size_t)h->p.img_nx * h->p.img_ny * 4, h->stream));
   GC_CUDA(h, cudaMemsetAsync(h->fin, 0xff, (size_t)h->L.cap_pad * 16, h->stream));     // NaN / all-ones = still drifting
   if (h->ff_on) GC_CUDA(h, cudaMemsetAsync(h->tree.tc, 0, sizeof(TreeCtrl), h->stream)); // far-field counters restart too
@@ -1379,6 +1374,12 @@ int gcoreccd_save_collected_file(gcoreccd_t* h, const char* path, uint64_t* n_wr
 #ifdef GC_TIMING
 int gcoreccd_debug_timing(long long* out) {      // development builds only (-DGC_TIMING): phase timestamps of k_steps
   return cudaMemcpyFromSymbol(out, gc::g_dbg, sizeof(gc::g_dbg)) == cudaSuccess ? 0 : -5;
+}
+int gcoreccd_debug_probes(long long* out) {
+  return cudaMemcpyFromSymbol(out, gc::g_pp, sizeof(gc::g_pp)) == cudaSuccess ? 0 : -5;
+}
+int gcoreccd_debug_gtimes(unsigned long long* out) {
+  return cudaMemcpyFromSymbol(out, gc::g_gt, sizeof(gc::g_gt)) == cudaSuccess ? 0 : -5;
 }
 #endif
 
