@@ -13,8 +13,13 @@ over the 131,072-hole cloud of BASELINE.json:configs[2].  Prints ONE JSON line (
   roofline   field kernel: 20 FLOP x pairs / CUDA-event duration of that kernel, against the FP32 non-tensor
              peak 148 SM x 128 lanes x 2 x sm_max_mhz
   cpu_baseline  the FP64 oracle, as it stands, on this box's host cores on a bounded sample of the same workload
+  per_config    configs 0-4 of BASELINE.json: per-step rate at step 0 and seconds per event (load -> full collection)
+  n_sweep       per-step time against N = 2^10 .. 2^20 at the cfg-2 geometry, Coulomb on and off (Fig. 4)
+  sharded_virtual  cfg3 sharded over 8 virtual ranks on this GPU (each rank's kernels timed alone)
 N > 1: replicas only (BASELINE.json north_star: one GPU per event, no sharding): every rank runs its own
-event; value = all ranks' pairs / max-over-ranks device time.
+event; value = all ranks' pairs / max-over-ranks device time.  `python bench.py --gpus N` without torchrun spawns the
+N ranks itself (one per device) and fails loudly if the box has fewer than N GPUs.  With N > 1 the line also carries a
+`sharded` record: ONE cfg3 event's targets sharded over the N ranks (strong scaling, exchange included).
 """
 import argparse
 import json
@@ -74,6 +79,10 @@ class ClockSampler:
     def mark_end(self):
         self.t1 = time.perf_counter()
 
+    def window(self, t0, t1):
+        """Summary of the samples taken in [t0, t1] (a secondary leg's timed region)."""
+        return self._summary([r for t, r in list(self.rows) if t0 <= t <= t1 + 0.06])
+
     def stop(self):
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
@@ -83,7 +92,9 @@ class ClockSampler:
             self.proc.wait(timeout=5)
         except Exception:
             self.proc.kill()
-        inside = [r for t, r in self.rows if self.t0 is not None and self.t0 <= t <= (self.t1 or t) + 0.06]
+        return self._summary([r for t, r in self.rows if self.t0 is not None and self.t0 <= t <= (self.t1 or t) + 0.06])
+
+    def _summary(self, inside):
         sm, mx, reasons = [], 0.0, set()
         for r in inside:
             try:
@@ -159,12 +170,176 @@ def run_reference(args):
     return 0
 
 
+
+# ----------------------------------------------------------------------------------------------- secondary legs
+def _peak_pairs(peaks):
+    return SM_COUNT * LANES * 2.0 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / FLOP_PER_PAIR
+
+
+def leg_per_config(torch, binding, workloads, stream, peaks, sampler, configs=(0, 1, 2, 3, 4), reuse=None):
+    """BASELINE.json configs 0-4 (north_star: "throughput on synthetic clouds and tracks ... as pair interactions/s, and
+    as seconds per event"): per-step rate at step 0 (CUDA events around step(10) right after the load, best of 3) and
+    seconds per event (wall clock: load_carriers from pinned host -> run_to_collection -> read_image; best of 3, cfg4
+    once).  `reuse` = {cfg: event record} already measured by the caller (the headline's cfg2 event)."""
+    peak = _peak_pairs(peaks)
+    out = []
+    for cfg in configs:
+        w = workloads.make(cfg)
+        xyz, n = w["xyz"], len(w["xyz"])
+        sim = binding.from_workload(w, stream=stream)
+        host_in = torch.from_numpy(xyz).pin_memory()
+        t_leg0 = time.perf_counter()
+        k_steps = 10
+        best_ms, na0 = 1e30, 0
+        for _ in range(3 if cfg < 4 else 2):
+            sim.reset()
+            sim.load_carriers_ptr(host_in.data_ptr(), n)
+            st0 = sim.state()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); sim.step(k_steps); e1.record(); torch.cuda.synchronize()
+            st1 = sim.state()
+            ms = e0.elapsed_time(e1)
+            if ms < best_ms:
+                best_ms, pairs10, na0 = ms, st1["pair_interactions"] - st0["pair_interactions"], st0["n_active"]
+        row = {"config": cfg, "workload": w["name"], "n_loaded": n, "n_active_at_step_0": na0,
+               "ms_per_step_at_step_0": best_ms / k_steps,
+               "G_pairs_per_s_at_step_0": pairs10 / (best_ms * 1e-3) / 1e9,
+               "frac_of_fp32_peak_at_step_0": pairs10 / (best_ms * 1e-3) / peak}
+        if reuse and cfg in reuse:
+            row["event"] = reuse[cfg]
+        else:
+            runs = []
+            for _ in range(3 if cfg < 4 else 1):
+                sim.reset()
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                sim.load_carriers_ptr(host_in.data_ptr(), n)
+                done, left, rc = sim.run_to_collection(10 ** 7)
+                img, over = sim.read_image()
+                torch.cuda.synchronize()
+                runs.append(time.perf_counter() - t0)
+                st2 = sim.state()
+                assert left == 0 and int(img.sum()) + over == n, "hole count not conserved (cfg%d)" % cfg
+            ev_s = min(runs)
+            row["event"] = {"seconds": ev_s, "seconds_median": float(np.median(runs)), "runs": len(runs), "steps": done,
+                            "pair_interactions": st2["pair_interactions"], "holes": n,
+                            "avg_G_pairs_per_s": st2["pair_interactions"] / ev_s / 1e9,
+                            "avg_frac_of_fp32_peak": st2["pair_interactions"] / ev_s / peak,
+                            "collected_in_window": int(img.sum())}
+        row["clocks"] = sampler.window(t_leg0, time.perf_counter())
+        out.append(row)
+        sim.close()
+    return out
+
+
+def leg_n_sweep(torch, binding, workloads, stream, peaks, sizes):
+    """Per-step device time against N at the cfg-2 geometry, Coulomb on and off: the shape of the paper's Fig. 4
+    experiment.  CUDA events around step(K) after a warm-up of 8 steps, best of 3."""
+    peak = _peak_pairs(peaks)
+    rows = []
+    for n in sizes:
+        w = workloads.make(WORKLOAD_CFG, n=n)
+        row = {"n": n}
+        for name, flags in (("coulomb_on", 0), ("coulomb_off", binding.COULOMB_OFF)):
+            sim = binding.from_workload(w, flags=flags, stream=stream)
+            sim.load_carriers(w["xyz"])
+            k = 16 if (flags or n <= 131072) else 4
+            sim.step(8 if n <= 131072 else 2)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            best = 1e30
+            for _ in range(3 if n <= 262144 else 2):
+                e0.record(); sim.step(k); e1.record(); torch.cuda.synchronize()
+                best = min(best, e0.elapsed_time(e1) / k)
+            row[name + "_us_per_step"] = best * 1e3
+            if not flags:
+                na = sim.state()["n_active"]
+                row["G_pairs_per_s"] = na * float(na) / (best * 1e-3) / 1e9
+                row["frac_of_fp32_peak"] = na * float(na) / (best * 1e-3) / peak
+            sim.close()
+        rows.append(row)
+    return rows
+
+
+def leg_sharded_virtual(torch, binding, workloads, sharded, stream, peaks, cfg, G, steps, warmup, farfield=-1.0):
+    """ONE event's targets sharded over G virtual ranks on ONE GPU: the ranks' kernels run one
+    after the other on one stream and are timed separately (shard_local + shard_commit, CUDA events); the per-step
+    all-gather over NVLink is NOT in these numbers (one GPU available)."""
+    w = workloads.make(int(cfg))
+    xyz, n = w["xyz"], len(w["xyz"])
+    alloc = lambda nb: torch.empty(nb, dtype=torch.uint8, device="cuda")
+    es = [binding.from_workload(w, stream=stream) for _ in range(G)]
+    vr = sharded.VirtualRanks(es, alloc)
+    vr.load_carriers(xyz)
+    if farfield >= 0:
+        for e in es:
+            e.set_farfield(farfield)
+    vr.step(warmup)
+    st = vr.refresh()
+    na = st["n_active"]
+    K = steps
+    evs = [[(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+            for _ in range(G)] for _ in range(K)]
+    for k in range(K):                                    # VirtualRanks.step unrolled so each rank's kernels are bracketed
+        msgs = vr.msgs[vr.k & 1]; vr.k += 1
+        for g_, (e, m) in enumerate(zip(es, msgs)):
+            evs[k][g_][0].record(); e.shard_local(m.data_ptr(), vr.nbytes); evs[k][g_][1].record()
+        ptrs = [m.data_ptr() for m in msgs]
+        for g_, e in enumerate(es):
+            e.shard_commit(ptrs, vr.nbytes); evs[k][g_][2].record()
+    torch.cuda.synchronize()
+    local_ms = np.array([[evs[k][g_][0].elapsed_time(evs[k][g_][1]) for g_ in range(G)] for k in range(K)])
+    commit_ms = np.array([[(evs[k][g_ - 1][2] if g_ else evs[k][G - 1][1]).elapsed_time(evs[k][g_][2]) for g_ in range(G)]
+                          for k in range(K)])
+    per_rank = (local_ms + commit_ms).mean(axis=0)
+    st1 = vr.refresh()
+    rec = {"mode": "sharded-virtual", "farfield_theta": farfield if farfield >= 0 else None, "virtual_ranks": G,
+           "workload": w["name"], "n_holes": n, "n_active_start": na, "n_active_end": st1["n_active"], "steps": K,
+           "per_rank_ms_per_step": [float(v) for v in per_rank],
+           "max_rank_ms_per_step": float(per_rank.max()), "sum_ranks_ms_per_step": float(per_rank.sum()),
+           "commit_ms": float(commit_ms.mean()), "message_bytes": vr.nbytes,
+           "frac_of_fp32_peak_per_rank": (float(na * float(na) / G / (per_rank.max() * 1e-3) / _peak_pairs(peaks))
+                                          if farfield < 0 else None),      # pairs evaluated only in the exact path
+           "note": "each rank's kernels measured alone on one B200; the per-step all-gather of G messages over NVLink "
+                   "is not included (one GPU available)"}
+    for e in es:
+        e.close()
+    return rec
+
+
+def leg_sharded_real(torch, dist, binding, workloads, sharded, replicas, stream, rank, world, cfg, steps, warmup, exchange):
+    """ONE event sharded over the `world` ranks of this job (torchrun / --gpus N): strong scaling, device time of
+    `steps` sharded steps, exchange (NCCL all-gather, or symmetric-memory peer loads) included, max over ranks."""
+    w = workloads.make(int(cfg))
+    alloc = lambda nb: torch.empty(nb, dtype=torch.uint8, device="cuda")
+    if exchange == "symm":
+        xf = lambda mb: sharded.SymmMemExchange(torch, "cuda", mb, world)
+    else:
+        xf = lambda mb: sharded.DistExchange(torch, "cuda", mb, world)
+    ev = sharded.ShardedEvent(binding.from_workload(w, stream=stream), rank, world, xf, alloc)
+    ev.load_carriers(w["xyz"])
+    ev.step(warmup)
+    st0 = ev.refresh()
+    dist.barrier(); torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(); ev.step(steps); e1.record()
+    dist.barrier(); torch.cuda.synchronize()
+    tot = ev.totals(sharded.dist_reduce_sum(torch, "cuda"))
+    ms, _ = replicas.aggregate(e0.elapsed_time(e1), 0.0, device="cuda")
+    ev.e.close()
+    return {"mode": "sharded", "n_gpus": world, "workload": w["name"], "n_holes": len(w["xyz"]), "steps": steps,
+            "ms_per_step": ms / steps, "n_active_start": st0["n_active"], "n_active": tot["n_active"], "scaling": "strong",
+            "pair_interactions": tot["pair_interactions"],
+            "exchange": ("symmetric memory (peer loads in shard_commit)" if exchange == "symm" else
+                         "NCCL all_gather_into_tensor") + " of %d-byte messages" % ev.nbytes}
+
+
 # ----------------------------------------------------------------------------------------------- our arm
 def run_ours(args):
     import torch
     import torch.distributed as dist
     import workloads
-    from paper_2203_11043_b200 import binding, replicas
+    from paper_2203_11043_b200 import binding, replicas, sharded
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -209,7 +384,7 @@ def run_ours(args):
     barrier()
     sampler.mark_end()
     ms = sum(a.elapsed_time(b) for a, b in ev)
-    clocks = sampler.stop() if rank == 0 else None
+    clocks = sampler.window(sampler.t0, sampler.t1) if rank == 0 else None
     launches = sim.kernel_launches() - l0
     st = sim.state()
     pairs = st["pair_interactions"] - p0
@@ -223,16 +398,30 @@ def run_ours(args):
     adv_ms = float(np.mean([p["advance"] for p in prof]))
     peak_tf = SM_COUNT * LANES * 2.0 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12
     ach_tf = FLOP_PER_PAIR * float(n_act) ** 2 / (field_ms * 1e-3) / 1e12
-    traffic = None
-    try:
+    traffic, traffic_src, adv_inst = None, None, None
+    try:                                                               # NOT measured by this run: a stored ncu capture
         with open(os.path.join(ROOT, "profiles", "field_traffic.json")) as f:
-            traffic = json.load(f).get("dram_bytes_per_launch")
+            tj = json.load(f)
+        traffic, adv_inst = tj.get("dram_bytes_per_launch"), tj.get("advance_warp_inst_per_warp")
+        traffic_src = "static: profiles/field_traffic.json (%s)" % tj.get("source", "ncu capture")
     except Exception:
         pass
+    # a2..a8 (k_advance): not bound by HBM (its bytes are L2-resident) and not by FP64 throughput (pipe 14 % busy) but by
+    # the latency of a ~1,500-instruction dependent chain per carrier at 0.86 waves; the floor quoted is
+    # the instruction-issue time of that stream: warps x instructions / (SMs x 4 schedulers x clock)
+    clock_hz = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
+    issue_floor_ms = (adv_inst * (n_act / 32.0) / (SM_COUNT * 4.0 * clock_hz) * 1e3) if adv_inst else None
+    adv = {"kernel": "k_advance", "ms": adv_ms, "algorithmic_bytes_per_carrier": 32 + 12 * 16,
+           "GBps_of_algorithmic_bytes": (32.0 + 12.0 * 16) * n_act / (adv_ms * 1e-3) / 1e9, "hbm_peak_GBps": peaks.get("hbm_gbs"),
+           "frac_of_hbm_peak": (32.0 + 12.0 * 16) * n_act / (adv_ms * 1e-3) / 1e9 / float(peaks.get("hbm_gbs", 6650.0)),
+           "bound": "latency of the per-carrier dependent chain (L2 round trips of the chunk partials + FP64 update), 0.86 waves",
+           "warp_inst_per_warp": adv_inst, "issue_floor_ms": issue_floor_ms,
+           "frac_of_issue_floor": (issue_floor_ms / adv_ms) if issue_floor_ms else None}
     roofline = {"bound": "alu", "kernel": "k_field", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
-                "frac": ach_tf / peak_tf, "traffic": traffic, "peak_source": "148 SM x 128 FP32 lanes x 2 x sm_max_mhz (%s)" % peak_src,
+                "frac": ach_tf / peak_tf, "traffic": traffic, "traffic_source": traffic_src,
+                "peak_source": "148 SM x 128 FP32 lanes x 2 x sm_max_mhz (%s)" % peak_src,
                 "flop_per_pair": FLOP_PER_PAIR, "field_ms": field_ms, "n_active": n_act,
-                "other_kernels": {"advance_ms": adv_ms}}
+                "other_kernels": {"advance": adv}}
 
     # ---- e2e through the C ABI with host buffers (copies inside the timed region)
     host_in = torch.from_numpy(xyz).pin_memory()
@@ -328,10 +517,30 @@ def run_ours(args):
             batched.append(best)
             bs.close()
 
+    # ---- ONE event sharded over the job's ranks (N > 1 only; strong scaling; not the headline, which is replicas)
+    sharded_rec = None
+    if world > 1 and not args.no_event:
+        sharded_rec = leg_sharded_real(torch, dist, binding, workloads, sharded, replicas, stream, rank, world, 3,
+                                       max(8, args.steps), args.warmup, "nccl")
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return 0
+
+    # ---- every config, the N sweep, 8 virtual ranks (rank 0, N = 1; each leg clock-sampled like the headline)
+    per_config = n_sweep = sharded_virtual = None
+    if world == 1 and not args.no_event and not args.quick:
+        per_config = leg_per_config(torch, binding, workloads, stream, peaks, sampler,
+                                    reuse={2: dict(event, avg_frac_of_fp32_peak=event["avg_G_pairs_per_s"] * 1e9 / _peak_pairs(peaks))})
+        t0 = time.perf_counter()
+        n_sweep = {"rows": leg_n_sweep(torch, binding, workloads, stream, peaks, [2 ** k for k in range(10, 21)]),
+                   "what": "cfg-2 geometry, us per step through gcoreccd_step (CUDA events, best of 3), Coulomb on / off"}
+        n_sweep["clocks"] = sampler.window(t0, time.perf_counter())
+        t0 = time.perf_counter()
+        sharded_virtual = leg_sharded_virtual(torch, binding, workloads, sharded, stream, peaks, 3, 8, 8, 3)
+        sharded_virtual["clocks"] = sampler.window(t0, time.perf_counter())
+    sampler.stop()
 
     # ---- CPU baseline: the oracle as it stands on a bounded sample (rank 0, N = 1 only)
     cpu = None
@@ -353,7 +562,8 @@ def run_ours(args):
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": n * 12, "d2h_bytes_per_step": n * 12,
                     "what": "reset + load_carriers(pinned host) + step(1) + read_carriers(host), wall clock"},
             "roofline": roofline, "cpu_baseline": cpu, "seconds_per_event": event, "farfield_variant": farfield,
-            "batched_events": batched}
+            "batched_events": batched, "per_config": per_config, "n_sweep": n_sweep, "sharded_virtual": sharded_virtual,
+            "sharded": sharded_rec}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
@@ -361,35 +571,14 @@ def run_ours(args):
 
 
 def run_sweep(args):
-    """N sweep at fixed geometry (cfg-2 cloud), Coulomb on and off, 16 steps each through the graph path: the shape of
-    the paper's Fig. 4 experiment.  One JSON line per size; not the headline number."""
+    """--sweep N,...: the n_sweep leg alone, one JSON line per size (not the headline number)."""
     import torch
     import workloads
     from paper_2203_11043_b200 import binding
     peaks, _ = measured_peaks()
-    peak_pairs = SM_COUNT * LANES * 2.0 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / FLOP_PER_PAIR
-    sizes = [int(t) for t in args.sweep.split(",")]
     stream = torch.cuda.Stream()
     torch.cuda.set_stream(stream)
-    for n in sizes:
-        w = workloads.make(WORKLOAD_CFG, n=n)
-        row = {"n": n}
-        for name, flags in (("coulomb_on", 0), ("coulomb_off", binding.COULOMB_OFF)):
-            sim = binding.from_workload(w, flags=flags, stream=stream)
-            sim.load_carriers(w["xyz"])
-            sim.step(8)
-            torch.cuda.synchronize()
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            best = 1e30
-            for _ in range(3):
-                e0.record(); sim.step(16); e1.record(); torch.cuda.synchronize()
-                best = min(best, e0.elapsed_time(e1) / 16.0)
-            row[name + "_ms_per_step"] = best
-            if not flags:
-                na = sim.state()["n_active"]
-                row["G_pairs_per_s"] = na * float(na) / (best * 1e-3) / 1e9
-                row["frac_of_fp32_peak"] = na * float(na) / (best * 1e-3) / peak_pairs
-            sim.close()
+    for row in leg_n_sweep(torch, binding, workloads, stream, peaks, [int(t) for t in args.sweep.split(",")]):
         print(json.dumps(row), flush=True)
     return 0
 
@@ -407,79 +596,57 @@ def run_sharded(args):
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     torch.cuda.set_device(local)
-    w = workloads.make(int(args.sharded))
-    xyz, n = w["xyz"], len(w["xyz"])
     stream = torch.cuda.Stream()
     torch.cuda.set_stream(stream)
-    alloc = lambda nb: torch.empty(nb, dtype=torch.uint8, device="cuda")
     peaks, _ = measured_peaks()
-    peak_pairs = SM_COUNT * LANES * 2.0 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / FLOP_PER_PAIR
     if world > 1 or args.exchange != "virtual":        # torchrun (any world size, also 1): the real multi-process path
         if not dist.is_initialized():
             if "RANK" not in os.environ:
                 os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=os.environ.get("MASTER_PORT", "29511"), RANK="0", WORLD_SIZE="1")
             dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-        if args.exchange == "symm":
-            xf = lambda mb: sharded.SymmMemExchange(torch, "cuda", mb, world)
-        else:
-            xf = lambda mb: sharded.DistExchange(torch, "cuda", mb, world)
-        ev = sharded.ShardedEvent(binding.from_workload(w, stream=stream), rank, world, xf, alloc)
-        ev.load_carriers(xyz)
-        if args.farfield >= 0:
-            ev.e.set_farfield(args.farfield)
-        ev.step(args.warmup)
-        st0 = ev.refresh()
-        dist.barrier(); torch.cuda.synchronize()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record(); ev.step(args.steps); e1.record()
-        dist.barrier(); torch.cuda.synchronize()
-        tot = ev.totals(sharded.dist_reduce_sum(torch, "cuda"))
-        ms, _ = replicas.aggregate(e0.elapsed_time(e1), 0.0, device="cuda")
-        line = None
+        rec = leg_sharded_real(torch, dist, binding, workloads, sharded, replicas, stream, rank, world, int(args.sharded),
+                               args.steps, args.warmup, args.exchange)
         if rank == 0:
-            line = {"mode": "sharded", "n_gpus": world, "workload": w["name"], "n_holes": n, "steps": args.steps,
-                    "ms_per_step": ms / args.steps, "n_active": tot["n_active"], "scaling": "strong",
-                    "pair_interactions": tot["pair_interactions"],
-                    "exchange": ("symmetric memory (peer loads in shard_commit)" if args.exchange == "symm" else
-                                 "NCCL all_gather_into_tensor") + " of %d-byte messages" % ev.nbytes}
-            print(json.dumps(line), flush=True)
+            print(json.dumps(rec), flush=True)
         dist.destroy_process_group()
         return 0
-    G = args.virtual_ranks
-    es = [binding.from_workload(w, stream=stream) for _ in range(G)]
-    vr = sharded.VirtualRanks(es, alloc)
-    vr.load_carriers(xyz)
-    if args.farfield >= 0:
-        for e in es:
-            e.set_farfield(args.farfield)
-    vr.step(args.warmup)
-    st = vr.refresh()
-    na = st["n_active"]
-    K = args.steps
-    evs = [[(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
-            for _ in range(G)] for _ in range(K)]
-    for k in range(K):                                    # VirtualRanks.step unrolled so each rank's kernels are bracketed
-        msgs = vr.msgs[vr.k & 1]; vr.k += 1
-        for g_, (e, m) in enumerate(zip(es, msgs)):
-            evs[k][g_][0].record(); e.shard_local(m.data_ptr(), vr.nbytes); evs[k][g_][1].record()
-        ptrs = [m.data_ptr() for m in msgs]
-        for g_, e in enumerate(es):
-            e.shard_commit(ptrs, vr.nbytes); evs[k][g_][2].record()
-    torch.cuda.synchronize()
-    local_ms = np.array([[evs[k][g_][0].elapsed_time(evs[k][g_][1]) for g_ in range(G)] for k in range(K)])
-    commit_ms = np.array([[(evs[k][g_ - 1][2] if g_ else evs[k][G - 1][1]).elapsed_time(evs[k][g_][2]) for g_ in range(G)]
-                          for k in range(K)])
-    per_rank = (local_ms + commit_ms).mean(axis=0)
-    st1 = vr.refresh()
-    line = {"mode": "sharded-virtual", "farfield_theta": args.farfield if args.farfield >= 0 else None, "virtual_ranks": G, "workload": w["name"], "n_holes": n, "n_active_start": na,
-            "n_active_end": st1["n_active"], "steps": K, "per_rank_ms_per_step": [float(v) for v in per_rank],
-            "max_rank_ms_per_step": float(per_rank.max()), "sum_ranks_ms_per_step": float(per_rank.sum()),
-            "commit_ms": float(commit_ms.mean()), "message_bytes": vr.nbytes,
-            "frac_of_fp32_peak_per_rank": (float(na * float(na) / G / (per_rank.max() * 1e-3) / peak_pairs)
-                                           if args.farfield < 0 else None),      # pairs evaluated only in the exact path
-            "note": "each rank's kernels measured alone on one B200; the per-step all-gather of G messages over NVLink "
-                    "is not included (one GPU available)"}
-    print(json.dumps(line), flush=True)
+    rec = leg_sharded_virtual(torch, binding, workloads, sharded, stream, peaks, int(args.sharded), args.virtual_ranks,
+                              args.steps, args.warmup, args.farfield)
+    print(json.dumps(rec), flush=True)
+    return 0
+
+
+def run_microbench(args):
+    """--microbench: instruction-throughput probes behind DESIGN.md 6.1 / 6.8 (one SM; cycles per warp-instruction per
+    SM sub-partition; 2.0 = a packed FP32x2 instruction at full lane rate).  One JSON line."""
+    from paper_2203_11043_b200 import binding
+    rows = []
+    for kind, name in enumerate(binding.MICRO_KINDS):
+        rows.append({"kind": name, **{"warps_%d" % w: round(binding.microbench(kind, 4096, w), 3) for w in (1, 2, 4)}})
+    print(json.dumps({"microbench": rows, "unit": "cycles per warp-instruction per SM sub-partition"}), flush=True)
+    return 0
+
+
+def _spawned(local_rank, args, port):
+    os.environ.update(RANK=str(local_rank), LOCAL_RANK=str(local_rank), WORLD_SIZE=str(args.gpus),
+                      MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    sys.exit(dispatch(args))
+
+
+def spawn_ranks(args):
+    """`python bench.py --gpus N` without torchrun: one process per GPU of this node, same code path as under torchrun."""
+    import socket
+    import torch
+    have = torch.cuda.device_count()
+    if have < args.gpus:
+        sys.stderr.write("bench.py: --gpus %d asked for but this box has %d CUDA device(s); refusing to run fewer ranks "
+                         "than asked (launch on a node with %d GPUs, or pass --gpus %d)\n" % (args.gpus, have, args.gpus, max(have, 1)))
+        return 2
+    with socket.socket() as s_:
+        s_.bind(("127.0.0.1", 0))
+        port = s_.getsockname()[1]
+    import torch.multiprocessing as mp
+    mp.spawn(_spawned, args=(args, port), nprocs=args.gpus, join=True)
     return 0
 
 
@@ -491,6 +658,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-event", action="store_true", help="skip the seconds-per-event run")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--microbench", action="store_true", help="instruction-throughput probes (DESIGN.md 6.1 / 6.8)")
+    ap.add_argument("--quick", action="store_true", help="skip the per_config / n_sweep / sharded_virtual legs")
     ap.add_argument("--sweep", default="", help="comma-separated hole counts: per-step time vs N (not the headline)")
     ap.add_argument("--sharded", default="", help="config number: one event sharded over the ranks (not the headline)")
     ap.add_argument("--virtual-ranks", type=int, default=8, help="with --sharded on ONE GPU: ranks emulated sequentially")
@@ -498,6 +667,17 @@ def main():
     ap.add_argument("--exchange", default="virtual", choices=["virtual", "nccl", "symm"],
                     help="with --sharded: how the shard messages travel (virtual = one process, no exchange)")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl != "reference" and not args.sweep:
+        return spawn_ranks(args)
+    if "WORLD_SIZE" in os.environ and int(os.environ["WORLD_SIZE"]) != args.gpus and not args.sharded:
+        sys.stderr.write("bench.py: --gpus %d but WORLD_SIZE=%s\n" % (args.gpus, os.environ["WORLD_SIZE"]))
+        return 2
+    return dispatch(args)
+
+
+def dispatch(args):
+    if args.microbench:
+        return run_microbench(args)
     if args.sharded:
         return run_sharded(args)
     if args.sweep:

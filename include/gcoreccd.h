@@ -279,6 +279,14 @@ uint64_t gcoreccd_kernel_launches(gcoreccd_t* h);
 int gcoreccd_debug_normals(gcoreccd_t* h, const uint32_t* id_host, const uint64_t* step_host, uint64_t n,
                            double* n_xyz_host, uint32_t* words_host);
 
+/* Instruction-throughput probe (no handle; current device): runs `iters` x 32 instructions of one kind on one SM with
+ * `warps_per_subpartition` (1..4) warps per SM sub-partition and returns the cycles per warp-instruction per
+ * sub-partition.  Kinds: 0 FFMA2 three distinct operands, 1 FFMA2 a*a+c, 2 FFMA2 one operand shared by consecutive
+ * instructions, 3 FADD2, 4 FMUL2, 5 scalar FFMA three distinct, 6 scalar FFMA shared operand, 7 DFMA, 8 MUFU.RSQ,
+ * 9 the 11 packed instructions + 2 MUFU of one eq. 6 interaction pair (per packed instruction).  The evidence behind
+ * DESIGN.md 6.1 / 6.8 (`python bench.py --microbench`); not on the hot path. */
+int gcoreccd_debug_microbench(int kind, uint32_t iters, uint32_t warps_per_subpartition, double* cycles_per_inst_host);
+
 const char* gcoreccd_strerror(int code);
 const char* gcoreccd_last_error(gcoreccd_t* h);   /* detail of the last failure on this handle ("" if none) */
 const char* gcoreccd_version(void);

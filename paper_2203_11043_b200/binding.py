@@ -24,7 +24,7 @@ EXPORTS = ["gcoreccd_workspace_size", "gcoreccd_create", "gcoreccd_destroy", "gc
            "gcoreccd_load_carriers_file", "gcoreccd_save_collected_file",
            "gcoreccd_set_farfield", "gcoreccd_farfield_stats",
            "gcoreccd_set_shard", "gcoreccd_shard_message_bytes", "gcoreccd_shard_local", "gcoreccd_shard_commit",
-           "gcoreccd_profile_step", "gcoreccd_set_persistent", "gcoreccd_kernel_launches", "gcoreccd_debug_normals", "gcoreccd_strerror",
+           "gcoreccd_profile_step", "gcoreccd_set_persistent", "gcoreccd_kernel_launches", "gcoreccd_debug_normals", "gcoreccd_debug_microbench", "gcoreccd_strerror",
            "gcoreccd_last_error", "gcoreccd_version"]
 
 
@@ -127,6 +127,8 @@ def lib():
     L.gcoreccd_kernel_launches.argtypes = [vp]
     L.gcoreccd_debug_normals.restype = C.c_int
     L.gcoreccd_debug_normals.argtypes = [vp, u32p, u64p, C.c_uint64, C.POINTER(C.c_double), u32p]
+    L.gcoreccd_debug_microbench.restype = C.c_int
+    L.gcoreccd_debug_microbench.argtypes = [C.c_int, C.c_uint32, C.c_uint32, C.POINTER(C.c_double)]
     L.gcoreccd_strerror.restype = C.c_char_p
     L.gcoreccd_strerror.argtypes = [C.c_int]
     L.gcoreccd_last_error.restype = C.c_char_p
@@ -147,6 +149,19 @@ def version():
 
 def xray_hole_count(E_e_eV, w_eV=3.77):
     return int(lib().gcoreccd_xray_hole_count(float(E_e_eV), float(w_eV)))
+
+
+MICRO_KINDS = ["FFMA2 three distinct operands", "FFMA2 a*a+c", "FFMA2 shared operand", "FADD2", "FMUL2",
+               "FFMA scalar three distinct", "FFMA scalar shared operand", "DFMA", "MUFU.RSQ", "eq. 6 mix (per packed instruction)"]
+
+
+def microbench(kind, iters=4096, warps_per_subpartition=2):
+    """Cycles per warp-instruction per SM sub-partition (include/gcoreccd.h gcoreccd_debug_microbench)."""
+    out = C.c_double()
+    rc = lib().gcoreccd_debug_microbench(int(kind), int(iters), int(warps_per_subpartition), C.byref(out))
+    if rc != OK:
+        raise GcoreccdError(rc, "gcoreccd_debug_microbench")
+    return float(out.value)
 
 
 def workspace_size(max_carriers, img_nx, img_ny):

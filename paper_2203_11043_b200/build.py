@@ -16,7 +16,7 @@ LIB = os.path.join(LIBDIR, "libgcoreccd.so")
 HEADER = os.path.join(os.path.dirname(_HERE), "include", "gcoreccd.h")
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
+              "-Xcompiler", "-fPIC", "-shared", "-cudart", "static", "-ldl"]
 
 
 def _sources():

@@ -11,6 +11,8 @@
 #include <cstdlib>
 #include <vector>
 
+#include <nvtx3/nvToolsExt.h>      // header-only NVTX v3: ranges are no-ops unless a tool (nsys, ncu) is attached
+
 #include "gc_common.cuh"
 #include "gc_advance.cuh"
 #include "gc_compact.cuh"
@@ -18,6 +20,7 @@
 #include "gc_field.cuh"
 #include "gc_frontend.cuh"
 #include "gc_integrate.cuh"
+#include "gc_microbench.cuh"
 #include "gc_persist.cuh"
 #include "gc_shard.cuh"
 #include "gc_tree.cuh"
@@ -148,6 +151,12 @@ struct gcoreccd {
 
 namespace {
 
+// NVTX range around a host-side phase (SURVEY.md section 5 "Tracing"): field / advance / re-sort / load / batch of steps
+struct Range {
+  explicit Range(const char* name) { nvtxRangePushA(name); }
+  ~Range() { nvtxRangePop(); }
+};
+
 struct DeviceGuard {
   int prev;
   bool changed;
@@ -226,6 +235,7 @@ int launch_tree_field(gcoreccd_t* h) {
   k_tree_reset<<<1, 256, 0, h->stream>>>(T.tc, sort ? 1 : 0);
   h->launches += 1;
   if (sort) {
+    Range r_sort("gcoreccd: Hilbert re-sort");
     k_tree_bbox<<<std::min<uint32_t>(tiles, (uint32_t)h->num_sms * 4u), kTPB, 0, h->stream>>>(h->A.x, h->A.y, h->A.z, h->ctrl, T.tc);
     k_tree_keys<<<tiles, kTPB, 0, h->stream>>>(h->A.x, h->A.y, h->A.z, h->ctrl, T.tc, T.key[0], T.val[0]);
     const uint32_t sb = (uint32_t)((nb + kSortBlock - 1) / kSortBlock);
@@ -257,6 +267,7 @@ int launch_tree_field(gcoreccd_t* h) {
 }
 
 int launch_field(gcoreccd_t* h, int v) {
+  Range r_field(h->ff_parts ? "gcoreccd: field (treecode)" : "gcoreccd: field (all pairs)");
   if (h->ff_parts) return launch_tree_field(h);
   const int g = h->grid_field[v];
   const uint32_t pc = (uint32_t)h->L.part_cap;
@@ -274,6 +285,7 @@ int launch_field(gcoreccd_t* h, int v) {
 void enqueue_step(gcoreccd_t* h, uint32_t tiles) {
   const bool coulomb = !(h->dp.flags & GCORECCD_COULOMB_OFF);
   if (coulomb) launch_field(h, h->variant);
+  Range r_adv("gcoreccd: advance (a2..a8)");
   k_advance<<<tiles, kTPB, 0, h->stream>>>(h->A, h->ctrl, h->Ep, (uint32_t)h->L.part_cap, h->sink, h->scan, h->dp,
                                            plan_args(h, h->variant), coulomb ? 1u : 0u);
   h->launches += 1;
@@ -281,6 +293,7 @@ void enqueue_step(gcoreccd_t* h, uint32_t tiles) {
 
 // Small populations: up to 2^20 steps in ONE cooperative launch (gc_persist.cuh).
 int launch_persistent(gcoreccd_t* h, uint32_t n_steps) {
+  Range r_p("gcoreccd: persistent steps (field + advance per step, one launch)");
   const int v = h->variant;
   SoA A = h->A; SoA B = h->B; Ctrl* ctrl = h->ctrl; float* Ep = h->Ep; uint32_t pc = (uint32_t)h->L.part_cap; Sink sink = h->sink;
   unsigned long long* scan = h->scan; DevParams dp = h->dp; PlanArgs pa = plan_args(h, v);
@@ -369,6 +382,7 @@ int ensure_graph(gcoreccd_t* h, uint32_t tiles) {
 
 int enqueue_steps(gcoreccd_t* h, uint64_t n_steps) {
   if (n_steps == 0 || h->n_bound == 0) return 0;
+  Range r_steps("gcoreccd: batch of steps");
   int rc = ensure_variant(h);
   if (rc) return rc;
   const uint32_t tiles = bucket_tiles(tiles_for(h->n_bound));
@@ -617,6 +631,7 @@ int gcoreccd_load_carriers(gcoreccd_t* h, const float* xyz, uint64_t n, int on_d
   if (!h || (!xyz && n)) return GCORECCD_ERR_INVALID;
   if (n == 0) return GCORECCD_OK;
   if (events_busy(h)) return fail(h, GCORECCD_ERR_STATE, "load_carriers: a batch of events is still drifting (run_events or reset first)");
+  Range r_load("gcoreccd: load_carriers");
   DeviceGuard guard(h->device);
   int rc = sync_ctrl(h);
   if (rc) return rc;
@@ -1152,6 +1167,7 @@ int gcoreccd_run_events(gcoreccd_t* h, uint64_t max_steps, uint64_t* events_left
   if (!h) return GCORECCD_ERR_INVALID;
   auto& B = h->evb;
   if (!B.loaded) return fail(h, GCORECCD_ERR_STATE, "run_events: no batch loaded");
+  Range r_ev("gcoreccd: run_events");
   DeviceGuard guard(h->device);
   int ret = GCORECCD_OK;
   if (B.carriers_left > 0) {
@@ -1369,6 +1385,38 @@ int gcoreccd_save_collected_file(gcoreccd_t* h, const char* path, uint64_t* n_wr
   const bool ok = fclose(f) == 0;
   if (n_written) *n_written = w;
   return ok ? GCORECCD_OK : fail(h, GCORECCD_ERR_INVALID, "save_collected_file: write failed");
+}
+
+int gcoreccd_debug_microbench(int kind, uint32_t iters, uint32_t warps_per_subpartition, double* cycles_per_inst) {
+  if (kind < 0 || kind >= kMicroKinds || iters == 0 || warps_per_subpartition < 1 || warps_per_subpartition > 4 || !cycles_per_inst)
+    return GCORECCD_ERR_INVALID;
+  const int threads = 128 * (int)warps_per_subpartition;      // 4 sub-partitions x 32 lanes x warps
+  long long* d_cyc = nullptr;
+  float* d_sink = nullptr;
+  if (cudaMalloc((void**)&d_cyc, 16 * sizeof(long long)) != cudaSuccess) return GCORECCD_ERR_NOMEM;
+  if (cudaMalloc((void**)&d_sink, 4) != cudaSuccess) { cudaFree(d_cyc); return GCORECCD_ERR_NOMEM; }
+  for (int rep = 0; rep < 2; ++rep) {                           // first launch warms the instruction cache
+    switch (kind) {
+      case 0: k_microbench<0><<<1, threads>>>(iters, 1.0f, d_cyc, d_sink); break;
+      case 1: k_microbench<1><<<1, threads>>>(iters, 1.0f, d_cyc, d_sink); break;
+      case 2: k_microbench<2><<<1, threads>>>(iters, 1.0f, d_cyc, d_sink); break;
+      case 3: k_microbench<3><<<1, threads>>>(iters, 1.0f, d_cyc, d_sink); break;
+      case 4: k_microbench<4><<<1, threads>>>(iters, 1.0f, d_cyc, d_sink); break;
+      case 5: k_microbench<5><<<1, threads>>>(iters, 1.0f, d_cyc, d_sink); break;
+      case 6: k_microbench<6><<<1, threads>>>(iters, 1.0f, d_cyc, d_sink); break;
+      case 7: k_microbench<7><<<1, threads>>>(iters, 1.0f, d_cyc, d_sink); break;
+      case 8: k_microbench<8><<<1, threads>>>(iters, 1.0f, d_cyc, d_sink); break;
+      default: k_microbench<9><<<1, threads>>>(iters, 1.0f, d_cyc, d_sink); break;
+    }
+  }
+  long long h_cyc[16];
+  cudaError_t e = cudaMemcpy(h_cyc, d_cyc, sizeof(h_cyc), cudaMemcpyDeviceToHost);
+  cudaFree(d_cyc); cudaFree(d_sink);
+  if (e != cudaSuccess) return GCORECCD_ERR_CUDA;
+  long long worst = 0;
+  for (int w = 0; w < threads / 32; ++w) worst = std::max(worst, h_cyc[w]);
+  *cycles_per_inst = (double)worst / ((double)iters * micro_inst_per_iter(kind) * (double)warps_per_subpartition);
+  return GCORECCD_OK;
 }
 
 #ifdef GC_TIMING

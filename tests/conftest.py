@@ -41,10 +41,11 @@ def pytest_terminal_summary(terminalreporter):
     log = os.environ.get("GCORECCD_EXCUSE_LOG")
     if log:
         with open(log, "w") as f:
-            for lab, n, k, rs in EXCUSED:
-                f.write("%d %d %s %s\n" % (k, n, lab, rs))
+            for e in EXCUSED:
+                f.write("%d %d %s %s ext=%d knock=%d\n" % (e[2], e[1], e[0], e[3], e[4] if len(e) > 4 else 0, e[5] if len(e) > 5 else 0))
     tot = sum(e[1] for e in EXCUSED)
     exc = sum(e[2] for e in EXCUSED)
     terminalreporter.write_line("R21 excuse clause: %d trajectory checks, %d carriers compared, %d excused (%.4f %%); "
-                                "largest single check: %d" % (len(EXCUSED), tot, exc, 100.0 * exc / max(tot, 1),
-                                                                max(e[2] for e in EXCUSED)))
+                                "largest single check: %d; R21b extended radius: %d, knock-on: %d"
+                                % (len(EXCUSED), tot, exc, 100.0 * exc / max(tot, 1), max(e[2] for e in EXCUSED),
+                                   sum(e[4] for e in EXCUSED if len(e) > 4), sum(e[5] for e in EXCUSED if len(e) > 5)))

@@ -70,21 +70,42 @@ def closest_encounters(history, suspects):
     return closest
 
 
-def traj_assert(xyz, ids, oxyz, oids, history, n_total, tol, r_enc=R_ENC, max_frac=0.02, label=""):
+def traj_assert(xyz, ids, oxyz, oids, history, n_total, tol, r_enc=R_ENC, max_frac=0.02, label="",
+                r_ext=None, max_ext=0, r_knock=None, max_knock=0):
     """GPU (xyz, ids) vs FP32-state oracle (oxyz, oids) after some steps; `history` = the oracle's (xyz, ids) before
     each of those steps.  DESIGN.md R21: a carrier may exceed `tol` (or differ in its retire flag) only if the ORACLE's
     trajectory shows a neighbour closer than r_enc = 0.1 um inside the window, and at most max_frac = 2 % (+2) may do
     so.  The number of excused carriers is recorded (EXCUSED) and bounded here, so the clause cannot silently absorb a
-    regression.  Returns the per-carrier max-coordinate error."""
+    regression.  DESIGN.md R21b (dense batched events only; the single-event tests leave these at 0): at most max_ext
+    carriers per check may instead show an encounter inside r_ext (several steps of amplification at 0.1-0.2 um), and
+    at most max_knock may be the knock-on of an excused carrier (closer than r_knock to one inside the window).
+    Returns the per-carrier max-coordinate error."""
     common = np.intersect1d(ids, oids)
     xyz_c, oxyz_c = xyz[np.isin(ids, common)], oxyz[np.isin(oids, common)]
     d = np.abs(xyz_c.astype(np.float64) - oxyz_c).max(axis=1) if len(common) else np.zeros(0)
     suspects = sorted(set(common[d > tol].tolist()) | set(np.setxor1d(ids, oids).tolist()))   # incl. retire-flag mismatches
     closest = closest_encounters(history, suspects) if suspects else {}
-    EXCUSED.append((label, int(n_total), len(suspects), sorted(round(r, 4) for r in closest.values())))
+    primary = [i for i, r in closest.items() if r < r_enc]
+    ext = [i for i, r in closest.items() if not r < r_enc and r_ext is not None and r < r_ext]
+    rest = [i for i in closest if i not in primary and i not in ext]
+    knock = []
+    if rest and r_knock is not None and (primary or ext):
+        for i in rest:
+            near = np.inf
+            for hx, hid in history:
+                k = np.searchsorted(hid, i)
+                kp = np.searchsorted(hid, primary + ext)
+                kp = kp[(kp < len(hid))]
+                kp = kp[np.isin(hid[kp], primary + ext)]
+                if k < len(hid) and hid[k] == i and len(kp):
+                    near = min(near, float(np.linalg.norm(hx[kp] - hx[k], axis=1).min()))
+            if near < r_knock:
+                knock.append(i)
+    EXCUSED.append((label, int(n_total), len(suspects), sorted(round(r, 4) for r in closest.values()), len(ext), len(knock)))
     if os.environ.get("GCORECCD_TRAJ_DIAG"):                 # survey mode: record every suspect, assert nothing
         return d
     assert len(suspects) <= max_frac * n_total + 2, (label, len(suspects), n_total)
-    bad = {i: r for i, r in closest.items() if not r < r_enc}
+    bad = {i: closest[i] for i in rest if i not in knock}
     assert not bad, (label, bad, "exceeds %g um without an oracle-side encounter inside %g um" % (tol, r_enc))
+    assert len(ext) <= max_ext and len(knock) <= max_knock, (label, len(ext), len(knock), [closest[i] for i in ext + knock])
     return d
