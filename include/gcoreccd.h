@@ -233,6 +233,13 @@ int gcoreccd_set_shard(gcoreccd_t* h, uint32_t rank, uint32_t world);
 uint64_t gcoreccd_shard_message_bytes(gcoreccd_t* h);
 int gcoreccd_shard_local(gcoreccd_t* h, void* msg_dev, uint64_t msg_bytes);
 int gcoreccd_shard_commit(gcoreccd_t* h, const void* const* msgs_host, uint32_t n_msgs, uint64_t msg_bytes);
+/* Peer-mapped messages (CUDA IPC / symmetric memory: msgs_host[g] points INTO rank g's own buffer): with on != 0 the
+ * commit kernel itself waits, message by message, until the header of THIS step has arrived (a 64-bit word written
+ * last, release at system scope, by shard_local: (epoch << 32) | step + 1, epoch changing at every reset / set_shard),
+ * so no barrier between shard_local and shard_commit is needed.  Requires two message buffers used alternately and
+ * ranks that really run at the same time on different GPUs; never set it when the messages of a step are produced
+ * AFTER the commit is enqueued on the same device (the kernel would wait forever).  Default off. */
+int gcoreccd_set_shard_wait(gcoreccd_t* h, int on);
 
 /* ---- Far-field approximation of eq. 6 — a VARIANT, off by default --------------------------
  * The exact path sums all N_a^2 ordered pairs.  With set_farfield(theta >= 0) step a1 is replaced by

@@ -23,7 +23,7 @@ EXPORTS = ["gcoreccd_workspace_size", "gcoreccd_create", "gcoreccd_destroy", "gc
            "gcoreccd_xray_hole_count", "gcoreccd_generate_cloud", "gcoreccd_generate_xray_events",
            "gcoreccd_load_carriers_file", "gcoreccd_save_collected_file",
            "gcoreccd_set_farfield", "gcoreccd_farfield_stats",
-           "gcoreccd_set_shard", "gcoreccd_shard_message_bytes", "gcoreccd_shard_local", "gcoreccd_shard_commit",
+           "gcoreccd_set_shard", "gcoreccd_shard_message_bytes", "gcoreccd_shard_local", "gcoreccd_shard_commit", "gcoreccd_set_shard_wait",
            "gcoreccd_profile_step", "gcoreccd_set_persistent", "gcoreccd_kernel_launches", "gcoreccd_debug_normals", "gcoreccd_debug_microbench", "gcoreccd_strerror",
            "gcoreccd_last_error", "gcoreccd_version"]
 
@@ -115,6 +115,8 @@ def lib():
     L.gcoreccd_shard_local.argtypes = [vp, vp, C.c_uint64]
     L.gcoreccd_shard_commit.restype = C.c_int
     L.gcoreccd_shard_commit.argtypes = [vp, C.POINTER(vp), C.c_uint32, C.c_uint64]
+    L.gcoreccd_set_shard_wait.restype = C.c_int
+    L.gcoreccd_set_shard_wait.argtypes = [vp, C.c_int]
     L.gcoreccd_set_farfield.restype = C.c_int
     L.gcoreccd_set_farfield.argtypes = [vp, C.c_double, C.c_uint32, C.c_uint64]
     L.gcoreccd_farfield_stats.restype = C.c_int
@@ -427,6 +429,9 @@ class Gcoreccd:
     def shard_commit(self, msg_ptrs, msg_bytes):
         arr = (C.c_void_p * len(msg_ptrs))(*[int(p) for p in msg_ptrs])
         self._check(lib().gcoreccd_shard_commit(self._h, arr, len(msg_ptrs), int(msg_bytes)), "shard_commit")
+
+    def set_shard_wait(self, on=True):
+        self._check(lib().gcoreccd_set_shard_wait(self._h, int(bool(on))), "set_shard_wait")
 
     def profile_step(self):
         ms = (C.c_float * 4)()

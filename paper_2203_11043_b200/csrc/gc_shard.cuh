@@ -13,7 +13,8 @@
 // k_shard_compact fills it; k_shard_commit reads G of them through a table of G device pointers.  Those pointers
 // may be slices of a local all-gather receive buffer (NCCL plumbing) or peer-mapped buffers of the other ranks
 // (symmetric memory over NVLink: the gather is then fused into the commit's loads) — the kernel is the same.
-// No kernel waits on another rank: ordering between ranks is the collective's / the host barrier's job.
+// By default no kernel waits on another rank: ordering between ranks is the collective's / the host barrier's job.
+// With gcoreccd_set_shard_wait (peer-mapped messages) the commit kernel spins on the headers' `ready` words instead.
 #pragma once
 #include "gc_common.cuh"
 
@@ -28,7 +29,23 @@ struct ShardHeader {
   uint32_t n_before;     // n_active the step started from (must agree on all ranks)
   uint32_t rank;
   uint64_t step;         // index of the step that produced the message
+  unsigned long long ready;   // written LAST, release at system scope: (epoch << 32) | (uint32)(step + 1); see header_ready
 };
+
+// Flag synchronisation for peer-mapped messages (symmetric memory over NVLink): with `wait` set, k_shard_commit spins
+// on each header's `ready` word until it carries THIS step's value instead of relying on a host-enqueued barrier
+// between shard_local and shard_commit.  `epoch` changes at every reset / set_shard (all ranks call them in lockstep),
+// so a stale header of an earlier event in the same buffer can never match.  Two message buffers, alternated, are
+// enough: a rank overwrites buffer b at step s+2 only after committing step s+1, which needed every peer's message
+// of step s+1, which each peer wrote after ITS commit of step s, i.e. after reading buffer b.
+__device__ __forceinline__ unsigned long long header_ready(uint32_t epoch, uint64_t step) {
+  return ((unsigned long long)epoch << 32) | (unsigned long long)(uint32_t)(step + 1u);
+}
+__device__ __forceinline__ void header_wait(const char* msg, unsigned long long want) {
+  const unsigned long long* p = &reinterpret_cast<const ShardHeader*>(msg)->ready;
+  unsigned long long v;
+  do { asm volatile("ld.acquire.sys.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory"); } while (v != want);
+}
 
 struct ShardPtrs { const char* p[kShardMaxWorld]; };
 
@@ -39,7 +56,7 @@ __device__ __forceinline__ const float* msg_x(const char* m) { return reinterpre
 // Same ballot + scan as k_compact; the CTA that finishes last writes the header.  Grid = bs / 256 CTAs.
 __global__ void __launch_bounds__(kTPB)
 k_shard_compact(SoA B, Ctrl* __restrict__ ctrl, const uint32_t* __restrict__ tile_count, char* __restrict__ msg,
-                uint32_t bs, double z_well, uint32_t rank) {
+                uint32_t bs, double z_well, uint32_t rank, uint32_t epoch) {
   __shared__ uint32_t s_red[kTPB / 32];
   __shared__ uint32_t s_base, s_last;
   const uint32_t t0 = ctrl->plan.t0, nt = ctrl->plan.nt;
@@ -102,6 +119,8 @@ k_shard_compact(SoA B, Ctrl* __restrict__ ctrl, const uint32_t* __restrict__ til
     hd->step = ctrl->step;
     ctrl->blocks_done = 0;
     ctrl->n_next = 0;
+    __threadfence_system();                                  // payload (all CTAs', observed through the ticket) and header
+    asm volatile("st.release.sys.global.u64 [%0], %1;" ::"l"(&hd->ready), "l"(header_ready(epoch, ctrl->step)) : "memory");
   }
 }
 
@@ -111,12 +130,17 @@ k_shard_compact(SoA B, Ctrl* __restrict__ ctrl, const uint32_t* __restrict__ til
 // nt x n ordered pairs to the pair counter and plans the next step's share.  A header that disagrees on
 // (n_before, step) with this rank's own state means the ranks have diverged: sticky flag, reported as BAD_STATE.
 __global__ void __launch_bounds__(kTPB)
-k_shard_commit(ShardPtrs bufs, uint32_t world, uint32_t bs, SoA A, Ctrl* __restrict__ ctrl, PlanArgs pa) {
+k_shard_commit(ShardPtrs bufs, uint32_t world, uint32_t bs, SoA A, Ctrl* __restrict__ ctrl, PlanArgs pa, uint32_t wait,
+               uint32_t epoch) {
   __shared__ uint32_t s_base, s_count, s_last;
   const uint32_t tid = threadIdx.x;
   const uint32_t tiles_per = bs / kTPB;
   const uint32_t g = blockIdx.x / tiles_per, t = blockIdx.x - g * tiles_per;
   if (tid == 0) {
+    if (wait) {                                              // every message this CTA reads a count or carriers from
+      const unsigned long long want = header_ready(epoch, ctrl->step);
+      for (uint32_t k = 0; k <= g; ++k) header_wait(bufs.p[k], want);
+    }
     uint32_t base = 0;
     for (uint32_t k = 0; k < g; ++k) base += reinterpret_cast<const ShardHeader*>(bufs.p[k])->count;
     const ShardHeader* hd = reinterpret_cast<const ShardHeader*>(bufs.p[g]);
@@ -142,6 +166,10 @@ k_shard_commit(ShardPtrs bufs, uint32_t world, uint32_t bs, SoA A, Ctrl* __restr
   __syncthreads();
   if (s_last && tid < 32) {
     __threadfence();
+    if (wait) {
+      const unsigned long long want = header_ready(epoch, ctrl->step);
+      for (uint32_t r = g + 1; r < world; ++r) header_wait(bufs.p[r], want);   // (already seen up to g)
+    }
     uint32_t n_new = 0;
     for (uint32_t r = 0; r < world; ++r) n_new += reinterpret_cast<const ShardHeader*>(bufs.p[r])->count;
     const FieldPlan old = ctrl->plan;

@@ -122,6 +122,8 @@ struct gcoreccd {
   uint64_t persist_max;
   bool persist_on;                    // many-steps-per-launch path for small populations (gc_persist.cuh); test hook turns it off
   uint32_t shard_rank, shard_world;   // target sharding (gc_shard.cuh); world 1 = not sharded
+  uint32_t shard_epoch;               // changes at every reset / set_shard: tells this event's message headers from stale ones
+  bool shard_wait;                    // shard_commit spins on the message headers (peer-mapped messages, no host barrier)
   bool ff_on;                         // far-field approximation (gc_tree.cuh)
   float ff_theta;
   uint32_t ff_parts;                  // CTAs (= partial chunks) per group of 256 targets; 0 = all-pairs kernel in use
@@ -620,6 +622,7 @@ int gcoreccd_reset(gcoreccd_t* h) {
   GC_CUDA(h, cudaStreamSynchronize(h->stream));
   drop_graph(h);                                           // its grids were sized for the previous population
   clear_events(h);
+  h->shard_epoch += 1;
   h->n_loaded = 0;
   h->n_bound = 0;
   h->variant = -1;
@@ -891,7 +894,14 @@ int gcoreccd_set_shard(gcoreccd_t* h, uint32_t rank, uint32_t world) {
   if (h->n_loaded != 0 || h->evb.loaded) return fail(h, GCORECCD_ERR_STATE, "set_shard: only on an empty handle (reset first)");
   h->shard_rank = rank;
   h->shard_world = world;
+  h->shard_epoch += 1;
   h->variant = -1;
+  return GCORECCD_OK;
+}
+
+int gcoreccd_set_shard_wait(gcoreccd_t* h, int on) {
+  if (!h) return GCORECCD_ERR_INVALID;
+  h->shard_wait = on != 0;
   return GCORECCD_OK;
 }
 
@@ -921,7 +931,7 @@ int gcoreccd_shard_local(gcoreccd_t* h, void* msg_dev, uint64_t msg_bytes) {
   k_integrate<<<tiles, kTPB, 0, h->stream>>>(h->A, h->B, h->ctrl, h->Ep, (uint32_t)h->L.part_cap, h->sink,
                                              h->tile_count, h->dp);
   k_shard_compact<<<tiles, kTPB, 0, h->stream>>>(h->B, h->ctrl, h->tile_count, (char*)msg_dev, (uint32_t)bs,
-                                                 h->dp.z_well, h->shard_rank);
+                                                 h->dp.z_well, h->shard_rank, h->shard_epoch);
   h->launches += 2;
   GC_CUDA(h, cudaGetLastError());
   return GCORECCD_OK;
@@ -940,7 +950,8 @@ int gcoreccd_shard_commit(gcoreccd_t* h, const void* const* msgs_host, uint32_t 
   }
   DeviceGuard guard(h->device);
   const uint32_t tiles = (uint32_t)(bs / kTPB);
-  k_shard_commit<<<tiles * n_msgs, kTPB, 0, h->stream>>>(ptrs, n_msgs, (uint32_t)bs, h->A, h->ctrl, plan_args(h, h->variant));
+  k_shard_commit<<<tiles * n_msgs, kTPB, 0, h->stream>>>(ptrs, n_msgs, (uint32_t)bs, h->A, h->ctrl, plan_args(h, h->variant),
+                                                         h->shard_wait ? 1u : 0u, h->shard_epoch);
   h->launches += 1;
   GC_CUDA(h, cudaGetLastError());
   return GCORECCD_OK;

@@ -10,8 +10,10 @@ Exchanges (how the G messages reach a rank):
   DistExchange     torch.distributed.all_gather_into_tensor on the message bytes: NCCL over NVLink on GPUs, gloo in
                    the CPU tests (tests/test_sharded_gloo.py drives it with an oracle-backed engine).
   SymmMemExchange  the messages live in torch symmetric memory; shard_commit reads the PEERS' buffers directly, so
-                   the all-gather is fused into the commit kernel's loads over NVLink and the only collective left is
-                   a barrier.  Exercised at world size 1 only (tests, bench --exchange symm): this build's boxes have one GPU.
+                   the all-gather is fused into the commit kernel's loads over NVLink, and the kernel waits on the
+                   message headers itself (a release-ordered word per message): no collective and no barrier is
+                   left in a step.  Exercised at world size 1 only (tests, bench --exchange symm): this build's
+                   boxes have one GPU, and ranks that wait on one another must not share a GPU (B200_PROFILING.md).
   VirtualRanks     G handles on ONE device stepped one after the other on one stream, messages passed by pointer:
                    the same kernels and the same pointer-table commit as the multi-GPU path, with no kernel ever
                    waiting on another (B200_PROFILING.md: emulate ranks sequentially, never concurrently).
@@ -69,9 +71,12 @@ class SymmMemExchange:
         off = (self.k & 1) * self.max_bytes
         return self.buf[off: off + self.max_bytes]
 
+    flag_synchronised = True                  # ShardedEvent then switches the engine's commit kernel to header waits
+
     def gather(self, msg, nbytes):
+        """No collective and no barrier: shard_commit reads the peers' buffers and waits on their headers by itself
+        (include/gcoreccd.h gcoreccd_set_shard_wait); the host only hands it the G pointers."""
         off = (self.k & 1) * self.max_bytes
-        self.hdl.barrier()                    # every rank's message of this step is complete and visible
         ptrs = [int(p) + off for p in self.hdl.buffer_ptrs]
         self.k += 1
         return ptrs
@@ -97,7 +102,11 @@ class ShardedEvent:
         if self.nbytes > self.max_bytes:
             self.max_bytes = self.nbytes
             with self._on_engine_stream():   # buffers allocated by torch belong to the stream that uses them
+                if self.x is not None and getattr(self.x, "flag_synchronised", False):
+                    self.e._torch.cuda.synchronize()     # a larger symmetric buffer replaces one peers may still read
                 self.x = self._xf(self.max_bytes)
+                if getattr(self.x, "flag_synchronised", False):
+                    self.e.set_shard_wait(True)
                 if not hasattr(self.x, "message"):
                     self.msgs = [self._alloc(self.max_bytes), self._alloc(self.max_bytes)]
 

@@ -239,3 +239,29 @@ def test_snapshot_restart_at_steps_0_10_100_500_full_size(cfg, m):
     assert report[-1][1] < 0.75 * n_start                                    # the track really lost its front end by step 500
     print("cfg%d restart windows (step, n_active, worst |dr| um, worst field err): %s" % (cfg, report))
     sim.close()
+
+
+def test_four_million_holes_load_field_and_step():
+    """Capacity (include/gcoreccd.h GCORECCD_MAX_CARRIERS: "tested up to 4,194,304 holes"): the load path (validate,
+    unpack, look-back compaction over 16,384 tiles), one field evaluation and one whole step at 4x config 4, checked on
+    sampled carriers against the oracle, plus conservation, stable order and the workspace size the header promises."""
+    from paper_2203_11043_b200 import binding
+    n = 4 * 1048576
+    w = workloads.make(4, n=n)
+    assert len(w["xyz"]) == n
+    assert binding.workspace_size(n, 256, 256) < 260 * n                      # 32 B state + 192 B partials + 16 B records (+ image)
+    rng = np.random.default_rng(4)
+    sim = gpu_sim(w)
+    sim.load_carriers(w["xyz"])
+    st = sim.state()
+    assert st["n_loaded"] == n and st["n_active"] + st["n_collected"] == n
+    worst, worst_field, mism = _restart_window(sim, w, rng, 64, 1)
+    assert worst <= 2e-4 and worst_field <= 1e-4 and mism <= 1, (worst, worst_field, mism)
+    st1 = sim.state()
+    assert st1["step"] == 1 and st1["pair_interactions"] == st["n_active"] ** 2
+    xyz, ids = sim.read_carriers()
+    assert len(ids) == st1["n_active"] and np.all(np.diff(ids.astype(np.int64)) > 0)
+    img, over = sim.read_image()
+    assert int(img.sum()) + over + st1["n_active"] == n
+    print("4,194,304 holes: n_active %d -> %d, worst |dr| %.2e um, worst field err %.2e" % (st["n_active"], st1["n_active"], worst, worst_field))
+    sim.close()

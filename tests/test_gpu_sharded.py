@@ -63,6 +63,7 @@ def test_one_rank_shard_equals_the_unsharded_path_bit_for_bit():
     vr.load_carriers(w["xyz"])
     vr.step(12)
     ref = binding.from_workload(w)
+    ref.set_persistent(False)              # the two-launch path: same kernels and the same FP64 summation order as a shard
     ref.load_carriers(w["xyz"])
     ref.step(12)
     a, b = es[0].read_carriers(), ref.read_carriers()
@@ -257,3 +258,29 @@ def test_full_size_sharded_step_against_sampled_oracle():
     tot = vr.totals()
     assert tot["n_active"] + tot["n_collected"] == tot["n_loaded"] == len(w["xyz"])
     _close(es)
+
+
+def test_header_flag_synchronisation_equals_the_barrier_path():
+    """gcoreccd_set_shard_wait: the commit kernel waits on each message's `ready` word (epoch, step) instead of a host
+    barrier.  On one GPU the messages of a step are complete before the commit is enqueued (same stream), so the wait
+    falls through at once — what is checked here is the header protocol: the word written by shard_local matches what
+    shard_commit expects at every step, across a reset (new epoch, same buffers, stale headers of the first event in
+    them), and the result is bit-identical to the path without it."""
+    w = workloads.make(3, n=9000)
+    out = []
+    for wait in (False, True):
+        vr, es = _virtual(w, 3)
+        for e in es:
+            e.set_shard_wait(wait)
+        vr.load_carriers(w["xyz"])
+        vr.step(7)
+        for e in es:
+            e.reset()
+        vr.load_carriers(w["xyz"][:6000])                   # second event in the same message buffers
+        vr.step(9)
+        out.append((es[2].read_carriers(), vr.image(), vr.totals()))
+        _close(es)
+    (xa, ia), (xb, ib) = out[0][0], out[1][0]
+    assert np.array_equal(ia, ib) and np.array_equal(xa, xb)
+    assert np.array_equal(out[0][1], out[1][1]) and out[0][2] == out[1][2]
+    assert out[1][2]["step"] == 9 and out[1][2]["n_active"] < 6000

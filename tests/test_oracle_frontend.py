@@ -1,6 +1,7 @@
 """Pins for the oracle's X-ray front end: hole count N = E_e / w and the seeded Gaussian cloud.
-The generator is pinned by (a) the Philox known-answer path it shares with the pinned normal stream, re-derived
-here from the raw Philox words with the counter layout stated in DESIGN.md, (b) sample moments against N(c, sigma^2),
+The generator is pinned by (a) three holes computed without any oracle code (tests/golden/xray_cloud.txt, written by a
+pure-Python restatement of the definition whose Philox is pinned by the published vectors), (b) sample moments against
+N(c, sigma^2),
 (c) structural properties: index-addressed (chunked generation = one call), mirrored at the back surface."""
 import math
 
@@ -18,20 +19,18 @@ def test_hole_count_paper_values():
     assert g.xray_hole_count(-1.0) == 0 and g.xray_hole_count(10.0, 0.0) == 0
 
 
-def test_cloud_matches_box_muller_of_raw_words():
-    seed, c, s = 0x1234567890ABCDEF, (3.0, -7.0, 200.0), 0.8
-    xyz = g.xray_cloud(seed, 5, c, s, first_index=(1 << 32) + 9)
-    for i in range(5):
-        k = (1 << 32) + 9 + i
-        w = g.philox4x32_10([k & 0xffffffff, 0x58524159, k >> 32, 0], [seed & 0xffffffff, seed >> 32])
-        ua = ((int(w[0]) >> 9) + 0.5) / 2 ** 23
-        fa = (int(w[1]) >> 8) / 2 ** 24
-        ub = ((int(w[2]) >> 9) + 0.5) / 2 ** 23
-        fb = (int(w[3]) >> 8) / 2 ** 24
-        Ra, Rb = math.sqrt(-2 * math.log(ua)), math.sqrt(-2 * math.log(ub))
-        ref = np.array([c[0] + s * Ra * math.cos(2 * math.pi * fa), c[1] + s * Ra * math.sin(2 * math.pi * fa),
-                        c[2] + s * Rb * math.cos(2 * math.pi * fb)]).astype(np.float32)
-        assert np.array_equal(xyz[i], ref)
+def test_cloud_matches_three_holes_computed_without_the_oracle(golden):
+    # tests/golden/xray_cloud.txt: written by tests/golden/make_xray_cloud_golden.py, a pure-Python restatement of the
+    # definition (its Philox round function is itself pinned by the published known-answer vectors)
+    rows = golden("xray_cloud.txt")
+    assert len(rows) == 3
+    for r in rows:
+        seed, k, c, s = int(r[0]), int(r[1]), [float(v) for v in r[2:5]], float(r[5])
+        words, ref = [int(v, 16) for v in r[6:10]], np.array([float(v) for v in r[10:13]], dtype=np.float32)
+        assert g.philox4x32_10([k & 0xffffffff, 0x58524159, k >> 32, 0], [seed & 0xffffffff, seed >> 32]) == words
+        got = g.xray_cloud(seed, 1, c, s, first_index=k)[0]
+        # libm's log / cos may differ from Python's in the last FP64 bit: at most one FP32 ulp after rounding
+        assert np.all(np.abs(got.astype(np.float64) - ref) <= np.spacing(np.abs(ref)).astype(np.float64)), (got, ref)
 
 
 def test_cloud_moments():
