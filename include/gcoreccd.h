@@ -286,6 +286,15 @@ uint64_t gcoreccd_kernel_launches(gcoreccd_t* h);
 int gcoreccd_debug_normals(gcoreccd_t* h, const uint32_t* id_host, const uint64_t* step_host, uint64_t n,
                            double* n_xyz_host, uint32_t* words_host);
 
+/* Hole mobility of eq. 2 at n field magnitudes E (V/cm, host pointers) as the kernels evaluate it — piecewise
+ * degree-8 interpolants of (1 + (E/Ec)^beta)^(-1/beta) tabulated at create, relative error < 1e-15 — and by the direct
+ * exp/log form (test hook for a3; cm^2 / (V s)). */
+int gcoreccd_debug_mobility(gcoreccd_t* h, const double* E_host, uint64_t n, double* mu_table_host, double* mu_direct_host);
+
+/* The same table built and evaluated ON THE HOST (no GPU needed) for temperature T_K: lets the CPU test suite check the
+ * interpolants against an independent evaluation of eq. 2. */
+int gcoreccd_mobility_table_host(double T_K, const double* E_host, uint64_t n, double* mu_host);
+
 /* Instruction-throughput probe (no handle; current device): runs `iters` x 32 instructions of one kind on one SM with
  * `warps_per_subpartition` (1..4) warps per SM sub-partition and returns the cycles per warp-instruction per
  * sub-partition.  Kinds: 0 FFMA2 three distinct operands, 1 FFMA2 a*a+c, 2 FFMA2 one operand shared by consecutive

@@ -24,7 +24,7 @@ EXPORTS = ["gcoreccd_workspace_size", "gcoreccd_create", "gcoreccd_destroy", "gc
            "gcoreccd_load_carriers_file", "gcoreccd_save_collected_file",
            "gcoreccd_set_farfield", "gcoreccd_farfield_stats",
            "gcoreccd_set_shard", "gcoreccd_shard_message_bytes", "gcoreccd_shard_local", "gcoreccd_shard_commit", "gcoreccd_set_shard_wait",
-           "gcoreccd_profile_step", "gcoreccd_set_persistent", "gcoreccd_kernel_launches", "gcoreccd_debug_normals", "gcoreccd_debug_microbench", "gcoreccd_strerror",
+           "gcoreccd_profile_step", "gcoreccd_set_persistent", "gcoreccd_kernel_launches", "gcoreccd_debug_normals", "gcoreccd_debug_mobility", "gcoreccd_mobility_table_host", "gcoreccd_debug_microbench", "gcoreccd_strerror",
            "gcoreccd_last_error", "gcoreccd_version"]
 
 
@@ -129,6 +129,10 @@ def lib():
     L.gcoreccd_kernel_launches.argtypes = [vp]
     L.gcoreccd_debug_normals.restype = C.c_int
     L.gcoreccd_debug_normals.argtypes = [vp, u32p, u64p, C.c_uint64, C.POINTER(C.c_double), u32p]
+    L.gcoreccd_debug_mobility.restype = C.c_int
+    L.gcoreccd_debug_mobility.argtypes = [vp, C.POINTER(C.c_double), C.c_uint64, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    L.gcoreccd_mobility_table_host.restype = C.c_int
+    L.gcoreccd_mobility_table_host.argtypes = [C.c_double, C.POINTER(C.c_double), C.c_uint64, C.POINTER(C.c_double)]
     L.gcoreccd_debug_microbench.restype = C.c_int
     L.gcoreccd_debug_microbench.argtypes = [C.c_int, C.c_uint32, C.c_uint32, C.POINTER(C.c_double)]
     L.gcoreccd_strerror.restype = C.c_char_p
@@ -164,6 +168,17 @@ def microbench(kind, iters=4096, warps_per_subpartition=2):
     if rc != OK:
         raise GcoreccdError(rc, "gcoreccd_debug_microbench")
     return float(out.value)
+
+
+def mobility_table_host(T_K, E):
+    """eq. 2 through the kernels' interpolation table, built and evaluated on the host (no GPU)."""
+    e = np.ascontiguousarray(E, dtype=np.float64)
+    out = np.zeros_like(e)
+    dp = C.POINTER(C.c_double)
+    rc = lib().gcoreccd_mobility_table_host(float(T_K), e.ctypes.data_as(dp), e.size, out.ctypes.data_as(dp))
+    if rc != OK:
+        raise GcoreccdError(rc, "gcoreccd_mobility_table_host")
+    return out
 
 
 def workspace_size(max_carriers, img_nx, img_ny):
@@ -454,6 +469,15 @@ class Gcoreccd:
                                           out.ctypes.data_as(C.POINTER(C.c_double)), w.ctypes.data_as(C.POINTER(C.c_uint32)))
         self._check(rc, "gcoreccd_debug_normals")
         return out, w
+
+    def debug_mobility(self, E):
+        """(mu by the kernels' table, mu by the direct exp/log form) at field magnitudes E (V/cm)."""
+        e = np.ascontiguousarray(E, dtype=np.float64)
+        a, b = np.zeros_like(e), np.zeros_like(e)
+        dp = C.POINTER(C.c_double)
+        self._check(lib().gcoreccd_debug_mobility(self._h, e.ctypes.data_as(dp), e.size, a.ctypes.data_as(dp), b.ctypes.data_as(dp)),
+                    "gcoreccd_debug_mobility")
+        return a, b
 
     def synchronize(self):
         self._stream.synchronize()

@@ -63,6 +63,7 @@ struct DevParams {            // constants uploaded by value with every launch
   double a1_um;               // a1 * 1e-4  (V/cm per um)
   double a2;
   double mu0, inv_Ec, beta, inv_beta;   // eq. 2 with the T terms folded on the host
+  const double* mu_tab;       // eq. 2 as piecewise degree-8 interpolants of (1 + r^beta)^(-1/beta), r = E/Ec (gc_integrate.cuh)
   double drift_k;             // 1e-5 * dt
   double sigma_k;             // 2 * 0.1 * (k_B T / q) * dt
   double thickness, z_well;
@@ -73,6 +74,11 @@ struct DevParams {            // constants uploaded by value with every launch
   uint32_t seed_lo, seed_hi;
   int32_t nx, ny;
 };
+
+// eq. 2 table (gc_integrate.cuh mobility): binades 2^kMuEmin <= r < 2^kMuEmax of r = E/Ec, 16 sub-intervals each,
+// 9 monomial coefficients per sub-interval
+constexpr int kMuEmin = -16, kMuEmax = 16, kMuSub = 16, kMuDeg = 8;
+constexpr int kMuTabEntries = (kMuEmax - kMuEmin) * kMuSub * (kMuDeg + 1);
 
 struct Sink {                 // where a collected hole goes (a7)
   uint32_t* image;            // [ny][nx] integer pixel histogram

@@ -54,13 +54,34 @@ __device__ __forceinline__ void philox_normals(uint32_t seed_lo, uint32_t seed_h
   if (words) *words = w;
 }
 
-// eq. 2 with the temperature terms folded on the host: mu = mu0 / (1 + (E/Ec)^beta)^(1/beta), evaluated as
-// mu0 exp(-log1p(exp(beta log(E/Ec))) / beta): relative error ~1e-15 (FP64 log/exp), ten orders below what the
-// FP32 state can resolve, at a third of the dependent-instruction chain of two pow() calls (the per-carrier
-// chain is what bounds a small event's step, gc_events.cuh).  E = 0 gives log = -inf, exp = 0, mu = mu0.
-__device__ __forceinline__ double mobility(double E, const DevParams& P) {
-  const double t = exp(P.beta * log(E * P.inv_Ec));
+// eq. 2 with the temperature terms folded on the host: mu = mu0 f(r), f(r) = (1 + r^beta)^(-1/beta), r = E/Ec.
+//
+// Direct evaluation is mu0 exp(-log1p(exp(beta log r)) / beta): four FP64 transcendentals in series, ~2,400 cycles of
+// dependent instructions on a lone warp — the longest link of the per-carrier chain that bounds a small population's
+// step and a small event's step (gc_persist.cuh, gc_events.cuh).  f is analytic away from r = 0 and r^beta = -1, so on
+// a sixteenth of a binade it is reproduced to < 1e-19 relative by its degree-8 Chebyshev interpolant (nearest
+// singularity at 128 half-widths: error ~ 128^-9); gcoreccd_create tabulates those interpolants in long double for
+// 2^-16 <= r < 2^16 (E from 0.08 V/cm to 3e8 V/cm at 140 K) as monomial coefficients in u in [-1, 1].  Evaluation: exponent and
+// the top four mantissa bits select the row, u is exact, eight FMAs: ~150 cycles, rounding error ~2 ulp — the same
+// class as the four chained libm calls it replaces, ten orders below what the FP32 state resolves.  Outside the table
+// (r = 0, tiny, huge, NaN) the direct form runs.  mobility_direct is also what tests/ compare the table with.
+__device__ __forceinline__ double mobility_direct(double E, const DevParams& P) {
+  const double t = exp(P.beta * log(E * P.inv_Ec));          // E = 0: log = -inf, exp = 0, mu = mu0
   return P.mu0 * exp(-P.inv_beta * log1p(t));
+}
+__device__ __forceinline__ double mobility(double E, const DevParams& P) {
+  const double r = E * P.inv_Ec;
+  const long long bits = __double_as_longlong(r);
+  const int e = (int)((bits >> 52) & 0x7ff) - 1023;
+  if (e < kMuEmin || e >= kMuEmax || bits < 0) return mobility_direct(E, P);
+  const int j = (int)((bits >> 48) & 15);
+  const double m = __longlong_as_double((bits & 0x000fffffffffffffLL) | 0x3ff0000000000000LL);   // mantissa in [1, 2)
+  const double u = (m - (1.0 + ((double)j + 0.5) * (1.0 / kMuSub))) * (2.0 * kMuSub);         // exact, in [-1, 1)
+  const double* c = P.mu_tab + ((e - kMuEmin) * kMuSub + j) * (kMuDeg + 1);
+  double f = __ldg(c + kMuDeg);
+#pragma unroll
+  for (int k = kMuDeg - 1; k >= 0; --k) f = fma(f, u, __ldg(c + k));
+  return P.mu0 * f;
 }
 
 // a7: half-open pixel bins, floor, in FP64 on the stored FP32 position (exactly reproducible); the final position
@@ -269,6 +290,15 @@ k_set_snapshot(const float* __restrict__ xyz, const uint32_t* __restrict__ id, u
   const uint32_t i = blockIdx.x * kTPB + threadIdx.x;
   if (i >= n) return;
   A.x[i] = xyz[3 * (size_t)i]; A.y[i] = xyz[3 * (size_t)i + 1]; A.z[i] = xyz[3 * (size_t)i + 2]; A.id[i] = id[i];
+}
+
+// test hook: eq. 2 as the kernels evaluate it (table) and by the direct form
+__global__ void k_debug_mobility(const double* __restrict__ E, uint32_t n, DevParams P, double* __restrict__ mu_table,
+                                 double* __restrict__ mu_direct) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  mu_table[i] = mobility(E[i], P);
+  mu_direct[i] = mobility_direct(E[i], P);
 }
 
 __global__ void k_debug_normals(const uint32_t* __restrict__ id, const uint64_t* __restrict__ step, uint32_t n,

@@ -38,7 +38,7 @@ constexpr int kGraphSteps = 8;                        // steps per CUDA-graph la
 
 struct Layout {
   uint64_t cap_pad, part_cap, n_tiles, scan_entries, tree_scratch;
-  uint64_t off_ctrl, off_A, off_B, off_Ep, off_tiles, off_scan, off_image, off_fin, total;
+  uint64_t off_ctrl, off_A, off_B, off_Ep, off_tiles, off_scan, off_mutab, off_image, off_fin, total;
 };
 
 inline uint64_t align_up(uint64_t v, uint64_t a) { return (v + a - 1) / a * a; }
@@ -60,6 +60,7 @@ Layout make_layout(uint64_t max_carriers, int32_t nx, int32_t ny) {
   L.off_Ep = o;    o += align_up(3 * L.part_cap * 4, 256);
   L.off_tiles = o; o += align_up(L.n_tiles * 4, 256);
   L.off_scan = o;  o += align_up(L.scan_entries * 8, 256);
+  L.off_mutab = o; o += align_up((uint64_t)kMuTabEntries * 8, 256);      // eq. 2 interpolants (gc_integrate.cuh), 36 KB
   L.off_image = o; o += align_up((uint64_t)nx * (uint64_t)ny * 4, 256);
   L.off_fin = o;   o += align_up(L.cap_pad * 16, 256);
   L.total = o;
@@ -449,6 +450,43 @@ void free_events(gcoreccd_t* h) {
   memset(&h->evb, 0, sizeof(h->evb));
 }
 
+// eq. 2: degree-kMuDeg Chebyshev interpolants of f(r) = (1 + r^beta)^(-1/beta) on every sixteenth of a binade, in long
+// double, converted to monomial coefficients in u in [-1, 1] (gc_integrate.cuh mobility).  beta is the handle's double.
+void build_mobility_table(double beta, std::vector<double>& tab) {
+  constexpr int N = kMuDeg + 1;
+  const long double pi = 3.14159265358979323846264338327950288L;
+  const long double b = (long double)beta;
+  // monomial coefficients of the Chebyshev polynomials T_0 .. T_deg
+  long double T[N][N] = {};
+  T[0][0] = 1.0L;
+  if (N > 1) T[1][1] = 1.0L;
+  for (int n = 2; n < N; ++n)
+    for (int k = 0; k < N; ++k) T[n][k] = (k > 0 ? 2.0L * T[n - 1][k - 1] : 0.0L) - T[n - 2][k];
+  tab.assign(kMuTabEntries, 0.0);
+  for (int e = kMuEmin; e < kMuEmax; ++e) {
+    for (int j = 0; j < kMuSub; ++j) {
+      const long double mc = 1.0L + ((long double)j + 0.5L) / kMuSub, half = 0.5L / kMuSub;
+      long double fv[N], cheb[N];
+      for (int k = 0; k < N; ++k) {
+        const long double u = cosl(pi * ((long double)k + 0.5L) / N);
+        const long double r = ldexpl(mc + half * u, e);
+        fv[k] = powl(1.0L + powl(r, b), -1.0L / b);
+      }
+      for (int n = 0; n < N; ++n) {
+        long double acc = 0.0L;
+        for (int k = 0; k < N; ++k) acc += fv[k] * cosl(pi * (long double)n * ((long double)k + 0.5L) / N);
+        cheb[n] = acc * (n == 0 ? 1.0L : 2.0L) / N;
+      }
+      double* row = tab.data() + ((size_t)(e - kMuEmin) * kMuSub + j) * N;
+      for (int k = 0; k < N; ++k) {
+        long double mono = 0.0L;
+        for (int n = 0; n < N; ++n) mono += cheb[n] * T[n][k];
+        row[k] = (double)mono;
+      }
+    }
+  }
+}
+
 inline bool events_busy(const gcoreccd_t* h) { return h->evb.loaded && h->evb.carriers_left > 0; }
 
 }  // namespace
@@ -542,6 +580,14 @@ int gcoreccd_create(const gcoreccd_params* p, gcoreccd_t** out) {
   d.inv_Ec = 1.0 / (1.24 * std::pow(T, 1.68));
   d.beta = 0.46 * std::pow(T, 0.17);
   d.inv_beta = 1.0 / d.beta;
+  d.mu_tab = (const double*)(h->ws + h->L.off_mutab);
+  {
+    std::vector<double> tab;
+    build_mobility_table(d.beta, tab);
+    e = cudaMemcpyAsync(h->ws + h->L.off_mutab, tab.data(), tab.size() * 8, cudaMemcpyHostToDevice, h->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);             // `tab` leaves scope
+    if (e != cudaSuccess) { gcoreccd_destroy(h); return GCORECCD_ERR_CUDA; }
+  }
   d.drift_k = 1e-5 * p->dt_ns;
   d.sigma_k = 2.0 * 0.1 * (kB * T / q) * p->dt_ns;
   d.thickness = p->thickness_um;
@@ -991,6 +1037,50 @@ int gcoreccd_farfield_stats(gcoreccd_t* h, uint64_t* far_evals, uint64_t* near_e
 }
 
 uint64_t gcoreccd_kernel_launches(gcoreccd_t* h) { return h ? h->launches : 0; }
+
+int gcoreccd_mobility_table_host(double T_K, const double* E, uint64_t n, double* mu) {
+  if (!(T_K > 0) || !E || !mu) return GCORECCD_ERR_INVALID;
+  const double mu0 = 1.31e8 * std::pow(T_K, -2.2), inv_Ec = 1.0 / (1.24 * std::pow(T_K, 1.68)), beta = 0.46 * std::pow(T_K, 0.17);
+  std::vector<double> tab;
+  build_mobility_table(beta, tab);
+  for (uint64_t i = 0; i < n; ++i) {                         // the host twin of gc_integrate.cuh mobility()
+    const double r = E[i] * inv_Ec;
+    long long bits;
+    memcpy(&bits, &r, 8);
+    const int e = (int)((bits >> 52) & 0x7ff) - 1023;
+    if (e < kMuEmin || e >= kMuEmax || bits < 0) { mu[i] = mu0 * std::exp(-std::log1p(std::exp(beta * std::log(r))) / beta); continue; }
+    const int j = (int)((bits >> 48) & 15);
+    const long long mb = (bits & 0x000fffffffffffffLL) | 0x3ff0000000000000LL;
+    double m;
+    memcpy(&m, &mb, 8);
+    const double u = (m - (1.0 + ((double)j + 0.5) * (1.0 / kMuSub))) * (2.0 * kMuSub);
+    const double* c = tab.data() + ((size_t)(e - kMuEmin) * kMuSub + j) * (kMuDeg + 1);
+    double f = c[kMuDeg];
+    for (int k = kMuDeg - 1; k >= 0; --k) f = std::fma(f, u, c[k]);
+    mu[i] = mu0 * f;
+  }
+  return GCORECCD_OK;
+}
+
+int gcoreccd_debug_mobility(gcoreccd_t* h, const double* E, uint64_t n, double* mu_table, double* mu_direct) {
+  if (!h || !E || !mu_table || !mu_direct) return GCORECCD_ERR_INVALID;
+  if (n == 0) return GCORECCD_OK;
+  DeviceGuard guard(h->device);
+  double* buf = nullptr;
+  GC_CUDA(h, cudaMalloc((void**)&buf, n * 24));
+  cudaError_t e = cudaMemcpyAsync(buf, E, n * 8, cudaMemcpyHostToDevice, h->stream);
+  if (e == cudaSuccess) {
+    k_debug_mobility<<<(unsigned)((n + 255) / 256), 256, 0, h->stream>>>(buf, (uint32_t)n, h->dp, buf + n, buf + 2 * n);
+    h->launches += 1;
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess) e = cudaMemcpyAsync(mu_table, buf + n, n * 8, cudaMemcpyDeviceToHost, h->stream);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(mu_direct, buf + 2 * n, n * 8, cudaMemcpyDeviceToHost, h->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+  cudaFree(buf);
+  if (e != cudaSuccess) return fail(h, GCORECCD_ERR_CUDA, "debug_mobility", e);
+  return GCORECCD_OK;
+}
 
 int gcoreccd_debug_normals(gcoreccd_t* h, const uint32_t* id, const uint64_t* step, uint64_t n, double* out, uint32_t* words) {
   if (!h || !id || !step || !out || !words) return GCORECCD_ERR_INVALID;

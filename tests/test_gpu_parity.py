@@ -498,3 +498,19 @@ def test_persistent_kernel_runs_an_event_to_collection_and_stops_at_zero():
     assert abs(st["step"] - o.state()["step"]) <= 3
     assert st["pair_interactions"] == pytest.approx(o.state()["pair_interactions"], rel=0.02)
     s.close()
+
+
+def test_mobility_table_on_the_device_equals_the_host_table_and_the_direct_form():
+    # a3: the kernels evaluate eq. 2 through interpolants tabulated at create; the device must produce
+    # the host's bits (same table, same FMA Horner), and both agree with the direct exp/log form to double rounding
+    from paper_2203_11043_b200 import binding as b
+    for T in (140.0, 77.0):
+        w = workloads.make(0, n=8)
+        sim = gpu_sim(w, T_K=T)
+        rng = np.random.default_rng(5)
+        E = np.concatenate([np.logspace(-1, 8, 20001), rng.uniform(50.0, 5000.0, 20000), [0.0, 1e-30]])
+        tab, direct = sim.debug_mobility(E)
+        assert np.array_equal(tab, b.mobility_table_host(T, E))
+        ref = np.array([g.mobility(e, T) for e in E])
+        assert np.all(np.abs(tab - ref) <= 2e-15 * ref) and np.all(np.abs(direct - ref) <= 4e-15 * ref)
+        sim.close()
