@@ -4,8 +4,8 @@ peak; seconds per 131k-hole event").
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
 
-A "step" is one pass of the whole hot path (field + integrate/collect + compact = SURVEY §8(a) rows a1..a8)
-over the 131,072-hole cloud of BASELINE.json:configs[2].  Prints ONE JSON line (rank 0).
+A "step" is one pass of the whole hot path (k_field = a1, k_advance = a2..a8: update, collection, compaction; SURVEY
+§8(a) rows a1..a8) over the 131,072-hole cloud of BASELINE.json:configs[2].  Prints ONE JSON line (rank 0).
   value      pair interactions/s over the K timed steps, state resident in HBM, CUDA events on the launching
              stream, L2 flushed between timed steps (the state is only 2 MB; the path is ALU bound)
   e2e        same metric through the C ABI with HOST buffers: load_carriers(pinned host) + step(1) +
@@ -128,6 +128,13 @@ def oracle_sample(xyz, P, seconds_target, rng):
     return m * n / dt / 1e9, m, dt, g.num_threads()
 
 
+def config_dict(w, n, P):
+    """The same `config` for both arms (ours and --impl reference): the workload is what is compared."""
+    return {"workload": w["name"], "n_holes": n, "parallelism": "replicas only (one event per GPU)",
+            "l2": "flushed between timed steps (256 MB write); state is 2 MB, path is ALU bound",
+            "dt_ns": P["dt_ns"], "softening_um": P["softening_um"]}
+
+
 def image_sigma(img, P):
     """Standard deviations (um) of the collected image along x and y, from pixel centres."""
     im = np.asarray(img, dtype=np.float64)
@@ -162,7 +169,7 @@ def run_reference(args):
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": 1e3 * secs / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic", "impl": "reference",
-            "config": {"workload": w["name"], "n_holes": len(xyz), "sample": sample},
+            "config": config_dict(w, len(xyz), P),
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -176,7 +183,34 @@ def _peak_pairs(peaks):
     return SM_COUNT * LANES * 2.0 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / FLOP_PER_PAIR
 
 
-def leg_per_config(torch, binding, workloads, stream, peaks, sampler, configs=(0, 1, 2, 3, 4), reuse=None):
+def oracle_per_config(w, gpu_event):
+    """the oracle's rate on this config (eq. 6 at sampled targets x all sources, ~2 s) and its
+    seconds per event — run to completion for real on configs 0-1, extrapolated (the GPU run's sum of N_a^2 / the
+    oracle's rate) on configs 2-4."""
+    from oracle import goracle as g
+    P, xyz = w["params"], w["xyz"]
+    gps, m, dt, cores = oracle_sample(xyz, P, 2.0, np.random.default_rng(1))
+    rec = {"G_pairs_per_s": gps, "cores": cores, "kind": "oracle (FP64)",
+           "sample": "eq. 6 at %d sampled targets x all %d sources, %.1f s" % (m, len(xyz), dt)}
+    if w["config"] <= 1:
+        prm = g.make_params(T_K=P["T_K"], a1=P["a1"], a2=P["a2"], thickness_um=P["thickness_um"], z_well_um=P["z_well_um"],
+                            pixel_pitch_um=P["pixel_pitch_um"], dt_ns=P["dt_ns"], softening_um=P["softening_um"],
+                            eps_si=P["eps_si"], seed=P["seed"], img_nx=P["img_nx"], img_ny=P["img_ny"],
+                            img_x0_um=P["img_x0_um"], img_y0_um=P["img_y0_um"], flags=g.FP32_STATE)
+        sim = g.Sim(prm)
+        t0 = time.perf_counter()
+        sim.load(xyz)
+        sim.run(10 ** 7)
+        rec["seconds_per_event"] = time.perf_counter() - t0
+        rec["seconds_per_event_kind"] = "measured (run to full collection, %d steps)" % sim.state()["step"]
+        sim.close()
+    else:
+        rec["seconds_per_event"] = gpu_event["pair_interactions"] / (gps * 1e9)
+        rec["seconds_per_event_kind"] = "extrapolated: the GPU run's sum of N_a^2 / the oracle's sampled rate"
+    return rec
+
+
+def leg_per_config(torch, binding, workloads, stream, peaks, sampler, configs=(0, 1, 2, 3, 4), reuse=None, with_oracle=False):
     """BASELINE.json configs 0-4 (north_star: "throughput on synthetic clouds and tracks ... as pair interactions/s, and
     as seconds per event"): per-step rate at step 0 (CUDA events around step(10) right after the load, best of 3) and
     seconds per event (wall clock: load_carriers from pinned host -> run_to_collection -> read_image; best of 3, cfg4
@@ -227,8 +261,10 @@ def leg_per_config(torch, binding, workloads, stream, peaks, sampler, configs=(0
                             "avg_frac_of_fp32_peak": st2["pair_interactions"] / ev_s / peak,
                             "collected_in_window": int(img.sum())}
         row["clocks"] = sampler.window(t_leg0, time.perf_counter())
-        out.append(row)
         sim.close()
+        if with_oracle:
+            row["oracle"] = oracle_per_config(w, row["event"])
+        out.append(row)
     return out
 
 
@@ -532,7 +568,8 @@ def run_ours(args):
     per_config = n_sweep = sharded_virtual = None
     if world == 1 and not args.no_event and not args.quick:
         per_config = leg_per_config(torch, binding, workloads, stream, peaks, sampler,
-                                    reuse={2: dict(event, avg_frac_of_fp32_peak=event["avg_G_pairs_per_s"] * 1e9 / _peak_pairs(peaks))})
+                                    reuse={2: dict(event, avg_frac_of_fp32_peak=event["avg_G_pairs_per_s"] * 1e9 / _peak_pairs(peaks))},
+                                    with_oracle=not args.no_cpu_baseline)
         t0 = time.perf_counter()
         n_sweep = {"rows": leg_n_sweep(torch, binding, workloads, stream, peaks, [2 ** k for k in range(10, 21)]),
                    "what": "cfg-2 geometry, us per step through gcoreccd_step (CUDA events, best of 3), Coulomb on / off"}
@@ -554,9 +591,7 @@ def run_ours(args):
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
-            "config": {"workload": w["name"], "n_holes": n, "parallelism": "replicas only (one event per GPU)",
-                       "l2": "flushed between timed steps (256 MB write); state is 2 MB, path is ALU bound",
-                       "dt_ns": P["dt_ns"], "softening_um": P["softening_um"]},
+            "config": config_dict(w, n, P),
             "frac_of_fp32_peak": value * 1e9 * FLOP_PER_PAIR / 1e12 / (peak_tf * world),
             "clocks": clocks, "gpu_launches": launches,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": n * 12, "d2h_bytes_per_step": n * 12,

@@ -302,7 +302,12 @@ int launch_persistent(gcoreccd_t* h, uint32_t n_steps) {
   unsigned long long* scan = h->scan; DevParams dp = h->dp; PlanArgs pa = plan_args(h, v);
   void* args[] = {&A, &B, &ctrl, &Ep, &pc, &sink, &scan, &dp, &pa, &n_steps};
   const void* fn = v == 4 ? (const void*)k_steps<4, 1> : v == 3 ? (const void*)k_steps<2, 2> : (const void*)k_steps<1, 2>;
-  GC_CUDA(h, cudaLaunchCooperativeKernel(fn, dim3((unsigned)h->grid_field[v]), dim3(kTPB), args, 0, h->stream));
+  const cudaError_t e = cudaLaunchCooperativeKernel(fn, dim3((unsigned)h->grid_field[v]), dim3(kTPB), args, 0, h->stream);
+  if (e == cudaErrorCooperativeLaunchTooLarge) {             // fewer SMs than the occupancy query promised (MPS, green contexts)
+    cudaGetLastError();
+    return 1;                                                // the caller falls back to the two-launch path, for good
+  }
+  if (e != cudaSuccess) return fail(h, GCORECCD_ERR_CUDA, "cudaLaunchCooperativeKernel", e);
   h->launches += 1;
   return 0;
 }
@@ -406,10 +411,15 @@ int enqueue_steps(gcoreccd_t* h, uint64_t n_steps) {
     while (n_steps > 0) {
       const uint32_t chunk = (uint32_t)std::min<uint64_t>(n_steps, 1u << 20);
       rc = launch_persistent(h, chunk);
+      if (rc == 1) break;
       if (rc) return rc;
       n_steps -= chunk;
     }
-    return 0;
+    if (n_steps == 0) return 0;
+    h->persist_on = false;                                   // not all CTAs fit on this device partition: two launches per step
+    h->variant = -1;
+    rc = ensure_variant(h);
+    if (rc) return rc;
   }
   // stream capture is not permitted on the legacy / per-thread default streams: plain launches there
   const bool stream_ok = h->stream != cudaStreamLegacy && h->stream != cudaStreamPerThread && h->stream != nullptr;
@@ -774,7 +784,9 @@ int gcoreccd_run_to_collection(gcoreccd_t* h, uint64_t max_steps, uint64_t* step
   int ret = GCORECCD_OK;
   while (h->h_ctrl->n_active > 0) {
     if (done >= max_steps) { ret = GCORECCD_MAX_STEPS; break; }
-    uint64_t batch = (h->dp.flags & GCORECCD_COULOMB_OFF) ? (1ull << 20) : 4 * kGraphSteps;
+    // Coulomb off, or a population small enough for the persistent kernel: the launch itself loops until nobody drifts
+    uint64_t batch = ((h->dp.flags & GCORECCD_COULOMB_OFF) || variant_persistent(pick_variant(h, h->n_bound))) ? (1ull << 20)
+                                                                                                            : 4 * kGraphSteps;
     if (batch > max_steps - done) batch = max_steps - done;
     rc = enqueue_steps(h, batch);
     if (rc) return rc;
