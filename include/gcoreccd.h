@@ -299,7 +299,9 @@ int gcoreccd_mobility_table_host(double T_K, const double* E_host, uint64_t n, d
  * `warps_per_subpartition` (1..4) warps per SM sub-partition and returns the cycles per warp-instruction per
  * sub-partition.  Kinds: 0 FFMA2 three distinct operands, 1 FFMA2 a*a+c, 2 FFMA2 one operand shared by consecutive
  * instructions, 3 FADD2, 4 FMUL2, 5 scalar FFMA three distinct, 6 scalar FFMA shared operand, 7 DFMA, 8 MUFU.RSQ,
- * 9 the 11 packed instructions + 2 MUFU of one eq. 6 interaction pair (per packed instruction).  The evidence behind
+ * 9 the 11 packed instructions + 2 MUFU of one eq. 6 interaction pair (per packed instruction), 10 F2F f64->f32,
+ * 11 F2F f32->f64, 12 DADD, 13 one eq. 6 interaction per lane on the FP64 pipe, 14-16 the FP32 mix on 8 packs with
+ * 1 / 2 / 4 FP64-pipe targets interleaved (cycles per round of 8 packs).  The evidence behind
  * DESIGN.md 6.1 / 6.8 (`python bench.py --microbench`); not on the hot path. */
 int gcoreccd_debug_microbench(int kind, uint32_t iters, uint32_t warps_per_subpartition, double* cycles_per_inst_host);
 

@@ -275,6 +275,7 @@ int goracle_load_state(goracle_t* s, const double* xyz, const uint32_t* id, uint
   }
   s->n_active = n;
   if (s->n_loaded < n) s->n_loaded = n;
+  if (n && s->n_loaded < (uint64_t)maxid + 1) s->n_loaded = (uint64_t)maxid + 1; /* records cover every id of the snapshot */
   s->step = step;
   return 0;
 }

@@ -158,7 +158,10 @@ def xray_hole_count(E_e_eV, w_eV=3.77):
 
 
 MICRO_KINDS = ["FFMA2 three distinct operands", "FFMA2 a*a+c", "FFMA2 shared operand", "FADD2", "FMUL2",
-               "FFMA scalar three distinct", "FFMA scalar shared operand", "DFMA", "MUFU.RSQ", "eq. 6 mix (per packed instruction)"]
+               "FFMA scalar three distinct", "FFMA scalar shared operand", "DFMA", "MUFU.RSQ", "eq. 6 mix (per packed instruction)",
+               "F2F f64->f32", "F2F f32->f64", "DADD", "eq. 6 on the FP64 pipe (per interaction)",
+               "eq. 6 mix, 8 packs + 1 FP64 target (per round)", "eq. 6 mix, 8 packs + 2 FP64 targets (per round)",
+               "eq. 6 mix, 8 packs + 4 FP64 targets (per round)"]
 
 
 def microbench(kind, iters=4096, warps_per_subpartition=2):

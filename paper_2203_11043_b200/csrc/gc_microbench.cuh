@@ -20,8 +20,34 @@ enum MicroKind {
   kMicroDfma = 7,           // FP64 pipe: the bound of k_advance
   kMicroRsqrt = 8,          // MUFU.RSQ
   kMicroFieldMix = 9,       // the 11 packed instructions + 2 MUFU of one eq. 6 interaction pair, from registers
-  kMicroKinds = 10
+  kMicroF2F64to32 = 10,     // cvt.rn.f32.f64: which pipe converts, and how fast (FP64-pipe offload experiment)
+  kMicroF2F32to64 = 11,     // cvt.f64.f32
+  kMicroDadd = 12,
+  kMicroField64 = 13,       // one eq. 6 interaction per lane on the FP64 pipe: 3 DADD + 3 DFMA + F2F + MUFU + 2 FMUL + F2F + 3 DFMA
+  kMicroFieldMixD1 = 14,    // eq. 6 mix on 8 packs (16 FP32 targets) + 1 FP64-pipe target per lane, interleaved
+  kMicroFieldMixD2 = 15,    // ... + 2 FP64-pipe targets
+  kMicroFieldMixD4 = 16,    // ... + 4 FP64-pipe targets
+  kMicroKinds = 17
 };
+
+// one source against one target on the FP64 pipe: differences, r^2 and the accumulates in FP64, w = r^-3 through the FP32
+// MUFU.RSQ (relative error 2e-7: the same w the FP32 path uses)
+__device__ __forceinline__ void interact64(const double sx, const double sy, const double sz, const double ntx, const double nty,
+                                           const double ntz, const double eps2, double& ax, double& ay, double& az) {
+  const double dx = sx + ntx, dy = sy + nty, dz = sz + ntz;
+  double r2 = fma(dx, dx, eps2);
+  r2 = fma(dy, dy, r2);
+  r2 = fma(dz, dz, r2);
+  float r2f, inv;
+  asm("cvt.rn.f32.f64 %0, %1;" : "=f"(r2f) : "d"(r2));
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(inv) : "f"(r2f));
+  const float wf = (inv * inv) * inv;
+  double w;
+  asm("cvt.f64.f32 %0, %1;" : "=d"(w) : "f"(wf));
+  ax = fma(dx, w, ax);
+  ay = fma(dy, w, ay);
+  az = fma(dz, w, az);
+}
 
 template <int KIND>
 __global__ void __launch_bounds__(512, 1) k_microbench(uint32_t iters, float seed, long long* cycles, float* sink) {
@@ -35,6 +61,7 @@ __global__ void __launch_bounds__(512, 1) k_microbench(uint32_t iters, float see
     da[k] = (double)a[k].x; db[k] = (double)b[k].x; dc[k] = (double)c[k].x;
   }
   const float2 sh = make_float2(seed, seed + 1.0f);
+  const double dsz = (double)seed * 0.75;
   __syncthreads();
   const long long t0 = clock64();
 #pragma unroll 1
@@ -52,6 +79,10 @@ __global__ void __launch_bounds__(512, 1) k_microbench(uint32_t iters, float see
         else if (KIND == kMicroFfmaScalarShared) { c[k].x = __fmaf_rn(sh.x, b[k].x, c[k].x); c[k].y = __fmaf_rn(sh.x, b[k].y, c[k].y); }
         else if (KIND == kMicroDfma) dc[k] = fma(da[k], db[k], dc[k]);
         else if (KIND == kMicroRsqrt) { float y; asm volatile("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(c[k].x)); c[k].x = y + 1.5f; }
+        else if (KIND == kMicroF2F64to32) { float y; asm volatile("cvt.rn.f32.f64 %0, %1;" : "=f"(y) : "d"(dc[k])); dc[k] = da[k]; c[k].x += y; }
+        else if (KIND == kMicroF2F32to64) { double y; asm volatile("cvt.f64.f32 %0, %1;" : "=d"(y) : "f"(c[k].x)); dc[k] = y; }
+        else if (KIND == kMicroDadd) dc[k] = da[k] + dc[k];
+        else if (KIND == kMicroField64) interact64((double)sh.x, (double)sh.y, db[k], da[k], db[(k + 1) & 7], da[(k + 3) & 7], 1e-6, dc[k], da[k], db[k]);
         else {                                      // one source against target pack k: eq. 6 as in gc_field.cuh interact<>
           const float2 dx = __fadd2_rn(sh, a[k]), dy = __fadd2_rn(sh, b[k]), dz = __fadd2_rn(make_float2(sh.y, sh.x), a[k]);
           float2 r2 = __ffma2_rn(dx, dx, make_float2(1e-6f, 1e-6f));
@@ -66,6 +97,11 @@ __global__ void __launch_bounds__(512, 1) k_microbench(uint32_t iters, float see
           c[k] = __ffma2_rn(dx, w, c[k]);
           a[k] = __ffma2_rn(dy, w, a[k]);
           b[k] = __ffma2_rn(dz, w, b[k]);
+          constexpr int ND = KIND == kMicroFieldMixD1 ? 1 : KIND == kMicroFieldMixD2 ? 2 : KIND == kMicroFieldMixD4 ? 4 : 0;
+          if (ND > 0 && (k % (8 / (ND > 0 ? ND : 1))) == 0) {
+            const int q = k / (8 / (ND > 0 ? ND : 1));
+            interact64((double)sh.x, (double)sh.y, dsz, da[q], db[q], da[q + 4], 1e-6, dc[q], dc[q + 4], db[q + 4]);
+          }
         }
       }
     }
@@ -73,7 +109,7 @@ __global__ void __launch_bounds__(512, 1) k_microbench(uint32_t iters, float see
   const long long t1 = clock64();
   float acc = 0.f;
 #pragma unroll
-  for (int k = 0; k < 8; ++k) acc += c[k].x + c[k].y + a[k].x + b[k].y + (float)dc[k];
+  for (int k = 0; k < 8; ++k) acc += c[k].x + c[k].y + a[k].x + b[k].y + (float)dc[k] + (float)da[k] + (float)db[k];
   if (acc == 123.456f) sink[0] = acc;                // keeps the chains alive
   if ((threadIdx.x & 31u) == 0) cycles[threadIdx.x >> 5] = t1 - t0;
 }
@@ -83,7 +119,8 @@ __global__ void __launch_bounds__(512, 1) k_microbench(uint32_t iters, float see
 inline double micro_inst_per_iter(int kind) {
   if (kind == kMicroFfmaScalarThree || kind == kMicroFfmaScalarShared) return 64.0;
   if (kind == kMicroFieldMix) return 32.0 * 11.0;    // reported per PACKED instruction; MUFU rides along
-  return 32.0;
+  if (kind >= kMicroFieldMixD1) return 4.0;          // reported per round of 8 packs (+ 1 / 2 / 4 FP64 targets) per lane
+  return 32.0;                                       // kMicroField64: per interaction (its 9 FP64 + 2 F2F + 3 FP32 ride along)
 }
 
 }  // namespace gc

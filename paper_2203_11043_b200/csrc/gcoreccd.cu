@@ -193,8 +193,8 @@ inline bool persist_eligible(const gcoreccd_t* h, uint64_t n) {
          !(h->ff_on && n >= h->ff_min_active) && h->grid_field[3] > 0 && h->grid_field[4] > 0;
 }
 
-inline int pick_variant(const gcoreccd_t* h, uint64_t n) {
-  if (persist_eligible(h, n)) return n >= 12288 ? 4 : n >= 3072 ? 3 : 5;
+inline int pick_variant(const gcoreccd_t* h, uint64_t n, bool allow_persistent = true) {
+  if (allow_persistent && persist_eligible(h, n)) return n >= 12288 ? 4 : n >= 3072 ? 3 : 5;
   if (n >= 12288) return 2;            // 8 targets/thread, 1 CTA/SM: highest FMA-pipe utilisation (76 %)
   if (n >= 3072) return 1;             // 4 targets/thread, 3 CTAs/SM: more row blocks for balance
   return 0;                            // 2 targets/thread, 4 CTAs/SM
@@ -976,7 +976,8 @@ int gcoreccd_shard_local(gcoreccd_t* h, void* msg_dev, uint64_t msg_bytes) {
   if ((uintptr_t)msg_dev & 15u) return fail(h, GCORECCD_ERR_INVALID, "shard_local: message buffer must be 16-byte aligned");
   DeviceGuard guard(h->device);
   // the share shrinks with n_active: pick the field variant from the share, not from the whole population
-  const int v = pick_variant(h, (h->n_bound + h->shard_world - 1) / h->shard_world);
+  // (a shard of a world of ONE must plan like the two-launch path it is made of, not like the persistent kernel)
+  const int v = pick_variant(h, (h->n_bound + h->shard_world - 1) / h->shard_world, false);
   const uint32_t parts = h->ff_on && h->n_bound >= h->ff_min_active ? pick_parts(h) : 0u;   // treecode walk of the share
   if (v != h->variant || parts != h->ff_parts) {
     h->variant = v;
@@ -1519,7 +1520,14 @@ int gcoreccd_debug_microbench(int kind, uint32_t iters, uint32_t warps_per_subpa
       case 6: k_microbench<6><<<1, threads>>>(iters, 1.0f, d_cyc, d_sink); break;
       case 7: k_microbench<7><<<1, threads>>>(iters, 1.0f, d_cyc, d_sink); break;
       case 8: k_microbench<8><<<1, threads>>>(iters, 1.0f, d_cyc, d_sink); break;
-      default: k_microbench<9><<<1, threads>>>(iters, 1.0f, d_cyc, d_sink); break;
+      case 9: k_microbench<9><<<1, threads>>>(iters, 1.0f, d_cyc, d_sink); break;
+      case 10: k_microbench<10><<<1, threads>>>(iters, 1.0f, d_cyc, d_sink); break;
+      case 11: k_microbench<11><<<1, threads>>>(iters, 1.0f, d_cyc, d_sink); break;
+      case 12: k_microbench<12><<<1, threads>>>(iters, 1.0f, d_cyc, d_sink); break;
+      case 13: k_microbench<13><<<1, threads>>>(iters, 1.0f, d_cyc, d_sink); break;
+      case 14: k_microbench<14><<<1, threads>>>(iters, 1.0f, d_cyc, d_sink); break;
+      case 15: k_microbench<15><<<1, threads>>>(iters, 1.0f, d_cyc, d_sink); break;
+      default: k_microbench<16><<<1, threads>>>(iters, 1.0f, d_cyc, d_sink); break;
     }
   }
   long long h_cyc[16];

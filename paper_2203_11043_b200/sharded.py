@@ -180,6 +180,9 @@ class VirtualRanks:
 
     def __init__(self, engines, alloc):
         self.es, self.G = list(engines), len(engines)
+        if len({e._stream.cuda_stream for e in self.es}) != 1:
+            # every rank's commit reads every other rank's message: stream order IS the synchronisation here
+            raise ValueError("VirtualRanks: all engines must be created on the same CUDA stream")
         for g, e in enumerate(self.es):
             e.set_shard(g, self.G)
         self._alloc, self.max_bytes, self.msgs, self.k, self.nbytes = alloc, 0, None, 0, 0

@@ -42,22 +42,60 @@ def run(cfg, n=None, out=None, log=sys.stderr):
                         softening_um=P["softening_um"], eps_si=P["eps_si"], seed=P["seed"],
                         img_nx=P["img_nx"], img_ny=P["img_ny"], img_x0_um=P["img_x0_um"],
                         img_y0_um=P["img_y0_um"], flags=g.FP32_STATE)
-    sim = g.Sim(prm)
-    sim.load(w["xyz"])
     n0 = len(w["xyz"])
-    decay = [(0, sim.state()["n_active"])]
+    # A run of hours is checkpointed every EVERY steps (carriers, ids, step and what has been collected so far) and
+    # resumes from the checkpoint if one is there: the oracle's restart is bit-exact (tests/test_oracle_step.py,
+    # "restart equivalence"), a resumed run equals an uninterrupted one.  Everything collected before the
+    # checkpoint is carried in `base`; the segment after it adds its own image, records and counters.
+    ckpt = (out or os.path.join(HERE, "full_run_cfg%d.txt" % cfg)) + ".ckpt.npz"
+    sim = g.Sim(prm)
+    base = dict(img=np.zeros((P["img_ny"], P["img_nx"]), dtype=np.uint64), fin=np.full((n0, 3), np.nan),
+                fstep=np.full(n0, np.iinfo(np.uint64).max, dtype=np.uint64), pairs=0, oow=0, wall=0.0)
+    if os.path.exists(ckpt):
+        c = np.load(ckpt)
+        assert int(c["n0"]) == n0 and int(c["cfg"]) == cfg
+        sim.load_state(c["xyz"].astype(np.float64), c["ids"], int(c["step"]))
+        base.update(img=c["img"], fin=c["fin"], fstep=c["fstep"], pairs=int(c["pairs"]), oow=int(c["oow"]),
+                    wall=float(c["wall"]))
+        decay = [tuple(int(v) for v in r) for r in c["decay"]]
+        print("resumed from %s at step %d, n_active %d" % (ckpt, int(c["step"]), len(c["ids"])), file=log, flush=True)
+    else:
+        sim.load(w["xyz"])
+        decay = [(0, sim.state()["n_active"])]
+
+    def merged():
+        st = sim.state()
+        img = base["img"] + sim.image().astype(np.uint64)
+        f, fs = sim.collected()
+        fin, fstep = base["fin"].copy(), base["fstep"].copy()
+        m = fs[:n0] != np.iinfo(np.uint64).max
+        fin[:len(m)][m] = f[:n0][m]
+        fstep[:len(m)][m] = fs[:n0][m]
+        return st, img, fin, fstep, base["pairs"] + st["pair_interactions"], base["oow"] + st["n_out_of_window"]
+
     t0 = time.time()
+    last_save = t0
     while sim.state()["n_active"] > 0:
         sim.step(EVERY)
         st = sim.state()
         decay.append((st["step"], st["n_active"]))
         print("cfg%d step %d n_active %d pairs %.4g  %.0f s" % (cfg, st["step"], st["n_active"],
-                                                               st["pair_interactions"], time.time() - t0),
+                                                               base["pairs"] + st["pair_interactions"],
+                                                               base["wall"] + time.time() - t0),
               file=log, flush=True)
-    st = sim.state()
-    img = sim.image()
-    fin, fstep = sim.collected()
-    assert int(img.sum()) + st["n_out_of_window"] == n0 and st["n_collected"] == n0
+        if time.time() - last_save > float(os.environ.get("GOLDEN_CKPT_S", "600")) and st["n_active"] > 0:
+            _, img, fin, fstep, pairs, oow = merged()
+            xyz, ids = sim.carriers()
+            assert np.array_equal(xyz, xyz.astype(np.float32).astype(np.float64))   # FP32-state mode
+            np.savez_compressed(ckpt + ".tmp.npz", cfg=cfg, n0=n0, xyz=xyz.astype(np.float32), ids=ids, step=st["step"],
+                                img=img, fin=fin, fstep=fstep, pairs=pairs, oow=oow,
+                                wall=base["wall"] + time.time() - t0, decay=np.array(decay, dtype=np.int64))
+            os.replace(ckpt + ".tmp.npz", ckpt)
+            last_save = time.time()
+    st, img, fin, fstep, pairs, oow = merged()
+    assert int(img.sum()) + oow == n0 and not np.isnan(fin).any()
+    st = dict(st, pair_interactions=pairs, n_out_of_window=oow)
+    t0 -= base["wall"]
     lines = []
     A = lines.append
     A("# Oracle full run, load -> full collection.  Written by tests/golden/make_full_run_goldens.py %d%s"
@@ -89,6 +127,8 @@ def run(cfg, n=None, out=None, log=sys.stderr):
     with open(out + ".tmp", "w") as f:
         f.write("\n".join(lines) + "\n")
     os.replace(out + ".tmp", out)
+    if os.path.exists(ckpt):
+        os.remove(ckpt)
     sim.close()
     return out
 

@@ -46,7 +46,7 @@ def test_all_pairs_steps_are_bit_reproducible(n, persist):
 
 def test_events_treecode_and_sharded_paths_are_bit_reproducible():
     import torch
-    from paper_2203_11043_b200 import sharded
+    from paper_2203_11043_b200 import binding, sharded
     sizes = [5, 26, 40, 100, 200, 400, 700, 1500, 0, 3000, 4096]
     we = workloads.make_events(sizes)
     runs = []
@@ -76,7 +76,8 @@ def test_events_treecode_and_sharded_paths_are_bit_reproducible():
     w = workloads.make(1, n=8 * 700)
     runs = []
     for _ in range(2):
-        es = [gpu_sim(w) for _ in range(3)]
+        stream = torch.cuda.Stream()                          # virtual ranks are ordered by ONE stream
+        es = [binding.from_workload(w, stream=stream) for _ in range(3)]
         vr = sharded.VirtualRanks(es, lambda nb: torch.empty(nb, dtype=torch.uint8, device="cuda"))
         vr.load_carriers(w["xyz"])
         vr.step(9)
