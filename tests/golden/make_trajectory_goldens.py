@@ -51,15 +51,27 @@ def run(cfg, log=sys.stderr):
                         img_nx=P["img_nx"], img_ny=P["img_ny"], img_x0_um=P["img_x0_um"],
                         img_y0_um=P["img_y0_um"], flags=g.FP32_STATE)
     sim = g.Sim(prm)
-    sim.load(w["xyz"])
     n0 = len(w["xyz"])
     rng = np.random.default_rng(1000 + cfg)
-    _, ids0 = sim.carriers()
-    pick = np.sort(rng.choice(ids0, size=min(2 * M, len(ids0)), replace=False))     # candidates; survivors are cut to M
-    closest = {int(i): np.inf for i in pick}
-    n_act = [sim.state()["n_active"]]
-    t0 = time.time()
-    for s in range(STEPS):
+    # cfg4 is ten steps of 1.1e12 pairs each: the run is checkpointed after every step and resumes from the checkpoint
+    # (the oracle's restart is bit-exact: tests/test_oracle_step.py "restart equivalence"; FP32-state mode)
+    ckpt = os.path.join(HERE, "traj10_cfg%d.txt.ckpt.npz" % cfg)
+    if os.path.exists(ckpt):
+        c = np.load(ckpt)
+        assert int(c["n0"]) == n0
+        sim.load_state(c["xyz"].astype(np.float64), c["ids"], int(c["step"]))
+        pick, n_act, s_done, wall = c["pick"], [int(v) for v in c["n_act"]], int(c["step"]), float(c["wall"])
+        closest = {int(i): float(v) for i, v in zip(pick, c["closest"])}
+        print("resumed from %s at step %d" % (ckpt, s_done), file=log, flush=True)
+    else:
+        sim.load(w["xyz"])
+        _, ids0 = sim.carriers()
+        pick = np.sort(rng.choice(ids0, size=min(2 * M, len(ids0)), replace=False))     # candidates; survivors are cut to M
+        closest = {int(i): np.inf for i in pick}
+        n_act = [sim.state()["n_active"]]
+        s_done, wall = 0, 0.0
+    t0 = time.time() - wall
+    for s in range(s_done, STEPS):
         xyz, ids = sim.carriers()
         rows = np.searchsorted(ids, pick)
         ok = (rows < len(ids))
@@ -70,6 +82,13 @@ def run(cfg, log=sys.stderr):
         sim.step(1)
         n_act.append(sim.state()["n_active"])
         print("cfg%d step %d n_active %d  %.0f s" % (cfg, s + 1, n_act[-1], time.time() - t0), file=log, flush=True)
+        if s + 1 < STEPS and time.time() - t0 > float(os.environ.get("GOLDEN_CKPT_S", "300")):
+            xyz, ids = sim.carriers()
+            assert np.array_equal(xyz, xyz.astype(np.float32).astype(np.float64))
+            np.savez_compressed(ckpt + ".tmp.npz", n0=n0, xyz=xyz.astype(np.float32), ids=ids, step=s + 1, pick=pick,
+                                closest=np.array([closest[int(i)] for i in pick]), n_act=np.array(n_act),
+                                wall=time.time() - t0)
+            os.replace(ckpt + ".tmp.npz", ckpt)
     xyz, ids = sim.carriers()
     alive = pick[np.isin(pick, ids)]
     retired = pick[~np.isin(pick, ids)]
@@ -93,6 +112,8 @@ def run(cfg, log=sys.stderr):
     with open(out + ".tmp", "w") as f:
         f.write("\n".join(lines) + "\n")
     os.replace(out + ".tmp", out)
+    if os.path.exists(ckpt):
+        os.remove(ckpt)
     sim.close()
     return out
 
