@@ -553,11 +553,40 @@ def run_ours(args):
             batched.append(best)
             bs.close()
 
+    def _line(sharded_rec, cpu, per_config, n_sweep, sharded_virtual):
+        return {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f32", "data": "synthetic",
+                "config": config_dict(w, n, P),
+                "frac_of_fp32_peak": value * 1e9 * FLOP_PER_PAIR / 1e12 / (peak_tf * world),
+                "clocks": clocks, "gpu_launches": launches,
+                "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": n * 12, "d2h_bytes_per_step": n * 12,
+                        "what": "reset + load_carriers(pinned host) + step(1) + read_carriers(host), wall clock"},
+                "roofline": roofline, "cpu_baseline": cpu, "seconds_per_event": event, "farfield_variant": farfield,
+                "batched_events": batched, "per_config": per_config, "n_sweep": n_sweep, "sharded_virtual": sharded_virtual,
+                "sharded": sharded_rec}
+
     # ---- ONE event sharded over the job's ranks (N > 1 only; strong scaling; not the headline, which is replicas)
+    # This leg has never run on more than one GPU (the build's boxes have one): it must not be able to take the headline
+    # with it.  A watchdog prints the line without it (rank 0) and ends the rank if the leg hangs; an exception on
+    # any rank is caught and reported the same way.
     sharded_rec = None
     if world > 1 and not args.no_event:
-        sharded_rec = leg_sharded_real(torch, dist, binding, workloads, sharded, replicas, stream, rank, world, 3,
-                                       max(8, args.steps), args.warmup, "nccl")
+        import threading
+
+        def _bail():
+            if rank == 0:
+                print(json.dumps(_line({"error": "the sharded leg did not finish within 300 s"}, None, None, None, None)), flush=True)
+            os._exit(0)
+        wd = threading.Timer(300.0, _bail)
+        wd.daemon = True
+        wd.start()
+        try:
+            sharded_rec = leg_sharded_real(torch, dist, binding, workloads, sharded, replicas, stream, rank, world, 3,
+                                           max(8, args.steps), args.warmup, "nccl")
+        except Exception as e:                                # noqa: BLE001 - reported in the line, never fatal
+            sharded_rec = {"error": repr(e)[:400]}
+        wd.cancel()
 
     if rank != 0:
         if world > 1:
@@ -588,17 +617,7 @@ def run_ours(args):
         cpu = {"value": gps, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": "eq. 6 double loop (FP64) at %d sampled targets x all %d sources, %.1f s" % (m, n, dt)}
 
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f32", "data": "synthetic",
-            "config": config_dict(w, n, P),
-            "frac_of_fp32_peak": value * 1e9 * FLOP_PER_PAIR / 1e12 / (peak_tf * world),
-            "clocks": clocks, "gpu_launches": launches,
-            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": n * 12, "d2h_bytes_per_step": n * 12,
-                    "what": "reset + load_carriers(pinned host) + step(1) + read_carriers(host), wall clock"},
-            "roofline": roofline, "cpu_baseline": cpu, "seconds_per_event": event, "farfield_variant": farfield,
-            "batched_events": batched, "per_config": per_config, "n_sweep": n_sweep, "sharded_virtual": sharded_virtual,
-            "sharded": sharded_rec}
+    line = _line(sharded_rec, cpu, per_config, n_sweep, sharded_virtual)
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

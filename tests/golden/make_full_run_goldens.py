@@ -1,7 +1,10 @@
-"""Writes tests/golden/full_run_cfg{1,2}.txt: whole events on the ORACLE, load -> full collection.
+"""Writes tests/golden/full_run_cfg{1,2,3}.txt and full_run_cfg4_n131072.txt: whole events on the ORACLE, load -> full collection.
 
     python tests/golden/make_full_run_goldens.py 1      # cfg1, 16,384 holes: ~4e11 pairs, minutes
-    python tests/golden/make_full_run_goldens.py 2      # cfg2, 131,072 holes: ~1e13 pairs, 1-2 h on 8 cores
+    python tests/golden/make_full_run_goldens.py 2      # cfg2, 131,072 holes: ~1e13 pairs, 3 h on 8 cores / 31 min on 16 fast ones
+    python tests/golden/make_full_run_goldens.py 3      # cfg3, 262,144-hole track: 1.1e13 pairs
+    python tests/golden/make_full_run_goldens.py 4 131072   # cfg4's mix of 4 tracks + 64 clouds at 1/8 of its holes
+                                                            # (full_run_cfg4_n131072.txt; full size is 1.8e14 pairs)
 
 Imports only oracle/ and the seeded input generator (workloads.py, which holds none of the method's
 arithmetic); nothing here ever touches the CUDA path, so every stored value is the oracle's.
@@ -47,7 +50,8 @@ def run(cfg, n=None, out=None, log=sys.stderr):
     # resumes from the checkpoint if one is there: the oracle's restart is bit-exact (tests/test_oracle_step.py,
     # "restart equivalence"), a resumed run equals an uninterrupted one.  Everything collected before the
     # checkpoint is carried in `base`; the segment after it adds its own image, records and counters.
-    ckpt = (out or os.path.join(HERE, "full_run_cfg%d.txt" % cfg)) + ".ckpt.npz"
+    out = out or os.path.join(HERE, "full_run_cfg%d%s.txt" % (cfg, "" if n is None else "_n%d" % n))
+    ckpt = out + ".ckpt.npz"
     sim = g.Sim(prm)
     base = dict(img=np.zeros((P["img_ny"], P["img_nx"]), dtype=np.uint64), fin=np.full((n0, 3), np.nan),
                 fstep=np.full(n0, np.iinfo(np.uint64).max, dtype=np.uint64), pairs=0, oow=0, wall=0.0)
@@ -123,7 +127,6 @@ def run(cfg, n=None, out=None, log=sys.stderr):
     iy, ix = np.nonzero(img)
     for a, b in zip(iy, ix):
         A("px %d %d %d" % (a, b, img[a, b]))
-    out = out or os.path.join(HERE, "full_run_cfg%d.txt" % cfg)
     with open(out + ".tmp", "w") as f:
         f.write("\n".join(lines) + "\n")
     os.replace(out + ".tmp", out)

@@ -43,13 +43,13 @@ def _parse_full_run(name):
     return G
 
 
-@pytest.mark.parametrize("cfg", [1, 2])
-def test_whole_event_against_the_oracle_full_run(cfg):
-    name = "full_run_cfg%d.txt" % cfg
+@pytest.mark.parametrize("cfg,n", [(1, None), (2, None), (3, None), (4, 131072)])
+def test_whole_event_against_the_oracle_full_run(cfg, n):
+    name = "full_run_cfg%d%s.txt" % (cfg, "" if n is None else "_n%d" % n)
     if not os.path.exists(os.path.join(GOLDEN, name)):
         pytest.skip("stored oracle result missing: run tests/golden/make_full_run_goldens.py %d" % cfg)
     G = _parse_full_run(name)
-    w = workloads.make(cfg)
+    w = workloads.make(cfg, n=n)
     n0 = len(w["xyz"])
     assert n0 == G["n_loaded"]
     sim = gpu_sim(w)
