@@ -268,7 +268,7 @@ def leg_per_config(torch, binding, workloads, stream, peaks, sampler, configs=(0
     return out
 
 
-def leg_n_sweep(torch, binding, workloads, stream, peaks, sizes):
+def leg_n_sweep(torch, binding, workloads, stream, peaks, sizes, persist_mode=1):
     """Per-step device time against N at the cfg-2 geometry, Coulomb on and off: the shape of the paper's Fig. 4
     experiment.  CUDA events around step(K) after a warm-up of 8 steps, best of 3."""
     peak = _peak_pairs(peaks)
@@ -278,6 +278,8 @@ def leg_n_sweep(torch, binding, workloads, stream, peaks, sizes):
         row = {"n": n}
         for name, flags in (("coulomb_on", 0), ("coulomb_off", binding.COULOMB_OFF)):
             sim = binding.from_workload(w, flags=flags, stream=stream)
+            if persist_mode != 1:
+                sim.set_persistent(persist_mode)           # 0: two launches per step; 2: CTA-tile persistent kernels only
             sim.load_carriers(w["xyz"])
             k = 16 if (flags or n <= 131072) else 4
             sim.step(8 if n <= 131072 else 2)
@@ -632,7 +634,8 @@ def run_sweep(args):
     peaks, _ = measured_peaks()
     stream = torch.cuda.Stream()
     torch.cuda.set_stream(stream)
-    for row in leg_n_sweep(torch, binding, workloads, stream, peaks, [int(t) for t in args.sweep.split(",")]):
+    for row in leg_n_sweep(torch, binding, workloads, stream, peaks, [int(t) for t in args.sweep.split(",")],
+                           persist_mode=args.persist_mode):
         print(json.dumps(row), flush=True)
     return 0
 
@@ -714,6 +717,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--microbench", action="store_true", help="instruction-throughput probes (DESIGN.md 6.1 / 6.8)")
     ap.add_argument("--quick", action="store_true", help="skip the per_config / n_sweep / sharded_virtual legs")
+    ap.add_argument("--persist-mode", type=int, default=1, choices=[0, 1, 2],
+                    help="with --sweep: 0 two launches per step, 2 persistent CTA-tile kernels only, 1 default")
     ap.add_argument("--sweep", default="", help="comma-separated hole counts: per-step time vs N (not the headline)")
     ap.add_argument("--sharded", default="", help="config number: one event sharded over the ranks (not the headline)")
     ap.add_argument("--virtual-ranks", type=int, default=8, help="with --sharded on ONE GPU: ranks emulated sequentially")

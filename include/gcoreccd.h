@@ -274,7 +274,11 @@ int gcoreccd_profile_step(gcoreccd_t* h, float ms_host[4]);
 /* Small populations (below ~1e3 charges "the GPU is subutilised"): while the handle's upper bound on
  * n_active is <= max_active, gcoreccd_step / run_to_collection run all their steps in ONE cooperative launch of a
  * persistent kernel (field -> grid barrier -> a2..a8 -> grid barrier per step) instead of two launches per step.
- * on = 0 turns that off (tuning / test hook); max_active = 0 keeps the default (24,576).  Same physics, same Philox
+ * Up to 32 targets per SM (2,368 / 4,736 holes on 148 SMs) a warp owns its 2 / 4 targets for the whole step and a
+ * step costs ONE grid barrier (gc_persist_warp.cuh); run_to_collection lets a launch end when the population has decayed
+ * into the range of a smaller variant and continues with that one.
+ * on = 0 turns the persistent path off, on = 2 keeps it but without the warp-owner kernels (tuning / test hooks);
+ * max_active = 0 keeps the default (24,576).  Same physics, same Philox
  * counters; the FP32 summation order of eq. 6 differs between the two paths, nothing else.  All-pairs, unsharded
  * handles only (otherwise ignored). */
 int gcoreccd_set_persistent(gcoreccd_t* h, int on, uint64_t max_active);

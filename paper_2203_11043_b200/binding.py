@@ -457,7 +457,8 @@ class Gcoreccd:
         return dict(field=float(ms[0]), advance=float(ms[1]), step=float(ms[3]))
 
     def set_persistent(self, on=True, max_active=0):
-        self._check(lib().gcoreccd_set_persistent(self._h, int(bool(on)), int(max_active)), "gcoreccd_set_persistent")
+        mode = on if (isinstance(on, int) and not isinstance(on, bool)) else int(bool(on))   # 2: the CTA-tile kernels only
+        self._check(lib().gcoreccd_set_persistent(self._h, int(mode), int(max_active)), "gcoreccd_set_persistent")
 
     def kernel_launches(self):
         return int(lib().gcoreccd_kernel_launches(self._h))

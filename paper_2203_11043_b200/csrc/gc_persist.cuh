@@ -141,7 +141,7 @@ __device__ __forceinline__ unsigned long long gtime() { unsigned long long t; as
 template <int NPACK, int MINB>
 __global__ void __launch_bounds__(kTPB, MINB)
 k_steps(SoA A, SoA B, Ctrl* ctrl, float* Ep, uint32_t part_cap, Sink sink, unsigned long long* status, DevParams P, PlanArgs pa,
-        uint32_t n_steps) {
+        uint32_t n_steps, uint32_t n_exit) {
   __shared__ float4 s_xy[2][kTPB];
   __shared__ float2 s_z[2][kTPB];
   __shared__ PersistShared sh;
@@ -168,7 +168,7 @@ k_steps(SoA A, SoA B, Ctrl* ctrl, float* Ep, uint32_t part_cap, Sink sink, unsig
     __syncthreads();
     const FieldPlan plan = s_plan;
     const uint32_t n = plan.n;
-    if (n == 0) break;                                       // uniform over the grid
+    if (n == 0 || n < n_exit) break;                         // uniform over the grid; n_exit: a smaller variant takes over
     const uint64_t step = s_step;
     const uint32_t stamp = scan_stamp(seq0 + k);
     // a2..a8 tile size: the smallest that gives every tile a CTA of its own (more threads per carrier = shorter chains)

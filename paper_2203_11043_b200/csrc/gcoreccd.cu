@@ -21,6 +21,7 @@
 #include "gc_frontend.cuh"
 #include "gc_integrate.cuh"
 #include "gc_microbench.cuh"
+#include "gc_persist_warp.cuh"
 #include "gc_persist.cuh"
 #include "gc_shard.cuh"
 #include "gc_tree.cuh"
@@ -32,8 +33,9 @@ namespace {
 constexpr uint64_t kMaxCarriers = GCORECCD_MAX_CARRIERS;
 constexpr uint64_t kPersistMaxDefault = 24576;          // populations up to this run many steps per launch (gc_persist.cuh)
 constexpr uint64_t kPersistMaxLimit = 37888;            // 148 CTAs x 256: beyond, the one-step kernels are as fast
-constexpr int kNumVariants = 6;                       // 0-2: one-step field kernels (2/4/8 targets per thread); 3-4: persistent
-                                                      // multi-step kernels (4/8 targets per thread), 5: 2 targets per thread on 96 SMs for < 3,072 holes, gc_persist.cuh
+constexpr int kNumVariants = 8;                       // 0-2: one-step field kernels (2/4/8 targets per thread); 3-4: persistent
+                                                      // multi-step kernels (4/8 targets per thread), 5: 2 targets per thread on 96 SMs for < 3,072 holes, gc_persist.cuh;
+                                                      // 6-7: a warp owns 2 / 4 targets for the whole step, one CTA per SM (gc_persist_warp.cuh)
 constexpr int kGraphSteps = 8;                        // steps per CUDA-graph launch
 
 struct Layout {
@@ -121,6 +123,8 @@ struct gcoreccd {
   uint32_t graph_cadence;             // re-sort cadence baked into a treecode graph
   cudaEvent_t ev[4];
   uint64_t persist_max;
+  int persist_mode;                   // 1: every persistent kernel; 2: the CTA-tile kernels (k_steps) only
+  bool persist_early_exit;            // set by run_to_collection around its launches
   bool persist_on;                    // many-steps-per-launch path for small populations (gc_persist.cuh); test hook turns it off
   uint32_t shard_rank, shard_world;   // target sharding (gc_shard.cuh); world 1 = not sharded
   uint32_t shard_epoch;               // changes at every reset / set_shard: tells this event's message headers from stale ones
@@ -183,7 +187,10 @@ int fail(gcoreccd_t* h, int code, const char* what, cudaError_t e = cudaSuccess)
     if (e__ != cudaSuccess) return fail((h), GCORECCD_ERR_CUDA, #call, e__);   \
   } while (0)
 
-inline int variant_npack(int v) { return (v == 0 || v == 5) ? 1 : (v == 1 || v == 3) ? 2 : 4; }
+inline int variant_npack(int v) { return (v == 0 || v == 5 || v == 6) ? 1 : (v == 1 || v == 3 || v == 7) ? 2 : 4; }
+inline bool variant_warp_owner(int v) { return v == 6 || v == 7; }
+// holes a warp-owner variant can take: 2 NP targets per warp, 8 warps per CTA, one round
+inline uint64_t warp_owner_cap(const gcoreccd_t* h, int v);
 inline uint32_t variant_ib(int v) { return (uint32_t)kTPB * 2u * (uint32_t)variant_npack(v); }   // targets per row block
 inline bool variant_persistent(int v) { return v >= 3; }
 
@@ -193,8 +200,20 @@ inline bool persist_eligible(const gcoreccd_t* h, uint64_t n) {
          !(h->ff_on && n >= h->ff_min_active) && h->grid_field[3] > 0 && h->grid_field[4] > 0;
 }
 
+inline uint64_t warp_owner_cap(const gcoreccd_t* h, int v) {
+  return (uint64_t)h->grid_field[v] * (uint64_t)(kTPB / 32) * 2u * (uint64_t)variant_npack(v);
+}
+
 inline int pick_variant(const gcoreccd_t* h, uint64_t n, bool allow_persistent = true) {
-  if (allow_persistent && persist_eligible(h, n)) return n >= 12288 ? 4 : n >= 3072 ? 3 : 5;
+  if (allow_persistent && persist_eligible(h, n)) {
+    if (h->persist_mode == 1) {                              // (mode 2: the CTA-tile kernels only, for A/B measurements)
+      for (int v = 6; v <= 7; ++v)
+        if (n <= warp_owner_cap(h, v)) return v;             // 2,368 / 4,736 holes on 148 SMs (8 targets per warp was
+                                                             // tried: 9 % ahead at 9,472 holes, 6 % behind at 8,192, where
+                                                             // 64 targets per CTA leave 20 SMs without work)
+    }
+    return n >= 12288 ? 4 : n >= 3072 ? 3 : 5;
+  }
   if (n >= 12288) return 2;            // 8 targets/thread, 1 CTA/SM: highest FMA-pipe utilisation (76 %)
   if (n >= 3072) return 1;             // 4 targets/thread, 3 CTAs/SM: more row blocks for balance
   return 0;                            // 2 targets/thread, 4 CTAs/SM
@@ -300,9 +319,27 @@ int launch_persistent(gcoreccd_t* h, uint32_t n_steps) {
   const int v = h->variant;
   SoA A = h->A; SoA B = h->B; Ctrl* ctrl = h->ctrl; float* Ep = h->Ep; uint32_t pc = (uint32_t)h->L.part_cap; Sink sink = h->sink;
   unsigned long long* scan = h->scan; DevParams dp = h->dp; PlanArgs pa = plan_args(h, v);
-  void* args[] = {&A, &B, &ctrl, &Ep, &pc, &sink, &scan, &dp, &pa, &n_steps};
-  const void* fn = v == 4 ? (const void*)k_steps<4, 1> : v == 3 ? (const void*)k_steps<2, 2> : (const void*)k_steps<1, 2>;
-  const cudaError_t e = cudaLaunchCooperativeKernel(fn, dim3((unsigned)h->grid_field[v]), dim3(kTPB), args, 0, h->stream);
+  // run_to_collection lets the launch end as soon as the population has decayed into the range of a smaller variant
+  // (it reads Ctrl after every launch anyway); gcoreccd_step must take exactly n_steps
+  uint32_t n_exit = 0;
+  if (h->persist_early_exit && h->persist_mode == 1) {
+    if (v == 7) n_exit = (uint32_t)warp_owner_cap(h, 6) + 1u;
+    else if (v == 3 || v == 4) n_exit = (uint32_t)warp_owner_cap(h, 7) + 1u;
+  }
+  cudaError_t e;
+  if (variant_warp_owner(v)) {
+    void* args[] = {&A, &B, &ctrl, &sink, &scan, &dp, &pa, &n_steps, &n_exit};
+    const void* fn = v == 6 ? (const void*)k_steps_warp<1> : (const void*)k_steps_warp<2>;
+    // one CTA per 16 NP targets of the host's bound (the population only shrinks inside a launch), one CTA per SM at
+    // most: a CTA that owns no target would only make the grid barrier slower
+    const uint64_t per_cta = (uint64_t)(kTPB / 32) * 2u * (uint64_t)variant_npack(v);
+    const unsigned grid = (unsigned)std::max<uint64_t>(1, std::min<uint64_t>((uint64_t)h->grid_field[v], (h->n_bound + per_cta - 1) / per_cta));
+    e = cudaLaunchCooperativeKernel(fn, dim3(grid), dim3(kTPB), args, kWsSmemBytes, h->stream);
+  } else {
+    void* args[] = {&A, &B, &ctrl, &Ep, &pc, &sink, &scan, &dp, &pa, &n_steps, &n_exit};
+    const void* fn = v == 4 ? (const void*)k_steps<4, 1> : v == 3 ? (const void*)k_steps<2, 2> : (const void*)k_steps<1, 2>;
+    e = cudaLaunchCooperativeKernel(fn, dim3((unsigned)h->grid_field[v]), dim3(kTPB), args, 0, h->stream);
+  }
   if (e == cudaErrorCooperativeLaunchTooLarge) {             // fewer SMs than the occupancy query promised (MPS, green contexts)
     cudaGetLastError();
     return 1;                                                // the caller falls back to the two-launch path, for good
@@ -536,6 +573,8 @@ int gcoreccd_create(const gcoreccd_params* p, gcoreccd_t** out) {
   h->variant = -1;
   h->shard_world = 1;
   h->persist_on = true;
+  h->persist_mode = 1;
+  h->persist_early_exit = false;
   h->persist_max = kPersistMaxDefault;
   DeviceGuard guard(dev);
 
@@ -612,13 +651,17 @@ int gcoreccd_create(const gcoreccd_params* p, gcoreccd_t** out) {
   d.nx = p->img_nx; d.ny = p->img_ny;
 
   // persistent grid of the field kernel: resident CTAs per SM x SM count
-  int occ[kNumVariants] = {0, 0, 0, 0, 0, 0};
+  int occ[kNumVariants] = {0, 0, 0, 0, 0, 0, 0, 0};
   e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[0], k_field<1, 256, 4>, kTPB, 0);
   if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[1], k_field<2, 256, 3>, kTPB, 0);
   if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[2], k_field<4, 256, 1>, kTPB, 0);
   if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[3], k_steps<2, 2>, kTPB, 0);
   if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[4], k_steps<4, 1>, kTPB, 0);
   if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[5], k_steps<1, 2>, kTPB, 0);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_steps_warp<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kWsSmemBytes);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_steps_warp<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kWsSmemBytes);
+  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[6], k_steps_warp<1>, kTPB, kWsSmemBytes);
+  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[7], k_steps_warp<2>, kTPB, kWsSmemBytes);
   if (e != cudaSuccess) { fail(h, GCORECCD_ERR_CUDA, "occupancy query", e); gcoreccd_destroy(h); return GCORECCD_ERR_CUDA; }
   for (int v = 0; v < 3; ++v) h->grid_field[v] = h->num_sms * (occ[v] > 0 ? occ[v] : 1);
   int coop = 0;
@@ -626,6 +669,7 @@ int gcoreccd_create(const gcoreccd_params* p, gcoreccd_t** out) {
   for (int v = 3; v < 5; ++v) h->grid_field[v] = coop ? h->num_sms * std::min(occ[v], v == 3 ? 2 : 1) : 0;   // 0: no persistent path
   // < 3,072 holes: 96 tiles of 32 carriers at most; every CTA that only waits at the grid barriers makes them slower
   h->grid_field[5] = coop && occ[5] > 0 ? std::min(h->num_sms, 96) : 0;
+  for (int v = 6; v <= 7; ++v) h->grid_field[v] = coop && occ[v] > 0 ? h->num_sms : 0;   // one CTA per SM; 0: pick_variant never returns it
   int occ_tree = 0;
   e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_tree, k_tree_field, kTreeTPB, 0);
   if (e != cudaSuccess) { fail(h, GCORECCD_ERR_CUDA, "occupancy query", e); gcoreccd_destroy(h); return GCORECCD_ERR_CUDA; }
@@ -788,7 +832,9 @@ int gcoreccd_run_to_collection(gcoreccd_t* h, uint64_t max_steps, uint64_t* step
     uint64_t batch = ((h->dp.flags & GCORECCD_COULOMB_OFF) || variant_persistent(pick_variant(h, h->n_bound))) ? (1ull << 20)
                                                                                                             : 4 * kGraphSteps;
     if (batch > max_steps - done) batch = max_steps - done;
+    h->persist_early_exit = true;
     rc = enqueue_steps(h, batch);
+    h->persist_early_exit = false;
     if (rc) return rc;
     rc = sync_ctrl(h);
     if (rc) return rc;
@@ -922,7 +968,9 @@ int gcoreccd_profile_step(gcoreccd_t* h, float ms[4]) {
 
 int gcoreccd_set_persistent(gcoreccd_t* h, int on, uint64_t max_active) {
   if (!h || max_active > kPersistMaxLimit) return GCORECCD_ERR_INVALID;
+  if (on < 0 || on > 2) return GCORECCD_ERR_INVALID;
   h->persist_on = on != 0;
+  h->persist_mode = on == 2 ? 2 : 1;
   h->persist_max = max_active ? max_active : kPersistMaxDefault;
   h->variant = -1;                                         // re-pick the kernel variant (and re-plan) at the next step
   return GCORECCD_OK;

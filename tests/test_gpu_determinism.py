@@ -29,7 +29,8 @@ def _same(a, b):
 
 
 @pytest.mark.parametrize("n,persist", [(700, False), (3500, False), (13000, False), (40000, False),
-                                       (300, True), (2500, True), (5000, True), (12500, True), (24000, True)])
+                                       (300, True), (2500, True), (5000, True), (12500, True), (24000, True),
+                                       (300, 2), (2500, 2), (5000, 2)])
 def test_all_pairs_steps_are_bit_reproducible(n, persist):
     w = workloads.make(3, n=n)                                                 # a track: retirements every step
     runs = []

@@ -71,12 +71,14 @@ def test_normal_stream_matches_oracle_bit_for_bit_in_the_words():
 
 
 # ------------------------------------------------------------------ a2..a8: 10-step trajectories
-def _trajectory_check(w, flags_gpu, flags_or, steps=10, tol=TRAJ_TOL, **over):
+def _trajectory_check(w, flags_gpu, flags_or, steps=10, tol=TRAJ_TOL, persist=None, **over):
     """GPU vs FP32-state oracle after `steps` steps from identical FP32 inputs.  Explicit Euler with eps = 1e-3 um
     is chaotic through close encounters (a pair at 0.01 um is thrown ~5 um apart in one step, so a 1-ulp
     difference in r becomes ~0.05 um): a carrier may exceed `tol` only if the ORACLE's trajectory shows a
     neighbour closer than 0.1 um inside the window (R21); everyone else must be within `tol`."""
     sim = gpu_sim(w, flags=flags_gpu, **over)
+    if persist is not None:
+        sim.set_persistent(persist)
     sim.load_carriers(w["xyz"])
     o = oracle_sim(w, flags=flags_or | g.FP32_STATE, **over)
     o.load(w["xyz"])
@@ -98,6 +100,20 @@ def _trajectory_check(w, flags_gpu, flags_or, steps=10, tol=TRAJ_TOL, **over):
 @pytest.mark.parametrize("cfg,n", [(0, 1024), (0, 777), (1, 16384), (3, 8192)])
 def test_trajectory_parity_10_steps_full_physics(cfg, n):
     _trajectory_check(workloads.make(cfg, n=n), 0, 0)
+
+
+@pytest.mark.parametrize("cfg,n", [(0, 1024), (1, 4096), (2, 4000), (3, 8192), (0, 300), (3, 2368), (3, 4737)])
+@pytest.mark.parametrize("persist", [0, 2])
+def test_trajectory_parity_10_steps_every_launch_scheme(cfg, n, persist):
+    """The default scheme at these sizes is the warp-owner persistent kernel (gc_persist_warp.cuh; the test above and the
+    two extra sizes here).  The other two — two launches per step (0) and the CTA-tile persistent kernel (2) — are held
+    to the same oracle comparison."""
+    _trajectory_check(workloads.make(cfg, n=n), 0, 0, persist=persist)
+
+
+@pytest.mark.parametrize("cfg,n", [(1, 4096), (2, 4000), (0, 300), (3, 2368), (3, 2369), (3, 4736), (0, 2), (0, 33)])
+def test_trajectory_parity_10_steps_warp_owner_kernels(cfg, n):
+    _trajectory_check(workloads.make(cfg, n=n), 0, 0, persist=1)
 
 
 def test_trajectory_parity_flag_combinations():
@@ -442,14 +458,20 @@ def test_snapshot_is_validated_and_keeps_the_count_invariant():
 
 
 # ------------------------------------------------------------------ many steps per launch (gc_persist.cuh)
-@pytest.mark.parametrize("cfg,n", [(0, 1024), (0, 37), (1, 4096), (1, 16384), (3, 20000), (0, 1), (0, 65), (2, 24576)])
-def test_persistent_multi_step_kernel_equals_the_two_launch_path(cfg, n):
+@pytest.mark.parametrize("cfg,n,mode", [(0, 1024, 1), (0, 37, 1), (1, 4096, 1), (1, 16384, 1), (3, 20000, 1), (0, 1, 1), (0, 65, 1),
+                                        (2, 24576, 1), (3, 2368, 1), (3, 2369, 1), (3, 4736, 1), (3, 4737, 1), (2, 8000, 1), (3, 9472, 1), (3, 9473, 1),
+                                        (0, 17, 1),
+                                        (0, 1024, 2), (0, 37, 2), (1, 4096, 2), (0, 1, 2), (0, 65, 2), (2, 8000, 2)])
+def test_persistent_multi_step_kernel_equals_the_two_launch_path(cfg, n, mode):
     """Small populations run K steps in one cooperative launch (field -> grid barrier -> a2..a8 -> grid barrier).  Same
     physics and Philox counters as the two-launch path; only the FP32/FP64 summation order of the chunk partials of
     eq. 6 differs, so after 12 steps positions agree far inside the trajectory tolerance and every integer agrees
-    except for retire decisions at the plane."""
+    except for retire decisions at the plane.  mode 1: every persistent kernel — up to 2,368 / 4,736 holes a warp owns its
+    2 / 4 targets for the whole step (gc_persist_warp.cuh; sizes on both sides of those limits); mode 2: the CTA-tile kernels
+    (gc_persist.cuh) at every size."""
     w = workloads.make(cfg, n=n)
     a, b = gpu_sim(w), gpu_sim(w)
+    a.set_persistent(mode)
     b.set_persistent(False)
     a.load_carriers(w["xyz"]); b.load_carriers(w["xyz"])
     la = a.kernel_launches()
@@ -468,8 +490,9 @@ def test_persistent_multi_step_kernel_equals_the_two_launch_path(cfg, n):
     a.close(); b.close()
 
 
-def test_persistent_kernel_is_bit_reproducible_and_independent_of_the_batching():
-    w = workloads.make(3, n=12000)                                             # a track: holes retire every step
+@pytest.mark.parametrize("n", [12000, 7000, 3000, 1500])                       # CTA-tile kernels, a warp owns 4 / 2 targets
+def test_persistent_kernel_is_bit_reproducible_and_independent_of_the_batching(n):
+    w = workloads.make(3, n=n)                                                 # a track: holes retire every step
     runs = []
     for chunks in ((40,), (1, 7, 32), (13, 27)):
         s = gpu_sim(w)
@@ -481,17 +504,26 @@ def test_persistent_kernel_is_bit_reproducible_and_independent_of_the_batching()
     for (x, i), st, img in runs[1:]:
         assert np.array_equal(i, runs[0][0][1]) and np.array_equal(x, runs[0][0][0])
         assert st == runs[0][1] and np.array_equal(img, runs[0][2])
-    assert runs[0][1]["n_active"] < 12000 and runs[0][1]["step"] == 40
+    assert runs[0][1]["n_active"] < n and runs[0][1]["step"] == 40
 
 
-def test_persistent_kernel_runs_an_event_to_collection_and_stops_at_zero():
-    w = workloads.make(0, n=2000)
+@pytest.mark.parametrize("n,how", [(2000, "step"), (2000, "run"), (11000, "run")])
+def test_persistent_kernel_runs_an_event_to_collection_and_stops_at_zero(n, how):
+    w = workloads.make(0, n=n)
     s = gpu_sim(w)
     s.load_carriers(w["xyz"])
-    s.step(100000)                                                             # one launch; the loop ends when nobody drifts
+    l0 = s.kernel_launches()
+    if how == "step":
+        s.step(100000)                                                         # one launch; the loop ends when nobody drifts
+    else:
+        # run_to_collection: a launch ends when the population has decayed into the range of a smaller variant
+        # (11,000 holes: CTA-tile kernel -> a warp owns 4 -> 2 targets), each of them one launch (+ a re-plan)
+        done, left, rc = s.run_to_collection(100000)
+        assert left == 0 and rc == 0
+    assert s.kernel_launches() - l0 <= 10
     st = s.state()
     img, over = s.read_image()
-    assert st["n_active"] == 0 and int(img.sum()) + over == 2000 and 100 < st["step"] < 200
+    assert st["n_active"] == 0 and int(img.sum()) + over == n and 100 < st["step"] < 200
     o = oracle_sim(w, flags=g.FP32_STATE)
     o.load(w["xyz"])
     o.run(100000)
