@@ -281,7 +281,9 @@ def leg_n_sweep(torch, binding, workloads, stream, peaks, sizes, persist_mode=1)
             if persist_mode != 1:
                 sim.set_persistent(persist_mode)           # 0: two launches per step; 2: CTA-tile persistent kernels only
             sim.load_carriers(w["xyz"])
-            k = 16 if (flags or n <= 131072) else 4
+            # steps per timed call: a small population runs them all in ONE persistent launch, whose launch and exit
+            # (~10 us) would otherwise be a visible share of 16 steps of 7-15 us; events run hundreds of steps per launch
+            k = 64 if (not flags and n <= 16384) else 16 if (flags or n <= 131072) else 4
             sim.step(8 if n <= 131072 else 2)
             torch.cuda.synchronize()
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
