@@ -40,10 +40,12 @@ def main():
         conserved(s, n)
         s.close()
         done.append("k_field/k_advance n=%d" % n)
-    # persistent multi-step kernels k_steps<1|2|4> (grid barriers, look-back and two-level scans, ping-pong state)
-    for n in (300, 2500, 5000, 12500):
+    # persistent multi-step kernels: k_steps_warp<1|2> (a warp owns its targets: shuffle butterfly, one grid barrier per
+    # step, normals drawn in the barrier wait) and k_steps<1|2|4> (grid barriers, two-level scans, ping-pong state)
+    for n, mode in ((300, 1), (2500, 1), (5000, 1), (12500, 1), (300, 2), (2500, 2)):
         w = workloads.make(3, n=n)
         s = binding.from_workload(w, stream=stream)
+        s.set_persistent(mode)
         s.load_carriers(w["xyz"])
         s.step(7)
         conserved(s, n)
