@@ -36,9 +36,6 @@ constexpr uint64_t kPersistMaxLimit = 37888;            // 148 CTAs x 256: beyon
 constexpr int kNumVariants = 8;                       // 0-2: one-step field kernels (2/4/8 targets per thread); 3-4: persistent
                                                       // multi-step kernels (4/8 targets per thread), 5: 2 targets per thread on 96 SMs for < 3,072 holes, gc_persist.cuh;
                                                       // 6-7: a warp owns 2 / 4 targets for the whole step, one CTA per SM (gc_persist_warp.cuh)
-constexpr int kWsSplit = 1;                           // warps sharing the sources of one target group in k_steps_warp; 2 measured
-                                                      // SLOWER (4,096 holes: 16.1 vs 14.7 us per step): the source loop is at its
-                                                      // operand-read floor with two warps per sub-partition already
 constexpr int kGraphSteps = 8;                        // steps per CUDA-graph launch
 
 struct Layout {
@@ -209,7 +206,7 @@ inline uint64_t warp_owner_cap(const gcoreccd_t* h, int v) {
 
 inline int pick_variant(const gcoreccd_t* h, uint64_t n, bool allow_persistent = true) {
   if (allow_persistent && persist_eligible(h, n)) {
-    if (h->persist_mode == 1) {                              // (mode 2: the CTA-tile kernels only, for A/B measurements)
+    if (h->persist_mode != 2) {                              // (mode 2: the CTA-tile kernels only, for A/B measurements)
       for (int v = 6; v <= 7; ++v)
         if (n <= warp_owner_cap(h, v)) return v;             // 2,368 / 4,736 holes on 148 SMs (8 targets per warp was
                                                              // tried: 9 % ahead at 9,472 holes, 6 % behind at 8,192, where
@@ -325,19 +322,19 @@ int launch_persistent(gcoreccd_t* h, uint32_t n_steps) {
   // run_to_collection lets the launch end as soon as the population has decayed into the range of a smaller variant
   // (it reads Ctrl after every launch anyway); gcoreccd_step must take exactly n_steps
   uint32_t n_exit = 0;
-  if (h->persist_early_exit && h->persist_mode == 1) {
+  if (h->persist_early_exit && h->persist_mode != 2) {
     if (v == 7) n_exit = (uint32_t)warp_owner_cap(h, 6) + 1u;
     else if (v == 3 || v == 4) n_exit = (uint32_t)warp_owner_cap(h, 7) + 1u;
   }
   cudaError_t e;
   if (variant_warp_owner(v)) {
     void* args[] = {&A, &B, &ctrl, &sink, &scan, &dp, &pa, &n_steps, &n_exit};
-    const void* fn = v == 6 ? (const void*)k_steps_warp<1, kWsSplit> : (const void*)k_steps_warp<2, kWsSplit>;
+    const void* fn = v == 6 ? (const void*)k_steps_warp<1> : (const void*)k_steps_warp<2>;
     // one CTA per 16 NP targets of the host's bound (the population only shrinks inside a launch), one CTA per SM at
     // most: a CTA that owns no target would only make the grid barrier slower
     const uint64_t per_cta = (uint64_t)(kTPB / 32) * 2u * (uint64_t)variant_npack(v);
     const unsigned grid = (unsigned)std::max<uint64_t>(1, std::min<uint64_t>((uint64_t)h->grid_field[v], (h->n_bound + per_cta - 1) / per_cta));
-    e = cudaLaunchCooperativeKernel(fn, dim3(grid), dim3(kTPB * kWsSplit), args, kWsSmemBytes, h->stream);
+    e = cudaLaunchCooperativeKernel(fn, dim3(grid), dim3(kTPB), args, kWsSmemBytes, h->stream);
   } else {
     void* args[] = {&A, &B, &ctrl, &Ep, &pc, &sink, &scan, &dp, &pa, &n_steps, &n_exit};
     const void* fn = v == 4 ? (const void*)k_steps<4, 1> : v == 3 ? (const void*)k_steps<2, 2> : (const void*)k_steps<1, 2>;
@@ -661,10 +658,10 @@ int gcoreccd_create(const gcoreccd_params* p, gcoreccd_t** out) {
   if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[3], k_steps<2, 2>, kTPB, 0);
   if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[4], k_steps<4, 1>, kTPB, 0);
   if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[5], k_steps<1, 2>, kTPB, 0);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_steps_warp<1, kWsSplit>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kWsSmemBytes);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_steps_warp<2, kWsSplit>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kWsSmemBytes);
-  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[6], k_steps_warp<1, kWsSplit>, kTPB * kWsSplit, kWsSmemBytes);
-  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[7], k_steps_warp<2, kWsSplit>, kTPB * kWsSplit, kWsSmemBytes);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_steps_warp<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kWsSmemBytes);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_steps_warp<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kWsSmemBytes);
+  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[6], k_steps_warp<1>, kTPB, kWsSmemBytes);
+  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[7], k_steps_warp<2>, kTPB, kWsSmemBytes);
   if (e != cudaSuccess) { fail(h, GCORECCD_ERR_CUDA, "occupancy query", e); gcoreccd_destroy(h); return GCORECCD_ERR_CUDA; }
   for (int v = 0; v < 3; ++v) h->grid_field[v] = h->num_sms * (occ[v] > 0 ? occ[v] : 1);
   int coop = 0;
@@ -672,7 +669,7 @@ int gcoreccd_create(const gcoreccd_params* p, gcoreccd_t** out) {
   for (int v = 3; v < 5; ++v) h->grid_field[v] = coop ? h->num_sms * std::min(occ[v], v == 3 ? 2 : 1) : 0;   // 0: no persistent path
   // < 3,072 holes: 96 tiles of 32 carriers at most; every CTA that only waits at the grid barriers makes them slower
   h->grid_field[5] = coop && occ[5] > 0 ? std::min(h->num_sms, 96) : 0;
-  for (int v = 6; v <= 7; ++v) h->grid_field[v] = coop && occ[v] > 0 ? h->num_sms : 0;   // one CTA per SM; 0: pick_variant never returns it
+  for (int v = 6; v <= 7; ++v) h->grid_field[v] = coop && occ[v] > 0 ? std::min(h->num_sms, kSegMaxCtas) : 0;   // one CTA per SM; 0: pick_variant never returns it
   int occ_tree = 0;
   e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_tree, k_tree_field, kTreeTPB, 0);
   if (e != cudaSuccess) { fail(h, GCORECCD_ERR_CUDA, "occupancy query", e); gcoreccd_destroy(h); return GCORECCD_ERR_CUDA; }
