@@ -10,14 +10,16 @@
 //     FP64, fixed order) finishes eq. 6 and the warp goes straight on to a2..a8 for its own targets: no chunk partials,
 //     no plan, no barrier between the field and the update — ONE grid barrier per step.  One CTA of 8 warps per SM,
 //     NP = 1 or 2 by population, and only as many CTAs as the population needs.
-//   * A CTA compacts its survivors only LOCALLY: CTA t owns slots [t T, (t + 1) T) of the state arrays (T = 16 NP), its
-//     cnt_t survivors sit at the front of that segment in stable order, and it stores cnt_t in a word of its own before
-//     it arrives at the barrier.  After the barrier every CTA reads all the words (one per thread, once): the
-//     population and the prefix of every segment — the scan costs one read instead of two rounds of polling.  (The first
+//   * A CTA keeps the carriers it was dealt at launch (T = 16 NP of them) and compacts its survivors LOCALLY; it writes
+//     them at (prefix of its segment in the state it read) + (rank among its survivors) and stores its survivor count
+//     in a word of its own before it arrives at the barrier.  After the barrier every CTA reads all the words (one per
+//     thread, once): the population and the prefix of every segment — the scan costs one read instead of two rounds
+//     of polling, and the state is dense again as soon as a step collects nobody.  (The first
 //     form of this kernel compacted globally with the two-level scan of gc_advance.cuh before the barrier: 6.3 / 13.8 us
 //     per step at 1,024 / 4,096 holes against 5.8 / 13.6 us.)
 //   * The concatenation of the segments IS the stable compacted order; sources are staged in that order (dense
-//     segments: index = slot; otherwise a binary search over the prefix table in shared memory), so every FP32 sum is
+//     state: index = slot; after a step that collected somebody a binary search over the prefix table in shared
+//     memory), so every FP32 sum is
 //     taken in the order a dense state would give: results do not depend on how a run is cut into launches.
 //   * A CTA's targets of the next step are its own survivors: they stay in shared memory, and their Box-Muller
 //     chains for the next step are drawn (one KIND of chain per warp: no divergence) while the other CTAs arrive.
@@ -52,7 +54,7 @@ k_steps_warp(SoA A, SoA B, Ctrl* ctrl, Sink sink, unsigned long long* status, De
   __shared__ double s_bm[5][T];                // Box-Muller chains Ra, sa, ca, Rb, cb of the CTA's carriers
   __shared__ float s_cx[T], s_cy[T], s_cz[T];  // the CTA's own carriers (front of its segment), this step's targets
   __shared__ uint32_t s_cid[T];
-  __shared__ uint32_t s_cnt[kSegMaxCtas], s_pre[kSegMaxCtas + 1], s_ct[kWsWarps];
+  __shared__ uint32_t s_cnt[kSegMaxCtas], s_pre[kSegMaxCtas + 1], s_start[kSegMaxCtas], s_ct[kWsWarps];
   __shared__ uint32_t s_w[16];
   __shared__ uint32_t s_n;
   __shared__ unsigned long long s_step;
@@ -63,7 +65,6 @@ k_steps_warp(SoA A, SoA B, Ctrl* ctrl, Sink sink, unsigned long long* status, De
   unsigned long long pairs = 0;                // sum of n^2 over the steps taken (identical in every CTA)
   uint32_t k = 0, arrivals = 0;
   uint32_t n_prev = 0, cnt_own = 0;            // the previous step's population; this CTA's carriers after its last commit
-  bool dense = true;                           // slot = compacted index (table of the step before, until the new one is in)
 
   // Box-Muller chains of the CTA's `cnt` carriers (ids in s_cid) for step `for_step`: one KIND of chain per warp
   auto draw_chains = [&](uint32_t cnt, uint64_t for_step) {
@@ -100,15 +101,10 @@ k_steps_warp(SoA A, SoA B, Ctrl* ctrl, Sink sink, unsigned long long* status, De
       // were slower — the words' lines thrash)
       if (tid < G) c_mine = (uint32_t)ld_relaxed_u64(status + ((k - 1u) & 1u) * kSegWordStride + tid);
     }
-    // compacted index j -> slot of the segmented state, from the prefix table in shared memory
-    auto slot_of = [&](uint32_t j, bool dense_now) -> uint32_t {
-      if (dense_now) return j;
-      uint32_t lo = 0, hi = G;
-      while (hi - lo > 1u) { const uint32_t mid = (lo + hi) >> 1; if (s_pre[mid] <= j) lo = mid; else hi = mid; }
-      return lo * T + (j - s_pre[lo]);
-    };
-    // The first source tile is requested at once, with the PREVIOUS step's table (still in shared memory), so that its
-    // L2 round trip overlaps the table's: in most steps nobody is collected and the table has not changed.
+    // Where segment t of `cur` begins: where its owner wrote it, i.e. at the prefix the owner knew THEN (state k - 1's).
+    const uint32_t old_pre_mine = (k > 0 && tid < G) ? s_pre[tid] : 0u;
+    // The first source tile is requested at once, as if nobody had been collected in the step before (then `cur` is
+    // dense and as long as it was), so that its L2 round trip overlaps the count words': the usual case.
     float px[kPre], py[kPre], pz[kPre];
     const bool spec = k > 0 && cnt_own > 0;
     if (spec) {
@@ -116,8 +112,7 @@ k_steps_warp(SoA A, SoA B, Ctrl* ctrl, Sink sink, unsigned long long* status, De
       for (int u = 0; u < kPre; ++u) {
         const uint32_t j = (uint32_t)u * kTPB + tid;
         const bool ok = j < n_prev;
-        const uint32_t a = ok ? slot_of(j, dense) : 0u;
-        px[u] = ok ? __ldcg(cur.x + a) : kSentinel; py[u] = ok ? __ldcg(cur.y + a) : kSentinel; pz[u] = ok ? __ldcg(cur.z + a) : kSentinel;
+        px[u] = ok ? __ldcg(cur.x + j) : kSentinel; py[u] = ok ? __ldcg(cur.y + j) : kSentinel; pz[u] = ok ? __ldcg(cur.z + j) : kSentinel;
       }
     }
     GC_T(0);
@@ -126,28 +121,36 @@ k_steps_warp(SoA A, SoA B, Ctrl* ctrl, Sink sink, unsigned long long* status, De
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) { const uint32_t v = __shfl_up_sync(kFull, inc, o); if ((int)lane >= o) inc += v; }
     if (lane == 31u) s_ct[warp] = inc;
-    if (tid < G) s_cnt[tid] = c_mine;
-    __syncthreads();                                         // (every speculative address above is computed: s_pre may change)
+    __syncthreads();
     uint32_t base = 0, n = 0;
 #pragma unroll
     for (int w = 0; w < kWsWarps; ++w) { const uint32_t c = s_ct[w]; if ((uint32_t)w < warp) base += c; n += c; }
     const uint32_t pre_mine = base + inc - c_mine;
-    if (tid < G) s_pre[tid] = pre_mine;
+    if (tid < G) { s_cnt[tid] = c_mine; s_pre[tid] = pre_mine; s_start[tid] = k > 0 ? old_pre_mine : pre_mine; }
     if (tid == 0) { s_pre[G] = n; s_n = n; }
-    // dense (slot = compacted index) iff every segment in front of the last carrier is full
-    dense = __syncthreads_and(tid >= G || pre_mine == min(n, tid * T)) != 0;
+    __syncthreads();
     GC_T(1);
+    // `cur` is dense (slot = compacted index) iff nobody was collected in the step that wrote it: every survivor went to
+    // (prefix of its segment) + (rank in its segment), and those prefixes are still the right ones
+    const bool dense = k == 0 || n == n_prev;
     if (k == n_steps || n == 0 || n < n_exit) break;         // uniform over the grid; n_exit: a smaller variant takes over
     const uint64_t step = s_step + k;
     const uint32_t cnt = s_cnt[b];                           // this CTA's carriers
     const bool cta_active = cnt > 0;
     pairs += (unsigned long long)n * (unsigned long long)n;
-    if (!(spec && n == n_prev)) {                            // somebody was collected (or first step): stage with the new table
+    // compacted index j -> slot of `cur`: a binary search over the prefix table when the step before collected somebody
+    auto slot_of = [&](uint32_t j) -> uint32_t {
+      if (dense) return j;
+      uint32_t lo = 0, hi = G;
+      while (hi - lo > 1u) { const uint32_t mid = (lo + hi) >> 1; if (s_pre[mid] <= j) lo = mid; else hi = mid; }
+      return s_start[lo] + (j - s_pre[lo]);
+    };
+    if (!(spec && dense)) {                                  // somebody was collected (or first step): stage with the table
 #pragma unroll
       for (int u = 0; u < kPre; ++u) {
         const uint32_t j = (uint32_t)u * kTPB + tid;
         const bool ok = cta_active && j < n;
-        const uint32_t a = ok ? slot_of(j, dense) : 0u;
+        const uint32_t a = ok ? slot_of(j) : 0u;
         px[u] = ok ? __ldcg(cur.x + a) : kSentinel; py[u] = ok ? __ldcg(cur.y + a) : kSentinel; pz[u] = ok ? __ldcg(cur.z + a) : kSentinel;
       }
     }
@@ -184,7 +187,7 @@ k_steps_warp(SoA A, SoA B, Ctrl* ctrl, Sink sink, unsigned long long* status, De
         for (int u = 0; u < kPre; ++u) {
           const uint32_t j = j0 + kWsTile + (uint32_t)u * kTPB + tid;
           const bool ok = j < n;
-          const uint32_t a = ok ? slot_of(j, dense) : 0u;
+          const uint32_t a = ok ? slot_of(j) : 0u;
           px[u] = ok ? __ldcg(cur.x + a) : kSentinel; py[u] = ok ? __ldcg(cur.y + a) : kSentinel; pz[u] = ok ? __ldcg(cur.z + a) : kSentinel;
         }
       }
@@ -254,7 +257,7 @@ k_steps_warp(SoA A, SoA B, Ctrl* ctrl, Sink sink, unsigned long long* status, De
       uint32_t r = rank_in_warp;
       for (uint32_t w = 0; w < warp; ++w) r += s_w[w];
       s_cx[r] = xf; s_cy[r] = yf; s_cz[r] = zf; s_cid[r] = id;
-      const uint32_t a = b * T + r;
+      const uint32_t a = s_pre[b] + r;                       // this state's prefix: dense again if nobody is collected
       nxt.x[a] = xf; nxt.y[a] = yf; nxt.z[a] = zf;           // (ids travel with the owner; sources need coordinates only)
     }
     if (tid == 0) {
