@@ -18,8 +18,8 @@
 //     form of this kernel compacted globally with the two-level scan of gc_advance.cuh before the barrier: 6.3 / 13.8 us
 //     per step at 1,024 / 4,096 holes against 5.8 / 13.6 us.)
 //   * The concatenation of the segments IS the stable compacted order; sources are staged in that order (dense
-//     state: index = slot; after a step that collected somebody a binary search over the prefix table in shared
-//     memory), so every FP32 sum is
+//     state: index = slot; after a step that collected somebody through a map laid out in shared memory), so every
+//     FP32 sum is
 //     taken in the order a dense state would give: results do not depend on how a run is cut into launches.
 //   * A CTA's targets of the next step are its own survivors: they stay in shared memory, and their Box-Muller
 //     chains for the next step are drawn (one KIND of chain per warp: no divergence) while the other CTAs arrive.
@@ -55,6 +55,7 @@ k_steps_warp(SoA A, SoA B, Ctrl* ctrl, Sink sink, unsigned long long* status, De
   __shared__ float s_cx[T], s_cy[T], s_cz[T];  // the CTA's own carriers (front of its segment), this step's targets
   __shared__ uint32_t s_cid[T];
   __shared__ uint32_t s_cnt[kSegMaxCtas], s_pre[kSegMaxCtas + 1], s_start[kSegMaxCtas], s_ct[kWsWarps];
+  __shared__ unsigned short s_inv[kSegMaxCtas * 32];   // compacted index -> slot, when the state is not dense
   __shared__ uint32_t s_w[16];
   __shared__ uint32_t s_n;
   __shared__ unsigned long long s_step;
@@ -138,13 +139,23 @@ k_steps_warp(SoA A, SoA B, Ctrl* ctrl, Sink sink, unsigned long long* status, De
     const uint32_t cnt = s_cnt[b];                           // this CTA's carriers
     const bool cta_active = cnt > 0;
     pairs += (unsigned long long)n * (unsigned long long)n;
-    // compacted index j -> slot of `cur`: a binary search over the prefix table when the step before collected somebody
-    auto slot_of = [&](uint32_t j) -> uint32_t {
-      if (dense) return j;
-      uint32_t lo = 0, hi = G;
-      while (hi - lo > 1u) { const uint32_t mid = (lo + hi) >> 1; if (s_pre[mid] <= j) lo = mid; else hi = mid; }
-      return s_start[lo] + (j - s_pre[lo]);
-    };
+    // compacted index j -> slot of `cur`.  After a step that collected somebody the segments do not abut: a map is laid
+    // out in shared memory, one warp per segment at a time (a binary search per source over the prefix table was tried
+    // first: 5,700 cycles per 2,048-source tile; this is ~600 per step)
+    if (!dense && cta_active) {
+      for (uint32_t t0 = warp; t0 < G; t0 += 5u * (uint32_t)kWsWarps) {     // five segments' table entries in flight
+        uint32_t c[5], q[5], a[5];
+#pragma unroll
+        for (int u = 0; u < 5; ++u) {
+          const uint32_t t = min(t0 + (uint32_t)u * (uint32_t)kWsWarps, G - 1u);
+          c[u] = t0 + (uint32_t)u * (uint32_t)kWsWarps < G ? s_cnt[t] : 0u; q[u] = s_pre[t]; a[u] = s_start[t];
+        }
+#pragma unroll
+        for (int u = 0; u < 5; ++u) if (lane < c[u]) s_inv[q[u] + lane] = (unsigned short)(a[u] + lane);
+      }
+      __syncthreads();
+    }
+    auto slot_of = [&](uint32_t j) -> uint32_t { return dense ? j : (uint32_t)s_inv[j]; };
     if (!(spec && dense)) {                                  // somebody was collected (or first step): stage with the table
 #pragma unroll
       for (int u = 0; u < kPre; ++u) {
