@@ -116,6 +116,30 @@ def test_trajectory_parity_10_steps_warp_owner_kernels(cfg, n):
     _trajectory_check(workloads.make(cfg, n=n), 0, 0, persist=1)
 
 
+def test_carriers_appended_between_launches_cross_the_kernel_variants():
+    """load_carriers appends (ids continue, include/gcoreccd.h): 2,000 holes step in the warp-owner kernel (NP = 1),
+    2,500 more take the population into NP = 2, another 1,500 into the CTA-tile kernel; each hand-over re-plans from
+    the device-resident state.  Same sequence on the oracle, same R21 comparison."""
+    w = workloads.make(2, n=6000)                          # sigma = 2 um: sparse enough for strict R21
+    xyz = w["xyz"]
+    sim = gpu_sim(w)
+    o = oracle_sim(w, flags=g.FP32_STATE)
+    history = []
+    for lo, hi, steps in ((0, 2000, 4), (2000, 4500, 3), (4500, 6000, 3)):
+        sim.load_carriers(xyz[lo:hi])
+        o.load(xyz[lo:hi])
+        sim.step(steps)
+        for _ in range(steps):
+            history.append(o.carriers())
+            o.step(1)
+    (gx, gi), (ox, oi) = sim.read_carriers(), o.carriers()
+    st, ost = sim.state(), o.state()
+    assert st["step"] == ost["step"] == 10 and st["n_loaded"] == 6000
+    assert st["pair_interactions"] == ost["pair_interactions"]
+    traj_assert(gx, gi, ox, oi, history, 6000, TRAJ_TOL)
+    sim.close()
+
+
 def test_trajectory_parity_flag_combinations():
     from paper_2203_11043_b200 import binding as b
     w = workloads.make(0, n=600)
