@@ -4,7 +4,8 @@
     python tests/golden/make_full_run_goldens.py 2      # cfg2, 131,072 holes: ~1e13 pairs, 3 h on 8 cores / 31 min on 16 fast ones
     python tests/golden/make_full_run_goldens.py 3      # cfg3, 262,144-hole track: 1.1e13 pairs
     python tests/golden/make_full_run_goldens.py 4 131072   # cfg4's mix of 4 tracks + 64 clouds at 1/8 of its holes
-                                                            # (full_run_cfg4_n131072.txt; full size is 1.8e14 pairs)
+    python tests/golden/make_full_run_goldens.py 4 524288   # ... at 1/2: 4.4e13 pairs, 2.3 h on 16 fast cores
+                                                            # (full_run_cfg4_n<N>.txt; full size is 1.8e14 pairs)
 
 Imports only oracle/ and the seeded input generator (workloads.py, which holds none of the method's
 arithmetic); nothing here ever touches the CUDA path, so every stored value is the oracle's.
@@ -35,6 +36,7 @@ import workloads                      # noqa: E402  (seeded inputs only)
 from oracle import goracle as g       # noqa: E402
 
 EVERY = 25
+SUB = 5
 
 
 def run(cfg, n=None, out=None, log=sys.stderr):
@@ -80,9 +82,11 @@ def run(cfg, n=None, out=None, log=sys.stderr):
     t0 = time.time()
     last_save = t0
     while sim.state()["n_active"] > 0:
-        sim.step(EVERY)
+        # (in sub-chunks, so that a checkpoint can be taken between the recorded decay points of a slow run)
+        sim.step(min(SUB, EVERY - sim.state()["step"] % EVERY))
         st = sim.state()
-        decay.append((st["step"], st["n_active"]))
+        if st["step"] % EVERY == 0 or st["n_active"] == 0:
+            decay.append((st["step"], st["n_active"]))
         print("cfg%d step %d n_active %d pairs %.4g  %.0f s" % (cfg, st["step"], st["n_active"],
                                                                base["pairs"] + st["pair_interactions"],
                                                                base["wall"] + time.time() - t0),
