@@ -43,7 +43,7 @@ def _parse_full_run(name):
     return G
 
 
-@pytest.mark.parametrize("cfg,n", [(1, None), (2, None), (3, None), (4, 131072)])
+@pytest.mark.parametrize("cfg,n", [(1, None), (2, None), (3, None), (4, 131072), (4, 524288)])
 def test_whole_event_against_the_oracle_full_run(cfg, n):
     name = "full_run_cfg%d%s.txt" % (cfg, "" if n is None else "_n%d" % n)
     if not os.path.exists(os.path.join(GOLDEN, name)):
