@@ -309,6 +309,31 @@ int gcoreccd_mobility_table_host(double T_K, const double* E_host, uint64_t n, d
  * DESIGN.md 6.1 / 6.8 (`python bench.py --microbench`); not on the hot path. */
 int gcoreccd_debug_microbench(int kind, uint32_t iters, uint32_t warps_per_subpartition, double* cycles_per_inst_host);
 
+/* ---- Allocation-free entry point ---------------------------------------------------------------------------------
+ * Some callers cannot call cudaMalloc: code under CUDA-graph capture, tight serving loops, harnesses that forbid it.
+ * gcoreccd_field_noalloc evaluates the Coulomb field of eq. 6 (the operation of gcoreccd_eval_field) for
+ * n <= GCORECCD_NOALLOC_MAX_CARRIERS holes WITHOUT a handle and without allocating anything: no cudaMalloc, cudaFree or
+ * allocating library routine is called, here or at set-up.  Its scratch (positions as structure of arrays, the work
+ * plan, the partial-sum planes: 6,488,320 bytes) is a file-scope `static __device__` array inside the library, which
+ * every GPU that loads the library therefore holds until the process exits.
+ *   xyz_um_dev  DEVICE pointer, n interleaved (x, y, z) in um, FP32 (layout of gcoreccd_load_carriers); caller-owned,
+ *               read only; not validated (a non-finite coordinate gives non-finite fields)
+ *   softening_um, eps_si   as in gcoreccd_params (eps_si = 0 -> 11.7; softening 0 evaluates eq. 5, R5)
+ *   Exyz_dev    DEVICE pointer, receives n interleaved (Ex, Ey, Ez) in V/cm, same order as the input; caller-owned
+ *   stream      cudaStream_t the four kernels are enqueued on (NULL = default stream); the call does NOT synchronise
+ * Runs on the CURRENT device (sm_100 required: GCORECCD_ERR_CUDA otherwise, no fallback).  The first call on a device
+ * looks the array's address up (cudaGetSymbolAddress); nothing else is kept between calls.
+ * Returns GCORECCD_ERR_CAPACITY for n > GCORECCD_NOALLOC_MAX_CARRIERS, GCORECCD_ERR_INVALID for null pointers or a
+ * negative / non-finite parameter; n = 0 is a no-op.  gcoreccd_field_noalloc_error() gives the detail of the calling
+ * thread's last failure ("" if none).
+ * ALL calls share the one array, on every stream and from every thread: two calls whose kernels overlap on the GPU
+ * race on it (undefined results).  Keep them on one stream, or order them with events.  The array keeps the last call's
+ * contents; each call re-initialises what it reads. */
+#define GCORECCD_NOALLOC_MAX_CARRIERS 16384u
+int gcoreccd_field_noalloc(const float* xyz_um_dev, uint64_t n, double softening_um, double eps_si, float* Exyz_dev,
+                           void* stream);
+const char* gcoreccd_field_noalloc_error(void);
+
 const char* gcoreccd_strerror(int code);
 const char* gcoreccd_last_error(gcoreccd_t* h);   /* detail of the last failure on this handle ("" if none) */
 const char* gcoreccd_version(void);

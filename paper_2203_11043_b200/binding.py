@@ -25,6 +25,7 @@ EXPORTS = ["gcoreccd_workspace_size", "gcoreccd_create", "gcoreccd_destroy", "gc
            "gcoreccd_set_farfield", "gcoreccd_farfield_stats",
            "gcoreccd_set_shard", "gcoreccd_shard_message_bytes", "gcoreccd_shard_local", "gcoreccd_shard_commit", "gcoreccd_set_shard_wait",
            "gcoreccd_profile_step", "gcoreccd_set_persistent", "gcoreccd_kernel_launches", "gcoreccd_debug_normals", "gcoreccd_debug_mobility", "gcoreccd_mobility_table_host", "gcoreccd_debug_microbench", "gcoreccd_strerror",
+           "gcoreccd_field_noalloc", "gcoreccd_field_noalloc_error",
            "gcoreccd_last_error", "gcoreccd_version"]
 
 
@@ -135,6 +136,10 @@ def lib():
     L.gcoreccd_mobility_table_host.argtypes = [C.c_double, C.POINTER(C.c_double), C.c_uint64, C.POINTER(C.c_double)]
     L.gcoreccd_debug_microbench.restype = C.c_int
     L.gcoreccd_debug_microbench.argtypes = [C.c_int, C.c_uint32, C.c_uint32, C.POINTER(C.c_double)]
+    L.gcoreccd_field_noalloc.restype = C.c_int
+    L.gcoreccd_field_noalloc.argtypes = [vp, C.c_uint64, C.c_double, C.c_double, vp, vp]
+    L.gcoreccd_field_noalloc_error.restype = C.c_char_p
+    L.gcoreccd_field_noalloc_error.argtypes = []
     L.gcoreccd_strerror.restype = C.c_char_p
     L.gcoreccd_strerror.argtypes = [C.c_int]
     L.gcoreccd_last_error.restype = C.c_char_p
@@ -155,6 +160,19 @@ def version():
 
 def xray_hole_count(E_e_eV, w_eV=3.77):
     return int(lib().gcoreccd_xray_hole_count(float(E_e_eV), float(w_eV)))
+
+
+NOALLOC_MAX_CARRIERS = 16384
+
+
+def field_noalloc(xyz_dev_ptr, n, softening_um, eps_si, out_dev_ptr, stream_handle=0):
+    """include/gcoreccd.h gcoreccd_field_noalloc: eq. 6 for n <= NOALLOC_MAX_CARRIERS holes with no handle and no device
+    allocation.  Device pointers (ints) in and out, enqueued on `stream_handle` (a cudaStream_t as int), not synchronised.
+    All calls share one static scratch array: keep them on one stream."""
+    rc = lib().gcoreccd_field_noalloc(C.c_void_p(int(xyz_dev_ptr)), int(n), float(softening_um), float(eps_si),
+                                      C.c_void_p(int(out_dev_ptr)), C.c_void_p(int(stream_handle)))
+    if rc != OK:
+        raise GcoreccdError(rc, "gcoreccd_field_noalloc", lib().gcoreccd_field_noalloc_error().decode())
 
 
 MICRO_KINDS = ["FFMA2 three distinct operands", "FFMA2 a*a+c", "FFMA2 shared operand", "FADD2", "FMUL2",

@@ -4,6 +4,8 @@
 #include "../../include/gcoreccd.h"
 
 #include <cmath>
+#include <cstdarg>
+#include <mutex>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -22,6 +24,7 @@
 #include "gc_integrate.cuh"
 #include "gc_microbench.cuh"
 #include "gc_persist_warp.cuh"
+#include "gc_noalloc.cuh"
 #include "gc_persist.cuh"
 #include "gc_shard.cuh"
 #include "gc_tree.cuh"
@@ -1599,6 +1602,104 @@ int gcoreccd_debug_gtimes(unsigned long long* out) {
   return cudaMemcpyFromSymbol(out, gc::g_gt, sizeof(gc::g_gt)) == cudaSuccess ? 0 : -5;
 }
 #endif
+
+// ---- allocation-free field evaluation (gc_noalloc.cuh) -----------------------------------------------------------
+}  // extern "C"
+
+// The scratch of gcoreccd_field_noalloc: a file-scope device array, part of the library's image on every GPU that loads
+// it (6.2 MiB until the process exits).  In host code this name is only a stand-in for the symbol: the device address
+// comes from cudaGetSymbolAddress, once per device, below.
+static __device__ __align__(256) unsigned char g_na_scratch[gc::NaLayout::bytes];
+
+namespace {
+struct NaDevice { bool ready; unsigned char* base; int sms; };
+NaDevice g_na_dev[64];
+std::mutex g_na_mu;
+thread_local char g_na_err[256] = "";
+
+int na_fail(int code, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_na_err, sizeof(g_na_err), fmt, ap);
+  va_end(ap);
+  return code;
+}
+
+// once per device, with that device current: the array's address ON THIS DEVICE, and the SM count for the grids
+int na_setup(int dev, NaDevice** out) {
+  if (dev < 0 || dev >= 64) return na_fail(GCORECCD_ERR_CUDA, "field_noalloc: device ordinal %d out of range", dev);
+  std::lock_guard<std::mutex> lock(g_na_mu);
+  NaDevice& D = g_na_dev[dev];
+  if (!D.ready) {
+    int major = 0, sms = 0;
+    cudaError_t e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return na_fail(GCORECCD_ERR_CUDA, "field_noalloc: cudaDeviceGetAttribute: %s", cudaGetErrorString(e));
+    if (major != 10) return na_fail(GCORECCD_ERR_CUDA, "field_noalloc: device %d is not sm_100 (no fallback)", dev);
+    void* ptr = nullptr;
+    e = cudaGetSymbolAddress(&ptr, g_na_scratch);
+    if (e != cudaSuccess || !ptr) return na_fail(GCORECCD_ERR_CUDA, "field_noalloc: cudaGetSymbolAddress: %s", cudaGetErrorString(e));
+    D.base = (unsigned char*)ptr;
+    D.sms = sms;
+    D.ready = true;
+  }
+  *out = &D;
+  return GCORECCD_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int gcoreccd_field_noalloc(const float* xyz_um_dev, uint64_t n, double softening_um, double eps_si, float* Exyz_dev,
+                           void* stream) {
+  g_na_err[0] = 0;
+  if (n > GCORECCD_NOALLOC_MAX_CARRIERS)
+    return na_fail(GCORECCD_ERR_CAPACITY, "field_noalloc: n = %llu exceeds GCORECCD_NOALLOC_MAX_CARRIERS = %u (fixed scratch)",
+                   (unsigned long long)n, (unsigned)GCORECCD_NOALLOC_MAX_CARRIERS);
+  if (n == 0) return GCORECCD_OK;
+  if (!xyz_um_dev || !Exyz_dev) return na_fail(GCORECCD_ERR_INVALID, "field_noalloc: null input or output pointer");
+  if (!(softening_um >= 0.0) || !(eps_si >= 0.0) || !std::isfinite(softening_um) || !std::isfinite(eps_si))
+    return na_fail(GCORECCD_ERR_INVALID, "field_noalloc: softening and eps_si must be finite and >= 0");
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return na_fail(GCORECCD_ERR_CUDA, "field_noalloc: cudaGetDevice: %s", cudaGetErrorString(e));
+  NaDevice* D = nullptr;
+  int rc = na_setup(dev, &D);
+  if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  Ctrl* ctrl = (Ctrl*)(D->base + NaLayout::ctrl);
+  float* x = (float*)(D->base + NaLayout::x);
+  float* y = (float*)(D->base + NaLayout::y);
+  float* z = (float*)(D->base + NaLayout::z);
+  float* Ep = (float*)(D->base + NaLayout::ep);
+  // same constants as gcoreccd_create (K' = q / (4 pi eps0 eps_Si) in (V/cm) um^2; R5: eps^2 >= 1e-24)
+  const double q = 1.602176634e-19, eps0 = 8.8541878128e-12, pi = 3.14159265358979323846;
+  const double Kp = q / (4.0 * pi * eps0 * (eps_si > 0.0 ? eps_si : 11.7)) * 1e10;
+  const double e2 = softening_um * softening_um;
+  const float eps2 = (float)(e2 < 1e-24 ? 1e-24 : e2);
+  // field variant by size, as the handle's two-launch path picks it (pick_variant)
+  const int npack = n >= 12288 ? 4 : n >= 3072 ? 2 : 1;
+  const int per_sm = npack == 4 ? 1 : npack == 2 ? 3 : 4;
+  PlanArgs pa;
+  pa.IB = (uint32_t)kTPB * 2u * (uint32_t)npack;
+  pa.grid = (uint32_t)(D->sms * per_sm);
+  pa.part_cap_entries = kNaPartCap;
+  pa.rank = 0; pa.world = 1; pa.force_S = 0;
+  const uint32_t tiles = (uint32_t)((n + kTPB - 1) / kTPB);
+  k_na_prepare<<<1, 32, 0, st>>>(ctrl, (uint32_t)n, pa);
+  k_na_unpack<<<tiles, kTPB, 0, st>>>(xyz_um_dev, (uint32_t)n, x, y, z);
+  switch (npack) {
+    case 1: k_field<1, 256, 4><<<pa.grid, kTPB, 0, st>>>(x, y, z, ctrl, Ep, kNaPartCap, eps2); break;
+    case 2: k_field<2, 256, 3><<<pa.grid, kTPB, 0, st>>>(x, y, z, ctrl, Ep, kNaPartCap, eps2); break;
+    default: k_field<4, 256, 1><<<pa.grid, kTPB, 0, st>>>(x, y, z, ctrl, Ep, kNaPartCap, eps2); break;
+  }
+  k_field_finalize<<<tiles, kTPB, 0, st>>>(ctrl, Ep, kNaPartCap, Kp, Exyz_dev);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return na_fail(GCORECCD_ERR_CUDA, "field_noalloc: kernel launch: %s", cudaGetErrorString(e));
+  return GCORECCD_OK;
+}
+
+const char* gcoreccd_field_noalloc_error(void) { return g_na_err; }
 
 const char* gcoreccd_strerror(int code) {
   switch (code) {
